@@ -1,0 +1,125 @@
+/* sparse_sv.h -- C ABI of the B200-native sparse, truncated state-vector gate engine.
+ *
+ * Method: arxiv/paper_2607_07816 "A Sparse and Truncated State Vector Simulator for
+ * Peaked Circuits".  A state is stored only as its nonzero terms, each a
+ * (uint64 basis index, complex128 amplitude) pair.  All state
+ * arrays live in device memory for the whole simulation; only results cross to the
+ * host.
+ *
+ * Conventions:
+ *   - qubit q is bit q of the 64-bit key (LSB = qubit 0), 1 <= n_qubits <= 64;
+ *   - a gate matrix U is HOST memory, row-major 2^m x 2^m, U[r * 2^m + c]; bit j of the
+ *     local index r / c is the key's bit qubits[j]; 1 <= m <= 4;
+ *   - "probability" p = re*re + im*im in fp64; the total order used for truncation and
+ *     readout is (p descending, key ascending).
+ *
+ * Every pointer below is a HOST pointer unless it says DEVICE.  The handle owns all
+ * device memory it allocates; caller buffers are only read or written during the call
+ * and never freed.  No C++ exception crosses this boundary.  Return value: SV_OK or a
+ * negative error; on any error the logical state is unchanged (gates are applied out of
+ * place and committed by swapping buffers).  Work is enqueued on the state's CUDA
+ * stream; calls that return a value to the host synchronise that stream.
+ */
+#ifndef SPARSE_SV_H
+#define SPARSE_SV_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sv_state sv_state;              /* opaque */
+typedef struct { double re, im; } sv_c128;     /* = C99 double _Complex layout */
+
+enum {
+    SV_OK = 0,
+    SV_ERR_INVALID_ARG = -1,
+    SV_ERR_CAPACITY = -2,  /* a gate's output (before truncation) would exceed `capacity` */
+    SV_ERR_NOMEM = -3,
+    SV_ERR_CUDA = -4
+};
+
+/* gate classes reported by sv_get_stats */
+enum { SV_CLASS_NONE = 0, SV_CLASS_DIAGONAL = 1, SV_CLASS_XOR = 2, SV_CLASS_GROUP = 3 };
+
+typedef struct {
+    int      gate_class;   /* SV_CLASS_* of the last sv_apply_gate                          */
+    int      m;            /* its number of qubits                                          */
+    int      active_bits;  /* qubits on which U is not block diagonal (0 for diagonal)      */
+    int      passes;       /* full passes over the state the call made                      */
+    uint64_t n_in;         /* terms before the last call                                    */
+    uint64_t n_out;        /* terms after it (N_pre for a gate, N_kept for a truncate)      */
+    uint64_t launches;     /* kernels launched by this handle since creation                */
+} sv_stats;
+
+/* Bytes of device memory a state of this capacity needs (for sv_create_in_arena). */
+size_t sv_arena_bytes(uint64_t capacity);
+
+/* New state |0...0>: one term, key 0, amplitude 1+0i.  `capacity` is the
+ * largest number of terms that may exist at any instant, including a gate's output
+ * before truncation.  Allocates with cudaMalloc on the current device, uses its own
+ * stream. */
+int sv_create(int n_qubits, uint64_t capacity, sv_state **out);
+
+/* Same, inside caller-owned DEVICE memory (e.g. a torch uint8 tensor) of at least
+ * sv_arena_bytes(capacity) bytes, 256-byte aligned, on `cuda_stream` (a cudaStream_t;
+ * NULL = the legacy default stream).  The arena must outlive the handle. */
+int sv_create_in_arena(int n_qubits, uint64_t capacity, void *dev_arena, size_t arena_bytes,
+                       void *cuda_stream, sv_state **out);
+
+void sv_destroy(sv_state *s);
+
+/* Apply the m-qubit gate U to `qubits` (distinct, each < n_qubits): every tuple of 2^m
+ * amplitudes whose basis states differ only in those qubits is multiplied by U, the
+ * contributions to one basis state are summed in ascending local column index with
+ * separately rounded multiplies and adds, and results that are exactly 0+0i are dropped
+ * (PAPER.md:47, :110-120).  U is not checked for unitarity.  Asynchronous except for a
+ * term-count read-back when the gate can change the number of terms. */
+int sv_apply_gate(sv_state *s, const int *qubits, int m, const sv_c128 *U);
+
+/* Truncate: keep the smallest prefix, in (p desc, key asc)
+ * order, whose mass is >= min_mass * (current total mass); then at most max_terms of it;
+ * then multiply the kept amplitudes by 1/sqrt(kept mass).  max_terms == 0: no cap.
+ * min_mass >= 1: no mass threshold; min_mass <= 0 or NaN: SV_ERR_INVALID_ARG.  At least
+ * one term is kept.  If nothing is dropped the state is left bitwise untouched.
+ * *kept_fraction (nullable) receives kept mass / total mass. */
+int sv_truncate(sv_state *s, uint64_t max_terms, double min_mass, double *kept_fraction);
+
+/* *mass = sum of |a|^2 over all terms (Eq. 4) -- the mass, not its root. */
+int sv_norm(sv_state *s, double *mass);
+
+/* The min(k, count) most probable terms, sorted by (p desc, key asc) (PAPER.md:61,
+ * :132-134).  keys / amps / probs are caller-owned host arrays of k entries; any may be
+ * NULL.  *n_written (nullable) receives the number of records written. */
+int sv_top(sv_state *s, uint64_t k, uint64_t *keys, sv_c128 *amps, double *probs,
+           uint64_t *n_written);
+
+/* Current number of stored terms. */
+int sv_num_terms(sv_state *s, uint64_t *n);
+
+/* Replace the state by n host terms (test / checkpoint hook).  Keys must be distinct
+ * and < 2^n_qubits, amplitudes nonzero, n <= capacity; else SV_ERR_INVALID_ARG. */
+int sv_load(sv_state *s, const uint64_t *keys, const sv_c128 *amps, uint64_t n);
+
+/* Same with DEVICE source arrays (no host copy; used to time device-resident input). */
+int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amps, uint64_t n);
+
+/* Statistics of the last call and the launch counter. */
+int sv_get_stats(sv_state *s, sv_stats *out);
+
+/* Device-side structural check (tests): keys strictly ascending in the engine's storage
+ * order, all below 2^n_qubits, no stored exact zero.  *ok = 1 if all hold. */
+int sv_check_invariants(sv_state *s, int *ok);
+
+/* Last error message of this handle ("" if none); valid until the next call on it. */
+const char *sv_last_error(const sv_state *s);
+
+/* Block until all work enqueued on the state's stream has finished. */
+int sv_sync(sv_state *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARSE_SV_H */

@@ -1,0 +1,526 @@
+// Host side of the C ABI (include/sparse_sv.h): state, gate classification (SURVEY.md row
+// a-1), pass planning, truncation driver, readout and load.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/sparse_sv.h"
+#include "sv_internal.h"
+
+struct sv_state {
+    int n;
+    u64 cap;
+    cudaStream_t stream;
+    bool own_mem, own_stream;
+    unsigned char* arena;
+    u64* keys[2];
+    double2* amps[2];
+    int cur;
+    u64 count;
+    // physical layout: stored bit phys_of_log[q] holds logical qubit q (XOR the lazy X mask)
+    int phys_of_log[64];
+    u64 xmask;   // in physical positions
+    // device scratch
+    TileDesc* desc;
+    u64* status;
+    u64* hist;
+    SelState* sel;
+    GateTab* tab;
+    u64* d_count;
+    u32* tile_counter;
+    int* d_bad;
+    double* partials;
+    double* d_norm;
+    unsigned char* pinned;   // host, for small read-backs
+    sv_stats stats;
+    char err[256];
+};
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
+
+struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, total; };
+static ArenaLayout layout_for(u64 cap) {
+    ArenaLayout L; size_t o = 0;
+    for (int i = 0; i < 2; ++i) { L.keys[i] = o; o += align_up(cap * 8); }
+    for (int i = 0; i < 2; ++i) { L.amps[i] = o; o += align_up(cap * 16); }
+    L.desc = o; o += align_up(desc_entries(cap) * sizeof(TileDesc));
+    L.status = o; o += align_up(desc_entries(cap) * 8);
+    L.hist = o; o += align_up(3 * SV_SEL_BINS * 8);
+    L.sel = o; o += align_up(sizeof(SelState));
+    L.tab = o; o += align_up(sizeof(GateTab));
+    L.misc = o; o += 256;
+    L.partials = o; o += align_up(1024 * 8 + 8);
+    L.total = o;
+    return L;
+}
+
+static int fail(sv_state* s, int code, const char* msg) {
+    if (s) snprintf(s->err, sizeof(s->err), "%s", msg);
+    return code;
+}
+static int cuda_fail(sv_state* s, cudaError_t e, const char* where) {
+    if (s) snprintf(s->err, sizeof(s->err), "%s: %s", where, cudaGetErrorString(e));
+    return SV_ERR_CUDA;
+}
+#define CU(call)                                                           \
+    do {                                                                   \
+        cudaError_t e__ = (call);                                          \
+        if (e__ != cudaSuccess) return cuda_fail(s, e__, #call);           \
+    } while (0)
+#define CHECK_LAUNCH()                                                     \
+    do {                                                                   \
+        cudaError_t e__ = cudaGetLastError();                              \
+        if (e__ != cudaSuccess) return cuda_fail(s, e__, "kernel launch"); \
+    } while (0)
+
+static KeyMap keymap_of(const sv_state* s) {
+    KeyMap km;
+    memset(km.log_of_phys, 0xff, sizeof(km.log_of_phys));
+    for (int q = 0; q < s->n; ++q) km.log_of_phys[s->phys_of_log[q]] = (unsigned char)q;
+    km.xmask = s->xmask;
+    return km;
+}
+
+// move physical bit p to position 0 (bits below p shift up by one)
+static void layout_move(sv_state* s, int p) {
+    for (int q = 0; q < s->n; ++q) {
+        if (s->phys_of_log[q] < p) s->phys_of_log[q] += 1;
+        else if (s->phys_of_log[q] == p) s->phys_of_log[q] = 0;
+    }
+    const u64 low = (p == 0) ? 0 : (s->xmask & ((1ull << p) - 1));
+    const u64 hi = (p == 63) ? 0 : (s->xmask & ~((2ull << p) - 1));
+    s->xmask = hi | (low << 1) | ((s->xmask >> p) & 1ull);
+}
+
+extern "C" size_t sv_arena_bytes(uint64_t capacity) { return layout_for(capacity).total; }
+
+static int init_state(sv_state* s) {
+    s->cur = 0;
+    s->count = 1;
+    s->xmask = 0;
+    for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
+    const u64 k0 = 0;
+    const double2 a0 = make_double2(1.0, 0.0);   // ground state
+    CU(cudaMemcpyAsync(s->keys[0], &k0, 8, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaMemcpyAsync(s->amps[0], &a0, 16, cudaMemcpyHostToDevice, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    return SV_OK;
+}
+
+static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t arena_bytes, void* stream, bool own,
+                         sv_state** out) {
+    if (!out) return SV_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (n_qubits < 1 || n_qubits > 64 || capacity < 1 || capacity >= (1ull << 32) * 8) return SV_ERR_INVALID_ARG;
+    const ArenaLayout L = layout_for(capacity);
+    sv_state* s = new (std::nothrow) sv_state();
+    if (!s) return SV_ERR_NOMEM;
+    memset(s, 0, sizeof(*s));
+    s->n = n_qubits; s->cap = capacity; s->own_mem = own; s->own_stream = own;
+    if (own) {
+        if (cudaMalloc(&arena, L.total) != cudaSuccess) { cudaGetLastError(); delete s; return SV_ERR_NOMEM; }
+        cudaStream_t st;
+        if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { cudaFree(arena); delete s; return SV_ERR_CUDA; }
+        s->stream = st;
+    } else {
+        if (!arena || arena_bytes < L.total || ((uintptr_t)arena & 255)) { delete s; return SV_ERR_INVALID_ARG; }
+        s->stream = (cudaStream_t)stream;
+    }
+    s->arena = (unsigned char*)arena;
+    for (int i = 0; i < 2; ++i) { s->keys[i] = (u64*)(s->arena + L.keys[i]); s->amps[i] = (double2*)(s->arena + L.amps[i]); }
+    s->desc = (TileDesc*)(s->arena + L.desc);
+    s->status = (u64*)(s->arena + L.status);
+    s->hist = (u64*)(s->arena + L.hist);
+    s->sel = (SelState*)(s->arena + L.sel);
+    s->tab = (GateTab*)(s->arena + L.tab);
+    s->d_count = (u64*)(s->arena + L.misc);
+    s->tile_counter = (u32*)(s->arena + L.misc + 64);
+    s->d_bad = (int*)(s->arena + L.misc + 128);
+    s->d_norm = (double*)(s->arena + L.misc + 192);
+    s->partials = (double*)(s->arena + L.partials);
+    if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
+    if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
+        sv_destroy(s);
+        return SV_ERR_CUDA;
+    }
+    *out = s;
+    return SV_OK;
+}
+
+extern "C" int sv_create(int n_qubits, uint64_t capacity, sv_state** out) {
+    return create_common(n_qubits, capacity, nullptr, 0, nullptr, true, out);
+}
+extern "C" int sv_create_in_arena(int n_qubits, uint64_t capacity, void* dev_arena, size_t arena_bytes, void* cuda_stream,
+                                  sv_state** out) {
+    return create_common(n_qubits, capacity, dev_arena, arena_bytes, cuda_stream, false, out);
+}
+extern "C" void sv_destroy(sv_state* s) {
+    if (!s) return;
+    cudaStreamSynchronize(s->stream);
+    if (s->pinned) cudaFreeHost(s->pinned);
+    if (s->own_mem && s->arena) cudaFree(s->arena);
+    if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
+    delete s;
+}
+extern "C" const char* sv_last_error(const sv_state* s) { return s ? s->err : "null handle"; }
+extern "C" int sv_sync(sv_state* s) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    CU(cudaStreamSynchronize(s->stream));
+    return SV_OK;
+}
+extern "C" int sv_num_terms(sv_state* s, uint64_t* n) {
+    if (!s || !n) return SV_ERR_INVALID_ARG;
+    CU(cudaStreamSynchronize(s->stream));
+    *n = s->count;
+    return SV_OK;
+}
+extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
+    if (!s || !out) return SV_ERR_INVALID_ARG;
+    *out = s->stats;
+    return SV_OK;
+}
+
+static int read_back(sv_state* s, void* dst, const void* dsrc, size_t bytes) {
+    CU(cudaMemcpyAsync(s->pinned, dsrc, bytes, cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    memcpy(dst, s->pinned, bytes);
+    return SV_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// sv_apply_gate: classify (row a-1), plan the bit moves, launch
+// ---------------------------------------------------------------------------------------
+static inline bool is_zero(const sv_c128& z) { return z.re == 0.0 && z.im == 0.0; }
+
+extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c128* U) {
+    if (!s || !qubits || !U) return s ? fail(s, SV_ERR_INVALID_ARG, "null argument") : SV_ERR_INVALID_ARG;
+    if (m < 1 || m > SV_MAX_M) return fail(s, SV_ERR_INVALID_ARG, "m must be 1..4");
+    u64 seen = 0;
+    for (int j = 0; j < m; ++j) {
+        if (qubits[j] < 0 || qubits[j] >= s->n) return fail(s, SV_ERR_INVALID_ARG, "qubit out of range");
+        if (seen & (1ull << qubits[j])) return fail(s, SV_ERR_INVALID_ARG, "repeated qubit");
+        seen |= 1ull << qubits[j];
+    }
+    const int d = 1 << m;
+    s->err[0] = 0;
+    s->stats.m = m; s->stats.n_in = s->count; s->stats.n_out = s->count; s->stats.passes = 0;
+
+    // a-1: bit j is control-like iff U never connects patterns that differ in bit j
+    int active[SV_MAX_M], ctrl[SV_MAX_M], ma = 0, mc = 0;
+    for (int j = 0; j < m; ++j) {
+        bool mixes = false;
+        for (int r = 0; r < d && !mixes; ++r)
+            for (int c = 0; c < d; ++c)
+                if ((((r ^ c) >> j) & 1) && !is_zero(U[r * d + c])) { mixes = true; break; }
+        if (mixes) active[ma++] = j; else ctrl[mc++] = j;
+    }
+    s->stats.active_bits = ma;
+    int amask_l = 0;
+    for (int i = 0; i < ma; ++i) amask_l |= 1 << active[i];
+    // lazy X mask on the gate's qubits, as a local pattern
+    int xm = 0;
+    for (int j = 0; j < m; ++j) xm |= (int)((s->xmask >> s->phys_of_log[qubits[j]]) & 1ull) << j;
+    auto Ueff = [&](int r, int c) -> const sv_c128& { return U[(r ^ xm) * d + (c ^ xm)]; };   // in stored patterns
+
+    GateTab tab;
+    memset(&tab, 0, sizeof(tab));
+    if (s->count == 0) { s->stats.gate_class = SV_CLASS_NONE; return SV_OK; }
+
+    // XOR class: U[r][c] != 0 iff r == c ^ x0 (then x0 = all active bits); pure relabelling + phases
+    bool xor_class = ma > 0, diag_nonzero = true, unit_phase = true;
+    for (int c = 0; c < d && xor_class; ++c)
+        for (int r = 0; r < d; ++r) {
+            const bool want = (r == (c ^ amask_l));
+            if (want == is_zero(U[r * d + c])) { xor_class = false; break; }
+        }
+    if (ma == 0)
+        for (int c = 0; c < d; ++c) if (is_zero(U[c * d + c])) diag_nonzero = false;
+
+    if ((ma == 0 && diag_nonzero) || xor_class) {
+        // phase table in stored patterns: every gate bit acts as a control of a diagonal
+        tab.ma = 0; tab.mc = m;
+        for (int j = 0; j < m; ++j) tab.ctrl_pos[j] = s->phys_of_log[qubits[j]];
+        for (int cs = 0; cs < d; ++cs) {
+            const int ct = cs ^ xm;                       // true pattern of the stored pattern
+            const sv_c128 z = U[(ct ^ (xor_class ? amask_l : 0)) * d + ct];
+            tab.U[cs] = make_double2(z.re, z.im);
+            if (!(z.re == 1.0 && z.im == 0.0)) unit_phase = false;
+        }
+        if (xor_class)   // flip the lazy mask on the active bits: no data is touched
+            for (int i = 0; i < ma; ++i) s->xmask ^= 1ull << s->phys_of_log[qubits[active[i]]];
+        s->stats.gate_class = xor_class ? SV_CLASS_XOR : SV_CLASS_DIAGONAL;
+        if (!unit_phase) {
+            CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
+            s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->count, s->tab, s->stream);
+            CHECK_LAUNCH();
+            s->stats.passes = 1;
+        }
+        return SV_OK;
+    }
+
+    // GROUP class.  The active bits must occupy physical positions 0..ma-1.  Those already
+    // forming a prefix {0..k-1} stay; the others are moved to the LSB one pass each, the
+    // last move fused with the tuple mat-vec.
+    s->stats.gate_class = SV_CLASS_GROUP;
+    int need[SV_MAX_M], nneed = 0;
+    {
+        bool inlow[SV_MAX_M + 1] = {false, false, false, false, false};
+        for (int i = 0; i < ma; ++i) { const int p = s->phys_of_log[qubits[active[i]]]; if (p < ma) inlow[p] = true; }
+        int k = 0;
+        while (k < ma && inlow[k]) ++k;
+        for (int i = ma - 1; i >= 0; --i)
+            if (s->phys_of_log[qubits[active[i]]] >= k) need[nneed++] = active[i];
+    }
+    for (int t = 0; t + 1 < nneed; ++t) {   // pure moves: state preserving, committed one by one
+        const int p = s->phys_of_log[qubits[need[t]]];
+        if (p == 0) continue;
+        const int alt = s->cur ^ 1;
+        s->stats.launches += svk_move(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, p, s->desc, s->stream);
+        CHECK_LAUNCH();
+        s->cur = alt;
+        layout_move(s, p);
+        s->stats.passes += 1;
+    }
+    int plast = -1;
+    if (nneed > 0) {
+        plast = s->phys_of_log[qubits[need[nneed - 1]]];
+        if (plast == 0) plast = -1;
+    }
+    // layout after the final move (on a copy: committed only on success)
+    sv_state after = *s;
+    if (plast > 0) layout_move(&after, plast);
+    tab.ma = ma; tab.mc = mc;
+    int fpos[SV_MAX_M];
+    for (int i = 0; i < ma; ++i) fpos[i] = after.phys_of_log[qubits[active[i]]];   // in 0..ma-1
+    for (int i = 0; i < mc; ++i) tab.ctrl_pos[i] = after.phys_of_log[qubits[ctrl[i]]];
+    for (int t = 0; t < (1 << ma); ++t) {
+        int x = 0;
+        for (int i = 0; i < ma; ++i) x |= ((t >> i) & 1) << fpos[i];
+        tab.colorder[t] = x;
+    }
+    for (int cx = 0; cx < (1 << mc); ++cx)
+        for (int xr = 0; xr < (1 << ma); ++xr)
+            for (int xc = 0; xc < (1 << ma); ++xc) {
+                int r = 0, c = 0;
+                for (int i = 0; i < mc; ++i) { r |= ((cx >> i) & 1) << ctrl[i]; c |= ((cx >> i) & 1) << ctrl[i]; }
+                for (int i = 0; i < ma; ++i) { r |= ((xr >> fpos[i]) & 1) << active[i]; c |= ((xc >> fpos[i]) & 1) << active[i]; }
+                const sv_c128& z = Ueff(r, c);
+                tab.U[(((cx << ma) | xr) << ma) | xc] = make_double2(z.re, z.im);
+            }
+    CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
+    const int alt = s->cur ^ 1;
+    s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, plast, ma,
+                                   s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream);
+    CHECK_LAUNCH();
+    s->stats.passes += 1;
+    u64 nout = 0;
+    int rc = read_back(s, &nout, s->d_count, sizeof(u64));
+    if (rc != SV_OK) return rc;
+    if (nout > s->cap) {
+        s->stats.n_out = nout;
+        return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
+    }
+    if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; }
+    s->cur = alt;
+    s->count = nout;
+    s->stats.n_out = nout;
+    return SV_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// truncation driver (rows a-8, a-9)
+// ---------------------------------------------------------------------------------------
+static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
+    const KeyMap km = keymap_of(s);
+    s->stats.launches += svk_sel_init(s->sel, s->count, max_terms, min_mass, s->stream);
+    const int max_levels = 6 + (s->n + 11) / 12 + 1;
+    for (int it = 0; it < max_levels; ++it) {
+        s->stats.launches += svk_sel_hist(s->keys[s->cur], s->amps[s->cur], s->count, s->sel, km, s->n, s->hist, s->stream);
+        s->stats.launches += svk_sel_step(s->sel, s->hist, s->n, s->stream);
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        int rc = read_back(s, out, s->sel, sizeof(SelState));
+        if (rc != SV_OK) return rc;
+        if (out->done) return SV_OK;
+    }
+    return fail(s, SV_ERR_CUDA, "radix select did not converge");
+}
+
+extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, double* kept_fraction) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    if (!(min_mass > 0.0)) return fail(s, SV_ERR_INVALID_ARG, "min_mass must be > 0");
+    s->err[0] = 0;
+    s->stats.gate_class = SV_CLASS_NONE; s->stats.m = 0; s->stats.active_bits = 0; s->stats.passes = 0;
+    s->stats.n_in = s->count; s->stats.n_out = s->count;
+    if (kept_fraction) *kept_fraction = 1.0;
+    const bool needK = max_terms != 0 && max_terms < s->count, needM = min_mass < 1.0;
+    if (s->count == 0 || (!needK && !needM)) return SV_OK;
+    SelState ss;
+    int rc = run_select(s, max_terms, min_mass, &ss);
+    if (rc != SV_OK) return rc;
+    if (ss.final_count >= s->count) return SV_OK;   // nothing dropped: bitwise no-op (reading R7)
+    const int alt = s->cur ^ 1;
+    s->stats.launches += svk_compact(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, s->sel,
+                                     keymap_of(s), 1, s->status, s->tile_counter, s->d_count, s->stream);
+    CHECK_LAUNCH();
+    s->stats.passes += 1;
+    u64 nout = 0;
+    rc = read_back(s, &nout, s->d_count, sizeof(u64));
+    if (rc != SV_OK) return rc;
+    if (nout != ss.final_count) return fail(s, SV_ERR_CUDA, "internal: compaction count differs from select count");
+    s->cur = alt;
+    s->count = nout;
+    s->stats.n_out = nout;
+    if (kept_fraction) *kept_fraction = ss.kept_fraction;
+    return SV_OK;
+}
+
+extern "C" int sv_norm(sv_state* s, double* mass) {
+    if (!s || !mass) return SV_ERR_INVALID_ARG;
+    s->stats.launches += svk_norm(s->amps[s->cur], s->count, s->partials, s->d_norm, s->stream);
+    CHECK_LAUNCH();
+    return read_back(s, mass, s->d_norm, sizeof(double));
+}
+
+extern "C" int sv_check_invariants(sv_state* s, int* ok) {
+    if (!s || !ok) return SV_ERR_INVALID_ARG;
+    s->stats.launches += svk_check(s->keys[s->cur], s->amps[s->cur], s->count, s->n, s->d_bad, s->stream);
+    CHECK_LAUNCH();
+    int bad = 0;
+    int rc = read_back(s, &bad, s->d_bad, sizeof(int));
+    if (rc != SV_OK) return rc;
+    *ok = (bad == 0 && s->count <= s->cap) ? 1 : 0;
+    return SV_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// readout (row a-11): select k, gather, order by (p desc, key asc), copy to the host
+// ---------------------------------------------------------------------------------------
+struct TmpBuf {
+    void* p = nullptr;
+    ~TmpBuf() { if (p) cudaFree(p); }
+    int alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 256) == cudaSuccess ? 0 : -1; }
+};
+
+extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, double* probs, uint64_t* n_written) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    s->err[0] = 0;
+    const u64 kk = k < s->count ? k : s->count;
+    if (n_written) *n_written = kk;
+    if (kk == 0) return SV_OK;
+    if (kk >= (1ull << 32)) return fail(s, SV_ERR_INVALID_ARG, "sv_top supports k < 2^32");
+    SelState ss;
+    const int use_sel = kk < s->count;
+    if (use_sel) {
+        int rc = run_select(s, kk, 1.0, &ss);
+        if (rc != SV_OK) return rc;
+    }
+    const size_t a8 = align_up(kk * 8), a16 = align_up(kk * 16), a4 = align_up(kk * 4);
+    const size_t sscr = align_up(svk_sort_scratch_bytes(kk));
+    TmpBuf tb;
+    if (tb.alloc(a8 * 6 + a16 * 2 + a4 * 2 + sscr) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_top: scratch allocation failed"); }
+    unsigned char* b = (unsigned char*)tb.p;
+    u64* pat = (u64*)b; b += a8;
+    u64* lkey = (u64*)b; b += a8;
+    u64* ka = (u64*)b; b += a8;
+    u64* kb = (u64*)b; b += a8;
+    u64* okey = (u64*)b; b += a8;
+    double* oprob = (double*)b; b += a8;
+    double2* amp = (double2*)b; b += a16;
+    double2* oamp = (double2*)b; b += a16;
+    u32* va = (u32*)b; b += a4;
+    u32* vb = (u32*)b; b += a4;
+    u32* scr = (u32*)b;
+    cudaStream_t st = s->stream;
+    s->stats.launches += svk_gather_top(s->keys[s->cur], s->amps[s->cur], s->count, s->sel, use_sel, keymap_of(s), pat, lkey,
+                                        amp, s->d_count, kk, st);
+    CHECK_LAUNCH();
+    u64 got = 0;
+    int rc = read_back(s, &got, s->d_count, sizeof(u64));
+    if (rc != SV_OK) return rc;
+    if (got != kk) return fail(s, SV_ERR_CUDA, "internal: readout selected a different number of terms");
+    // order: logical key ascending first, then (stable) ~p ascending = p descending
+    CU(cudaMemcpyAsync(ka, lkey, kk * 8, cudaMemcpyDeviceToDevice, st));
+    s->stats.launches += svk_iota(va, kk, st);
+    int in_alt = 0;
+    s->stats.launches += svk_sort_pairs(ka, va, kb, vb, kk, s->n, scr, st, &in_alt);
+    u32* perm1 = in_alt ? vb : va;
+    u64* k2 = in_alt ? ka : kb;          // the buffer pair not holding perm1 becomes the next input
+    u32* v2 = in_alt ? va : vb;
+    s->stats.launches += svk_gather_u64(pat, perm1, k2, kk, 1, st);
+    CU(cudaMemcpyAsync(v2, perm1, kk * 4, cudaMemcpyDeviceToDevice, st));
+    u64* k2alt = in_alt ? kb : ka;
+    u32* v2alt = in_alt ? vb : va;
+    int in_alt2 = 0;
+    s->stats.launches += svk_sort_pairs(k2, v2, k2alt, v2alt, kk, 64, scr, st, &in_alt2);
+    u32* perm = in_alt2 ? v2alt : v2;
+    s->stats.launches += svk_gather_u64(lkey, perm, okey, kk, 0, st);
+    s->stats.launches += svk_gather_c128(amp, perm, oamp, kk, st);
+    s->stats.launches += svk_gather_u64(pat, perm, k2, kk, 0, st);   // k2 is free again
+    s->stats.launches += svk_pat_to_prob(k2, oprob, kk, st);
+    CHECK_LAUNCH();
+    if (keys) CU(cudaMemcpyAsync(keys, okey, kk * 8, cudaMemcpyDeviceToHost, st));
+    if (amps) CU(cudaMemcpyAsync(amps, oamp, kk * 16, cudaMemcpyDeviceToHost, st));
+    if (probs) CU(cudaMemcpyAsync(probs, oprob, kk * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return SV_OK;
+}
+
+// ---------------------------------------------------------------------------------------
+// load: establish the sorted storage order with the radix sort
+// ---------------------------------------------------------------------------------------
+extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c128* dev_amps, uint64_t n) {
+    if (!s || (n && (!dev_keys || !dev_amps))) return SV_ERR_INVALID_ARG;
+    s->err[0] = 0;
+    if (n > s->cap) return fail(s, SV_ERR_INVALID_ARG, "sv_load: n exceeds capacity");
+    if (n >= (1ull << 32)) return fail(s, SV_ERR_INVALID_ARG, "sv_load supports n < 2^32");
+    cudaStream_t st = s->stream;
+    const int alt = s->cur ^ 1;
+    if (n > 0) {
+        const size_t a8 = align_up(n * 8), a4 = align_up(n * 4);
+        TmpBuf tb;
+        if (tb.alloc(a8 * 2 + a4 * 2 + align_up(svk_sort_scratch_bytes(n))) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: scratch allocation failed"); }
+        unsigned char* b = (unsigned char*)tb.p;
+        u64* ka = (u64*)b; b += a8;
+        u64* kb = (u64*)b; b += a8;
+        u32* va = (u32*)b; b += a4;
+        u32* vb = (u32*)b; b += a4;
+        u32* scr = (u32*)b;
+        CU(cudaMemcpyAsync(ka, dev_keys, n * 8, cudaMemcpyDeviceToDevice, st));
+        s->stats.launches += svk_iota(va, n, st);
+        int in_alt = 0;
+        s->stats.launches += svk_sort_pairs(ka, va, kb, vb, n, 64, scr, st, &in_alt);
+        CU(cudaMemcpyAsync(s->keys[alt], in_alt ? kb : ka, n * 8, cudaMemcpyDeviceToDevice, st));
+        s->stats.launches += svk_gather_c128((const double2*)dev_amps, in_alt ? vb : va, s->amps[alt], n, st);
+        s->stats.launches += svk_check(s->keys[alt], s->amps[alt], n, s->n, s->d_bad, st);
+        CHECK_LAUNCH();
+        int bad = 0;
+        int rc = read_back(s, &bad, s->d_bad, sizeof(int));
+        if (rc != SV_OK) return rc;
+        if (bad) return fail(s, SV_ERR_INVALID_ARG, "sv_load: duplicate key, key >= 2^n or zero amplitude (state unchanged)");
+    }
+    s->cur = alt;
+    s->count = n;
+    s->xmask = 0;
+    for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
+    s->stats.n_in = n; s->stats.n_out = n; s->stats.gate_class = SV_CLASS_NONE;
+    return SV_OK;
+}
+
+extern "C" int sv_load(sv_state* s, const uint64_t* keys, const sv_c128* amps, uint64_t n) {
+    if (!s || (n && (!keys || !amps))) return SV_ERR_INVALID_ARG;
+    if (n > s->cap) return fail(s, SV_ERR_INVALID_ARG, "sv_load: n exceeds capacity");
+    TmpBuf tk, ta;
+    if (tk.alloc(n * 8) != 0 || ta.alloc(n * 16) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: staging allocation failed"); }
+    if (n) {
+        CU(cudaMemcpyAsync(tk.p, keys, n * 8, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaMemcpyAsync(ta.p, amps, n * 16, cudaMemcpyHostToDevice, s->stream));
+    }
+    int rc = sv_load_device(s, (const uint64_t*)tk.p, (const sv_c128*)ta.p, n);
+    cudaStreamSynchronize(s->stream);
+    return rc;
+}

@@ -1,0 +1,109 @@
+// Device-side helpers shared by the engine's kernels.
+#pragma once
+#include "sv_internal.h"
+
+#define SV_FLAG_AGG  (1ull << 62)
+#define SV_FLAG_INCL (2ull << 62)
+#define SV_VAL_MASK  ((1ull << 62) - 1)
+
+__device__ __forceinline__ u64 ld_relaxed_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u64(u64* p, u64 v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// Streaming 128-bit / 64-bit accesses (read once / written once: keep them out of L1).
+__device__ __forceinline__ double2 ld_stream_d2(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ u64 ld_stream_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.global.nc.L1::no_allocate.u64 %0, [%1];" : "=l"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream_d2(double2* p, double2 v) {
+    asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_stream_u64(u64* p, u64 v) {
+    asm volatile("st.global.L1::no_allocate.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// Decoupled look-back (single-pass chained scan).  Tile ids MUST be handed out by an
+// atomic counter so that every predecessor of a running tile has already started.
+// Returns the exclusive prefix of `total` over tiles 0..tile-1.  Called by one thread.
+__device__ __forceinline__ u64 lookback_exclusive(u64* status, u32 tile, u64 total) {
+    if (tile == 0) {
+        st_relaxed_u64(&status[0], SV_FLAG_INCL | total);
+        return 0;
+    }
+    st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
+    u64 excl = 0;
+    u32 j = tile - 1;
+    for (;;) {
+        u64 v;
+        do { v = ld_relaxed_u64(&status[j]); } while ((v >> 62) == 0);
+        excl += v & SV_VAL_MASK;
+        if ((v >> 62) == 2) break;
+        --j;
+    }
+    st_relaxed_u64(&status[tile], SV_FLAG_INCL | (excl + total));
+    return excl;
+}
+
+// Exclusive block scan of one int per thread (blockDim.x == SV_THREADS).  `red` holds
+// SV_THREADS/32 + 1 ints.  Returns the exclusive prefix; *total gets the block sum.
+__device__ __forceinline__ int block_excl_scan(int v, int* red, int* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    __syncthreads();  // protect `red` against a previous use
+    if (lane == 31) red[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        int w = (lane < SV_THREADS / 32) ? red[lane] : 0;
+        int winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, winc, d);
+            if (lane >= d) winc += t;
+        }
+        if (lane < SV_THREADS / 32) red[lane] = winc - w;
+        if (lane == SV_THREADS / 32 - 1) red[SV_THREADS / 32] = winc;
+    }
+    __syncthreads();
+    *total = red[SV_THREADS / 32];
+    return red[warp] + inc - v;
+}
+
+// Complex product and accumulation with every operation rounded separately (no FMA):
+// the arithmetic contract of DESIGN.md "Determinism" (D1).
+__device__ __forceinline__ void cmul_acc(double& sr, double& si, double ur, double ui, double ar, double ai) {
+    const double pr = __dsub_rn(__dmul_rn(ur, ar), __dmul_rn(ui, ai));
+    const double pi = __dadd_rn(__dmul_rn(ur, ai), __dmul_rn(ui, ar));
+    sr = __dadd_rn(sr, pr);
+    si = __dadd_rn(si, pi);
+}
+
+__device__ __forceinline__ double prob_of(double2 a) {  // p = re*re + im*im, no FMA (D2)
+    return __dadd_rn(__dmul_rn(a.x, a.x), __dmul_rn(a.y, a.y));
+}
+
+// stored (physical) key -> logical key: undo the lazy X mask, then the bit permutation.
+__device__ __forceinline__ u64 logical_key(u64 stored, const KeyMap& km) {
+    u64 t = stored ^ km.xmask, out = 0;
+    while (t) {
+        int p = __ffsll((long long)t) - 1;
+        t &= t - 1;
+        out |= 1ull << km.log_of_phys[p];
+    }
+    return out;
+}

@@ -1,0 +1,92 @@
+// Internal declarations shared by the engine's translation units (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+
+typedef unsigned long long u64;
+typedef unsigned int u32;
+
+#define SV_MAX_M 4
+#define SV_TILE_SLOTS 2048      // outputs one group tile may produce (8 per thread at 256 threads)
+#define SV_MOVE_TILE 2048       // elements per tile of a pure bit-move pass
+#define SV_THREADS 256
+#define SV_SEL_BINS 4096        // 12-bit digits for the radix select
+
+// Gate tables in device memory, in PHYSICAL pattern indexing.
+struct GateTab {
+    int ma;                 // active bits: they sit at physical positions 0..ma-1 when the group kernel runs
+    int mc;                 // control-like bits
+    int ctrl_pos[SV_MAX_M]; // physical position of control bit i (layout after the final move)
+    int colorder[16];       // colorder[t] = physical active pattern of the t-th logical column
+    double2 U[256];         // U[((cx << ma | xr) << ma) | xc]
+};
+
+// One tile boundary of a bit-move pass: a merge-path split inside one block (= maximal
+// range of keys that agree above the moved bit).  A = keys with the bit 0, B = bit 1.
+struct TileDesc {
+    u64 ia;   // first A element not yet consumed (global index)
+    u64 ib;   // first B element not yet consumed
+    u64 mid;  // start of the block's B run
+    u64 e;    // end of the block
+};
+
+// Radix-select state (device resident; one per handle).
+struct SelState {
+    u64 pat_prefix;      // resolved high bits of the cutoff probability pattern
+    u64 key_prefix;      // resolved high bits of the cutoff logical key (tie phase)
+    int level;           // next level to run: 0..5 = p levels, 6.. = key levels
+    int done;            // 1: PT/KT final
+    int count_active, mass_active;
+    u64 k_rem;           // terms still to take from the candidate bin (count criterion)
+    double mass_rem_hi, mass_rem_lo;   // mass still to collect (mass criterion), double-double
+    u64 kept_count;      // terms certainly kept so far
+    double kept_hi, kept_lo;           // their mass, double-double
+    double total_hi, total_lo;         // total mass S
+    u64 cand_count;      // size of the current candidate bin
+    u64 PT, KT;          // final predicate: keep iff pat > PT || (pat == PT && lkey <= KT)
+    double kept_mass, total_mass, scale, kept_fraction;
+    u64 final_count;     // number of terms the predicate keeps
+    u64 n_total;
+};
+
+struct KeyMap {          // stored (physical) key -> logical key
+    unsigned char log_of_phys[64];   // logical qubit of physical bit p (0xff = unused)
+    u64 xmask;                        // lazy X mask in physical positions
+};
+
+// ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
+int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
+
+int svk_move(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p,
+             TileDesc* desc, cudaStream_t st);
+
+// Final pass of a group gate.  p < 0: the active bits already sit at the LSBs (no move).
+// Writes the output term count to *d_count (may exceed cap: then nothing past cap is written).
+int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
+              const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count,
+              u64 cap, cudaStream_t st);
+
+int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
+
+int svk_sel_init(SelState* ss, u64 n, u64 max_terms, double min_mass, cudaStream_t st);
+int svk_sel_hist(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, int nq,
+                 u64* hist, cudaStream_t st);
+int svk_sel_step(SelState* ss, u64* hist, int nq, cudaStream_t st);
+int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
+                const SelState* ss, KeyMap km, int do_scale, u64* status, u32* tile_counter,
+                u64* d_count, cudaStream_t st);
+
+int svk_check(const u64* keys, const double2* amps, u64 n, int nq, int* d_bad, cudaStream_t st);
+
+// readout / load helpers
+int svk_gather_top(const u64* keys, const double2* amps, u64 n, const SelState* ss, int use_sel,
+                   KeyMap km, u64* o_pat, u64* o_lkey, double2* o_amp, u64* d_count, u64 kmax,
+                   cudaStream_t st);
+int svk_sort_pairs(u64* keys, u32* vals, u64* keys_alt, u32* vals_alt, u64 n, int bits,
+                   u32* hist_scratch, cudaStream_t st, int* result_in_alt);
+size_t svk_sort_scratch_bytes(u64 n);
+int svk_iota(u32* v, u64 n, cudaStream_t st);
+int svk_gather_u64(const u64* src, const u32* idx, u64* dst, u64 n, int invert, cudaStream_t st);
+int svk_gather_c128(const double2* src, const u32* idx, double2* dst, u64 n, cudaStream_t st);
+int svk_pat_to_prob(const u64* pat, double* prob, u64 n, cudaStream_t st);

@@ -1,0 +1,179 @@
+"""Thin Python binding of the C-ABI library (include/sparse_sv.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels of
+libsparse_sv.so.  PyTorch is used for device memory (the arena tensor) and the stream.
+There is no CPU fallback: importing this module without the built library raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libsparse_sv.so")
+
+SV_OK, SV_ERR_INVALID_ARG, SV_ERR_CAPACITY, SV_ERR_NOMEM, SV_ERR_CUDA = 0, -1, -2, -3, -4
+_ERRNAME = {-1: "SV_ERR_INVALID_ARG", -2: "SV_ERR_CAPACITY", -3: "SV_ERR_NOMEM", -4: "SV_ERR_CUDA"}
+CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
+
+EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
+           "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
+           "sv_check_invariants", "sv_last_error", "sv_sync"]
+
+
+class SvStats(C.Structure):
+    _fields_ = [("gate_class", C.c_int), ("m", C.c_int), ("active_bits", C.c_int), ("passes", C.c_int),
+                ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64)]
+
+
+class SvError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("%s: %s" % (_ERRNAME.get(code, str(code)), msg))
+        self.code = code
+
+
+def load_library(path: str = _LIBPATH):
+    if not os.path.exists(path):
+        raise ImportError("CUDA library %s is missing: run `python -m paper_2607_07816_b200.build` "
+                          "(there is no CPU fallback)" % path)
+    lib = C.CDLL(path)
+    vp, u64, i32, dbl = C.c_void_p, C.c_uint64, C.c_int, C.c_double
+    lib.sv_arena_bytes.restype = C.c_size_t
+    lib.sv_arena_bytes.argtypes = [u64]
+    lib.sv_create.restype = i32
+    lib.sv_create.argtypes = [i32, u64, C.POINTER(vp)]
+    lib.sv_create_in_arena.restype = i32
+    lib.sv_create_in_arena.argtypes = [i32, u64, vp, C.c_size_t, vp, C.POINTER(vp)]
+    lib.sv_destroy.restype = None
+    lib.sv_destroy.argtypes = [vp]
+    lib.sv_apply_gate.restype = i32
+    lib.sv_apply_gate.argtypes = [vp, vp, i32, vp]
+    lib.sv_truncate.restype = i32
+    lib.sv_truncate.argtypes = [vp, u64, dbl, C.POINTER(dbl)]
+    lib.sv_norm.restype = i32
+    lib.sv_norm.argtypes = [vp, C.POINTER(dbl)]
+    lib.sv_top.restype = i32
+    lib.sv_top.argtypes = [vp, u64, vp, vp, vp, C.POINTER(u64)]
+    lib.sv_num_terms.restype = i32
+    lib.sv_num_terms.argtypes = [vp, C.POINTER(u64)]
+    lib.sv_load.restype = i32
+    lib.sv_load.argtypes = [vp, vp, vp, u64]
+    lib.sv_load_device.restype = i32
+    lib.sv_load_device.argtypes = [vp, vp, vp, u64]
+    lib.sv_get_stats.restype = i32
+    lib.sv_get_stats.argtypes = [vp, C.POINTER(SvStats)]
+    lib.sv_check_invariants.restype = i32
+    lib.sv_check_invariants.argtypes = [vp, C.POINTER(i32)]
+    lib.sv_last_error.restype = C.c_char_p
+    lib.sv_last_error.argtypes = [vp]
+    lib.sv_sync.restype = i32
+    lib.sv_sync.argtypes = [vp]
+    return lib
+
+
+lib = load_library()
+
+
+class SparseSV:
+    """One sparse, truncated state on one GPU.  Starts in |0...0>."""
+
+    def __init__(self, n_qubits: int, capacity: int, device="cuda:0", torch_arena: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2607_07816_b200.engine needs a CUDA device (no CPU fallback)")
+        self.n = int(n_qubits)
+        self.capacity = int(capacity)
+        self.device = torch.device(device)
+        self._h = C.c_void_p()
+        self._arena = None
+        torch.cuda.set_device(self.device)
+        if torch_arena:
+            nbytes = int(lib.sv_arena_bytes(self.capacity))
+            self._arena = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            ptr = (self._arena.data_ptr() + 255) & ~255
+            self._stream = torch.cuda.current_stream(self.device)
+            rc = lib.sv_create_in_arena(self.n, self.capacity, ptr, nbytes, self._stream.cuda_stream, C.byref(self._h))
+        else:
+            rc = lib.sv_create(self.n, self.capacity, C.byref(self._h))
+        if rc != SV_OK:
+            raise SvError(rc, "sv_create failed (n=%d capacity=%d)" % (self.n, self.capacity))
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib.sv_destroy(self._h)
+            self._h = C.c_void_p()
+        self._arena = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk(self, rc):
+        if rc != SV_OK:
+            raise SvError(rc, lib.sv_last_error(self._h).decode())
+
+    def apply_gate(self, qubits, U):
+        q = np.ascontiguousarray(qubits, dtype=np.int32)
+        U = np.ascontiguousarray(U, dtype=np.complex128)
+        if U.shape != (1 << q.size, 1 << q.size):
+            raise ValueError("U must be 2^m x 2^m")
+        self._chk(lib.sv_apply_gate(self._h, q.ctypes.data, int(q.size), U.ctypes.data))
+
+    def truncate(self, max_terms: int = 0, min_mass: float = 1.0) -> float:
+        kept = C.c_double(1.0)
+        self._chk(lib.sv_truncate(self._h, int(max_terms), float(min_mass), C.byref(kept)))
+        return kept.value
+
+    def norm(self) -> float:
+        m = C.c_double(0.0)
+        self._chk(lib.sv_norm(self._h, C.byref(m)))
+        return m.value
+
+    def num_terms(self) -> int:
+        n = C.c_uint64(0)
+        self._chk(lib.sv_num_terms(self._h, C.byref(n)))
+        return int(n.value)
+
+    def top(self, k: int):
+        k = min(int(k), self.num_terms())
+        keys = np.empty(k, dtype=np.uint64)
+        amps = np.empty(k, dtype=np.complex128)
+        probs = np.empty(k, dtype=np.float64)
+        w = C.c_uint64(0)
+        self._chk(lib.sv_top(self._h, k, keys.ctypes.data, amps.ctypes.data, probs.ctypes.data, C.byref(w)))
+        w = int(w.value)
+        return keys[:w], amps[:w], probs[:w]
+
+    def export(self):
+        """All terms in (p desc, key asc) order (host arrays)."""
+        return self.top(self.num_terms())
+
+    def load(self, keys, amps):
+        keys = np.ascontiguousarray(keys, dtype=np.uint64)
+        amps = np.ascontiguousarray(amps, dtype=np.complex128)
+        if keys.shape != amps.shape:
+            raise ValueError("keys / amps shape mismatch")
+        self._chk(lib.sv_load(self._h, keys.ctypes.data, amps.ctypes.data, int(keys.size)))
+
+    def load_device(self, keys_t, amps_t):
+        """keys_t: torch int64/uint64 CUDA tensor; amps_t: torch complex128 CUDA tensor."""
+        n = int(keys_t.numel())
+        assert amps_t.numel() == n and keys_t.is_cuda and amps_t.is_cuda
+        assert keys_t.is_contiguous() and amps_t.is_contiguous()
+        self._chk(lib.sv_load_device(self._h, keys_t.data_ptr(), amps_t.data_ptr(), n))
+
+    def stats(self) -> dict:
+        st = SvStats()
+        self._chk(lib.sv_get_stats(self._h, C.byref(st)))
+        return {"class": CLASS_NAMES.get(st.gate_class, "?"), "m": st.m, "active_bits": st.active_bits,
+                "passes": st.passes, "n_in": int(st.n_in), "n_out": int(st.n_out), "launches": int(st.launches)}
+
+    def check_invariants(self) -> bool:
+        ok = C.c_int(0)
+        self._chk(lib.sv_check_invariants(self._h, C.byref(ok)))
+        return bool(ok.value)
+
+    def sync(self):
+        self._chk(lib.sv_sync(self._h))

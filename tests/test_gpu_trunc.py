@@ -1,0 +1,141 @@
+"""GPU parity: sv_truncate through the C ABI vs the CPU oracle, and
+step-locked circuit parity with truncation on (BASELINE.json configs[1], [3], [4] at scaled caps)."""
+import numpy as np
+import pytest
+
+from paper_2607_07816_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+from util_parity import assert_same_state, assert_truncation_parity, step_locked, MASS_TOL  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def eng():
+    from paper_2607_07816_b200 import engine
+    return engine
+
+
+def _oracle(n):
+    from oracle.sparse import SparseOracle
+    return SparseOracle(n)
+
+
+def _pair(eng, n, keys, amps, cap=None):
+    sv = eng.SparseSV(n, cap or (keys.size + 64))
+    o = _oracle(n)
+    sv.load(keys, amps)
+    o.load(keys, amps)
+    return sv, o
+
+
+@pytest.mark.parametrize("count,K,f,spread", [
+    (50000, 12345, 1.0, 2.0), (50000, 0, 0.97, 2.0), (50000, 20000, 0.999, 1.0), (50000, 100, 0.9999, 3.0),
+    (3000, 1, 1.0, 2.0), (3000, 2999, 1.0, 0.1), (70001, 0, 0.5, 0.01), (70001, 0, 1e-9, 2.0), (1, 1, 0.5, 1.0),
+    (200000, 65536, 1 - 1e-4, 1.5)])
+def test_truncate_random(eng, count, K, f, spread):
+    rng = np.random.default_rng(count + K)
+    keys, amps = W.random_state(rng, 44, count, spread=spread)
+    sv, o = _pair(eng, 44, keys, amps)
+    kg = sv.truncate(K, f)
+    ko = o.truncate(K, f)
+    assert abs(kg - ko) <= MASS_TOL
+    assert abs(sv.num_terms() - o.num_terms()) <= 2
+    assert_truncation_parity(sv.export()[:2], o.export()[:2])
+    assert sv.check_invariants()
+    assert abs(sv.norm() - 1.0) <= 1e-13
+
+
+def test_truncate_noop_bitwise(eng):
+    rng = np.random.default_rng(0)
+    keys, amps = W.random_state(rng, 30, 5000)
+    sv, o = _pair(eng, 30, keys, amps)
+    before = sv.export()
+    for K, f in ((0, 1.0), (5000, 1.0), (10 ** 9, 2.0), (0, 1.0 - 1e-17)):
+        assert sv.truncate(K, f) == 1.0
+    after = sv.export()
+    assert np.array_equal(before[0], after[0]) and np.array_equal(before[1], after[1])
+
+
+def test_truncate_flat_ties_by_key(eng):
+    """All p equal: the cut is decided by the LOGICAL key, ascending (reading R4), even after
+    gates have permuted the storage order and set the lazy X mask."""
+    n = 40
+    sv = eng.SparseSV(n, 1 << 13)
+    o = _oracle(n)
+    for q in (3, 39, 17, 0, 8, 21, 11, 5, 30, 2, 25, 13):
+        sv.apply_gate([q], W.mat_h())
+        o.apply_gate([q], W.mat_h())
+    for g in ((39,), (8,)):
+        sv.apply_gate(list(g), W.mat_x())
+        o.apply_gate(list(g), W.mat_x())
+    sv.apply_gate([3, 30], W.mat_mcx(2))
+    o.apply_gate([3, 30], W.mat_mcx(2))
+    for K, f in ((1000, 1.0), (0, 0.3), (77, 0.5)):
+        kg = sv.truncate(K, f)
+        ko = o.truncate(K, f)
+        assert abs(kg - ko) <= MASS_TOL
+        assert_same_state(sv.export()[:2], o.export()[:2])
+
+
+def test_truncate_many_ties_mixed(eng):
+    rng = np.random.default_rng(5)
+    keys, amps = W.random_state(rng, 36, 60000, spread=1.0)
+    amps = (np.round(amps * 512) / 512).astype(np.complex128)
+    amps[amps == 0] = 1 / 512
+    sv, o = _pair(eng, 36, keys, amps)
+    for K, f in ((40000, 1.0), (0, 0.9), (5000, 0.99)):
+        kg = sv.truncate(K, f)
+        ko = o.truncate(K, f)
+        assert abs(kg - ko) <= MASS_TOL
+        assert sv.num_terms() == o.num_terms()
+        assert_truncation_parity(sv.export()[:2], o.export()[:2])
+
+
+def _run_step_locked(eng, c, cap, every=1):
+    sv = eng.SparseSV(c.n, cap)
+    make = lambda: _oracle(c.n)
+    for i, g in enumerate(c.gates):
+        if i % every == 0:
+            step_locked(sv, make, g, c.max_terms, c.min_mass, c.truncate_every_gate)
+        else:
+            sv.apply_gate(g.qubits, g.U)
+            if c.truncate_every_gate:
+                sv.truncate(c.max_terms, c.min_mass)
+        assert sv.check_invariants()
+    return sv
+
+
+def test_config2_scaled_step_locked(eng):
+    """configs[1] mix at n=24 with the cap scaled to 2^12; every gate compared from the same pre-gate state."""
+    c = W.config2(num_gates=250, max_terms=1 << 12)
+    sv = _run_step_locked(eng, c, cap=1 << 14)
+    assert sv.num_terms() <= 1 << 12
+
+
+def test_config4_scaled_step_locked(eng):
+    """configs[3] (peaked, 3 layers, 10% 8x8, cap + mass 0.9999 after every gate) at n=16, K=2^11."""
+    c = W.config4(n=16, max_terms=1 << 11, variant="noh")
+    _run_step_locked(eng, c, cap=1 << 15)
+
+
+def test_config5_scaled_step_locked(eng):
+    """configs[4] mix at n=56 with K=2^12 and mass 1-1e-4; every gate compared."""
+    c = W.config5(num_gates=300, max_terms=1 << 12)
+    sv = _run_step_locked(eng, c, cap=1 << 16)
+    assert sv.num_terms() <= 1 << 12
+
+
+def test_config3_small_peak(eng):
+    """configs[2] construction at n=14 (cap = 2^n, never binding): top bit string equals s."""
+    c = W.config3(n=14, seed=2)
+    sv = eng.SparseSV(c.n, 1 << 15)
+    o = _oracle(c.n)
+    for g in c.gates:
+        sv.apply_gate(g.qubits, g.U)
+        o.apply_gate(g.qubits, g.U)
+        sv.truncate(c.max_terms, 1.0)
+    k, a, p = sv.top(1)
+    assert int(k[0]) == c.secret
+    assert_same_state(sv.export()[:2], o.export()[:2], strict_keys=False)
+    assert abs(sv.norm() - 1.0) <= 1e-12
