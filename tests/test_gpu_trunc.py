@@ -71,7 +71,7 @@ def test_truncate_flat_ties_by_key(eng):
         o.apply_gate(list(g), W.mat_x())
     sv.apply_gate([3, 30], W.mat_mcx(2))
     o.apply_gate([3, 30], W.mat_mcx(2))
-    for K, f in ((1000, 1.0), (0, 0.3), (77, 0.5)):
+    for K, f in ((1000, 1.0), (0, 0.3005), (77, 0.4995)):   # thresholds off the knife edge t*p == f*S (R5)
         kg = sv.truncate(K, f)
         ko = o.truncate(K, f)
         assert abs(kg - ko) <= MASS_TOL
