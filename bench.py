@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the sparse, truncated state-vector gate path on B200.
+
+Workload (config.workload = "cfg5"): BASELINE.json configs[4] -- n=56, the 4000-gate
+sparse-growth mix from seed 4, sv_truncate(K=2^28, 1-1e-4) after every gate.  The circuit
+is first run (untimed) until the state reaches the cap; a "step" is then the next
+`--gates-per-step` gates, each applied and truncated: one pass of the whole hot path
+(SURVEY.md rows a-1..a-9).  value = amplitude-terms entering a gate, summed over the
+timed gates, per second (whole job).  The state (6.4 GB at the cap) is far larger than L2,
+so no L2 flush is needed between steps.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "amplitude_terms_per_sec_per_gate"
+UNIT = "terms/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--k-log2", type=int, default=28, help="log2 of the hard cap K (28 = the config's own)")
+    ap.add_argument("--gates-per-step", type=int, default=32)
+    ap.add_argument("--cap-mult", type=int, default=8, help="capacity = cap-mult * K (8 = worst case of an 8x8 gate)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--jsonl", default="", help="optional per-gate JSONL log")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+            except Exception:
+                continue
+            names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+            for nm, v in zip(names, r[5:9]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(nm)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm)); out["sm_max_mhz"] = float(max(mx)); out["samples"] = len(sm)
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline of the default run, and the whole of --impl reference)
+# ------------------------------------------------------------------------------------------
+def oracle_sample(k_log2_sample, gates_per_step, steps, warmup, budget_s):
+    """The oracle, as it stands, on the same cfg5 circuit at a scaled cap: run to the cap,
+    then time steps of `gates_per_step` gates (apply + truncate), bounded by budget_s."""
+    from oracle.sparse import SparseOracle
+    from paper_2607_07816_b200 import workloads as W
+    c = W.config5(max_terms=1 << k_log2_sample)
+    o = SparseOracle(c.n)
+    gi = 0
+    while gi < len(c.gates) and o.num_terms() < 0.9 * c.max_terms:
+        g = c.gates[gi]; gi += 1
+        o.apply_gate(g.qubits, g.U); o.truncate(c.max_terms, c.min_mass)
+    terms, secs, done = 0, 0.0, 0
+    per_step = []
+    t_budget = time.perf_counter()
+    for s in range(warmup + steps):
+        t0 = time.perf_counter(); nt = 0
+        for _ in range(gates_per_step):
+            g = c.gates[gi % len(c.gates)]; gi += 1
+            nt += o.num_terms()
+            o.apply_gate(g.qubits, g.U); o.truncate(c.max_terms, c.min_mass)
+        dt = time.perf_counter() - t0
+        if s >= warmup:
+            terms += nt; secs += dt; done += 1; per_step.append(dt)
+        if time.perf_counter() - t_budget > budget_s and done >= 1:
+            break
+    return {"value": terms / secs if secs > 0 else 0.0, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "cfg5 circuit at cap 2^%d (full config: 2^28), %d step(s) of %d gates after reaching the cap, apply+truncate"
+                      % (k_log2_sample, done, gates_per_step),
+            "steps_done": done, "ms_per_step": 1e3 * secs / max(done, 1)}
+
+
+def run_reference(args):
+    from paper_2607_07816_b200 import dist
+    rank, _, world = dist.env_world()
+    if rank != 0:
+        return
+    r = oracle_sample(14, args.gates_per_step, args.steps, min(args.warmup, 1), budget_s=150.0)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": r["steps_done"], "warmup": min(args.warmup, 1), "ms_per_step": r["ms_per_step"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cfg5", "n_qubits": 56, "K_log2": 28, "min_mass": 1 - 1e-4,
+                       "gates_per_step": args.gates_per_step, "sampled_at_K_log2": 14},
+            "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": 1, "kind": "oracle", "sample": r["sample"]},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA engine arm
+# ------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2607_07816_b200 import dist, engine, workloads as W
+    rank, local_rank, world = dist.init("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    K = 1 << args.k_log2
+    c = W.config5(max_terms=K)
+    free_b, _ = torch.cuda.mem_get_info(dev)
+    cap_mult = args.cap_mult
+    while cap_mult > 2 and engine.lib.sv_arena_bytes(cap_mult * K) > 0.92 * free_b:
+        cap_mult -= 1
+    sv = engine.SparseSV(c.n, cap_mult * K, device=dev)
+    G = args.gates_per_step
+    log = open(args.jsonl, "w") if (args.jsonl and rank == 0) else None
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    # ---- untimed ramp: run the circuit until the state sits at the cap ----
+    gi = 0
+    while gi < len(c.gates) and sv.num_terms() < 0.9 * K:
+        g = c.gates[gi]; gi += 1
+        sv.apply_gate(g.qubits, g.U); sv.truncate(c.max_terms, c.min_mass)
+    ramp_gates = gi
+
+    per_gate = []   # (klass, name, n_in, n_pre, n_kept, passes, e_a0, e_a1, e_t1)
+
+    def one_step(record):
+        nonlocal gi
+        nt = 0
+        for _ in range(G):
+            g = c.gates[gi % len(c.gates)]; gi += 1
+            n_in = sv.num_terms()
+            if record:
+                e0, e1, e2 = ev(), ev(), ev()
+                e0.record()
+            sv.apply_gate(g.qubits, g.U)
+            if record:
+                st = sv.stats(); e1.record()
+            sv.truncate(c.max_terms, c.min_mass)
+            if record:
+                e2.record()
+                per_gate.append((g.klass, g.name, n_in, st["n_out"], sv.stats()["n_out"], st["passes"], e0, e1, e2))
+            nt += n_in
+        return nt
+
+    for _ in range(args.warmup):
+        one_step(False)
+    sv.profile(True)
+    l0 = sv.stats()["launches"]
+    clocks = ClockSampler(local_rank)
+    dist.barrier(); torch.cuda.synchronize()
+    clocks.start()
+    t_start, t_end = ev(), ev()
+    t_start.record()
+    terms = 0
+    for _ in range(args.steps):
+        terms += one_step(True)
+    t_end.record()
+    torch.cuda.synchronize(); dist.barrier()
+    clk = clocks.stop()
+    ms = t_start.elapsed_time(t_end)
+    launches = sv.stats()["launches"] - l0
+    prof = sv.profile_get()
+    sv.profile(False)
+    tot_terms, max_ms = dist.aggregate(terms, ms, dev)
+
+    # ---- per gate class summary (rank 0) ----
+    hbm, peak_kind = peaks()
+    classes = {}
+    for (kl, name, n_in, n_pre, n_kept, passes, e0, e1, e2) in per_gate:
+        ta, tt = e0.elapsed_time(e1), e1.elapsed_time(e2)
+        d = classes.setdefault(kl, {"gates": 0, "n_in": 0, "apply_ms": 0.0, "trunc_ms": 0.0, "apply_bytes": 0.0, "trunc_bytes": 0.0, "passes": 0})
+        d["gates"] += 1; d["n_in"] += n_in; d["apply_ms"] += ta; d["trunc_ms"] += tt; d["passes"] += passes
+        d["apply_bytes"] += 24.0 * (n_in + n_pre); d["trunc_bytes"] += 24.0 * (n_pre + n_kept)
+        if log:
+            log.write(json.dumps({"class": kl, "gate": name, "n_in": n_in, "n_pre": n_pre, "n_kept": n_kept, "passes": passes,
+                                  "apply_ms": ta, "trunc_ms": tt}) + "\n")
+    per_class = {}
+    for kl, d in classes.items():
+        per_class[kl] = {
+            "gates": d["gates"], "mean_passes": d["passes"] / d["gates"],
+            "apply_terms_per_s": d["n_in"] / (d["apply_ms"] * 1e-3) if d["apply_ms"] > 0 else None,
+            "apply_roofline_frac_of_8TBs": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / 8.0e12 if d["apply_ms"] > 0 else None,
+            "apply_roofline_frac_of_measured": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / (hbm * 1e9) if d["apply_ms"] > 0 else None,
+            "trunc_roofline_frac_of_measured": d["trunc_bytes"] / (d["trunc_ms"] * 1e-3) / (hbm * 1e9) if d["trunc_ms"] > 0 else None,
+            "apply_ms_mean": d["apply_ms"] / d["gates"], "trunc_ms_mean": d["trunc_ms"] / d["gates"]}
+
+    dom = max(prof, key=lambda k: prof[k]["ms"])
+    dk = prof[dom]
+    ach = dk["alg_bytes"] / (dk["ms"] * 1e-3) / 1e9 if dk["ms"] > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
+                "traffic": None, "peak_kind": peak_kind, "launches": dk["launches"],
+                "avg_launch_ms": dk["ms"] / max(dk["launches"], 1),
+                "alg_bytes_per_launch": dk["alg_bytes"] / max(dk["launches"], 1),
+                "kernels": {k: {"ms": v["ms"], "launches": v["launches"],
+                                "GBs": (v["alg_bytes"] / (v["ms"] * 1e-3) / 1e9) if v["ms"] > 0 else None} for k, v in prof.items()}}
+
+    # ---- e2e: host state in, top-k out, through the same C ABI ----
+    e2e = None
+    if not args.no_e2e:
+        n_state = sv.num_terms()
+        hk, ha, _ = sv.export()                       # untimed: the step's input, on the host
+        tk = torch.from_numpy(hk.view(np.int64)).pin_memory()
+        ta = torch.from_numpy(ha).pin_memory()
+        hk_p, ha_p = tk.numpy().view(np.uint64), ta.numpy()
+        g_start = gi
+        e_terms, e_ms, e_steps = 0, 0.0, max(1, min(args.steps, 3))
+        d2h = 0
+        for s in range(1 + e_steps):
+            gi = g_start
+            dist.barrier(); torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record()
+            sv.load(hk_p, ha_p)                       # H2D of this step's input state (pinned)
+            nt = one_step(False)
+            topk = sv.top(16)                         # D2H of the step's result
+            b.record(); torch.cuda.synchronize()
+            if s >= 1:
+                e_ms += a.elapsed_time(b)
+                e_terms += nt
+            d2h = int(topk[0].nbytes + topk[1].nbytes + topk[2].nbytes)
+        et, em = dist.aggregate(e_terms, e_ms, dev)
+        e2e = {"value": et / (em * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(hk_p.nbytes + ha_p.nbytes + G * 16 * 64),
+               "d2h_bytes_per_step": d2h, "steps": e_steps,
+               "note": "sv_load(host pinned state) + %d x (sv_apply_gate + sv_truncate) + sv_top(16); same gates every step" % G}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_sample(16, G, 2, 0, budget_s=args.cpu_seconds)
+        for k in ("steps_done", "ms_per_step"):
+            cpu.pop(k, None)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": tot_terms / (max_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "cfg5", "n_qubits": c.n, "K_log2": args.k_log2, "min_mass": c.min_mass,
+                           "gates_per_step": G, "capacity_terms": cap_mult * K, "ramp_gates": ramp_gates,
+                           "l2": "inputs larger than L2 (state %.2f GB)" % (24.0 * K / 1e9),
+                           "parallelism": "replicas x%d" % world},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
+                "per_class": per_class, "circuit_ms_per_gate": max_ms / (args.steps * G)}
+        print(json.dumps(line), flush=True)
+    if log:
+        log.close()
+    sv.close()
+    dist.shutdown()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

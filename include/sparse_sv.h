@@ -109,6 +109,17 @@ int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amp
 /* Statistics of the last call and the launch counter. */
 int sv_get_stats(sv_state *s, sv_stats *out);
 
+/* Optional per-kernel timing.  sv_profile(s, 1) resets the counters and makes every later
+ * launch of the main kernels be bracketed by CUDA events on the state's stream;
+ * sv_profile_get synchronises and returns, for one kernel, the summed device time, the
+ * number of launches and the ALGORITHMIC bytes they had to move (DESIGN.md "Kernels":
+ * diagonal 40 B/term; bit move 48 B/term; group 24 B x (N_in + N_out); select histogram
+ * 16 B/term; compaction 24 B x (N_in + N_kept)). */
+enum { SV_K_DIAG = 0, SV_K_MOVE = 1, SV_K_GROUP = 2, SV_K_SELHIST = 3, SV_K_COMPACT = 4, SV_K_COUNT = 5 };
+typedef struct { double ms; uint64_t launches; double alg_bytes; } sv_kernel_prof;
+int sv_profile(sv_state *s, int enable);
+int sv_profile_get(sv_state *s, int kernel, sv_kernel_prof *out);
+
 /* Device-side structural check (tests): keys strictly ascending in the engine's storage
  * order, all below 2^n_qubits, no stored exact zero.  *ok = 1 if all hold. */
 int sv_check_invariants(sv_state *s, int *ok);

@@ -37,7 +37,36 @@ struct sv_state {
     unsigned char* pinned;   // host, for small read-backs
     sv_stats stats;
     char err[256];
+    // optional per-kernel timing (sv_profile): CUDA events around the main kernels
+    bool prof_on;
+    int npend;
+    struct { int id; double bytes; } pend[64];
+    cudaEvent_t evpool[128];
+    bool ev_ready;
+    sv_kernel_prof prof[SV_K_COUNT];
 };
+
+static void prof_drain(sv_state* s) {
+    if (!s->npend) return;
+    cudaStreamSynchronize(s->stream);
+    for (int i = 0; i < s->npend; ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, s->evpool[2 * i], s->evpool[2 * i + 1]) == cudaSuccess) {
+            sv_kernel_prof& k = s->prof[s->pend[i].id];
+            k.ms += ms; k.launches += 1; k.alg_bytes += s->pend[i].bytes;
+        }
+    }
+    s->npend = 0;
+}
+// Reserve an event pair for one launch of kernel `id` moving `bytes` algorithmic bytes.
+static void prof_slot(sv_state* s, int id, double bytes, cudaEvent_t* e0, cudaEvent_t* e1) {
+    *e0 = *e1 = nullptr;
+    if (!s->prof_on) return;
+    if (s->npend == 64) prof_drain(s);
+    s->pend[s->npend].id = id; s->pend[s->npend].bytes = bytes;
+    *e0 = s->evpool[2 * s->npend]; *e1 = s->evpool[2 * s->npend + 1];
+    s->npend += 1;
+}
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
@@ -161,6 +190,7 @@ extern "C" int sv_create_in_arena(int n_qubits, uint64_t capacity, void* dev_are
 extern "C" void sv_destroy(sv_state* s) {
     if (!s) return;
     cudaStreamSynchronize(s->stream);
+    if (s->ev_ready) for (int i = 0; i < 128; ++i) cudaEventDestroy(s->evpool[i]);
     if (s->pinned) cudaFreeHost(s->pinned);
     if (s->own_mem && s->arena) cudaFree(s->arena);
     if (s->own_stream && s->stream) cudaStreamDestroy(s->stream);
@@ -176,6 +206,23 @@ extern "C" int sv_num_terms(sv_state* s, uint64_t* n) {
     if (!s || !n) return SV_ERR_INVALID_ARG;
     CU(cudaStreamSynchronize(s->stream));
     *n = s->count;
+    return SV_OK;
+}
+extern "C" int sv_profile(sv_state* s, int enable) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    prof_drain(s);
+    if (enable && !s->ev_ready) {
+        for (int i = 0; i < 128; ++i) CU(cudaEventCreate(&s->evpool[i]));
+        s->ev_ready = true;
+    }
+    memset(s->prof, 0, sizeof(s->prof));
+    s->prof_on = enable != 0;
+    return SV_OK;
+}
+extern "C" int sv_profile_get(sv_state* s, int kernel, sv_kernel_prof* out) {
+    if (!s || !out || kernel < 0 || kernel >= SV_K_COUNT) return SV_ERR_INVALID_ARG;
+    prof_drain(s);
+    *out = s->prof[kernel];
     return SV_OK;
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
@@ -255,7 +302,11 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.gate_class = xor_class ? SV_CLASS_XOR : SV_CLASS_DIAGONAL;
         if (!unit_phase) {
             CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
+            cudaEvent_t e0, e1;
+            prof_slot(s, SV_K_DIAG, 40.0 * (double)s->count, &e0, &e1);
+            if (e0) cudaEventRecord(e0, s->stream);
             s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->count, s->tab, s->stream);
+            if (e1) cudaEventRecord(e1, s->stream);
             CHECK_LAUNCH();
             s->stats.passes = 1;
         }
@@ -279,7 +330,9 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;
         const int alt = s->cur ^ 1;
-        s->stats.launches += svk_move(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, p, s->desc, s->stream);
+        cudaEvent_t e0, e1;
+        prof_slot(s, SV_K_MOVE, 48.0 * (double)s->count, &e0, &e1);
+        s->stats.launches += svk_move(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, p, s->desc, s->stream, e0, e1);
         CHECK_LAUNCH();
         s->cur = alt;
         layout_move(s, p);
@@ -313,13 +366,17 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
             }
     CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
     const int alt = s->cur ^ 1;
+    cudaEvent_t ge0, ge1;
+    prof_slot(s, SV_K_GROUP, 0.0, &ge0, &ge1);
+    const int gslot = s->npend - 1;
     s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, plast, ma,
-                                   s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream);
+                                   s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
     CHECK_LAUNCH();
     s->stats.passes += 1;
     u64 nout = 0;
     int rc = read_back(s, &nout, s->d_count, sizeof(u64));
     if (rc != SV_OK) return rc;
+    if (ge0) s->pend[gslot].bytes = 24.0 * ((double)s->count + (double)(nout > s->cap ? s->cap : nout));
     if (nout > s->cap) {
         s->stats.n_out = nout;
         return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
@@ -339,7 +396,11 @@ static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out
     s->stats.launches += svk_sel_init(s->sel, s->count, max_terms, min_mass, s->stream);
     const int max_levels = 6 + (s->n + 11) / 12 + 1;
     for (int it = 0; it < max_levels; ++it) {
+        cudaEvent_t e0, e1;
+        prof_slot(s, SV_K_SELHIST, 16.0 * (double)s->count, &e0, &e1);
+        if (e0) cudaEventRecord(e0, s->stream);
         s->stats.launches += svk_sel_hist(s->keys[s->cur], s->amps[s->cur], s->count, s->sel, km, s->n, s->hist, s->stream);
+        if (e1) cudaEventRecord(e1, s->stream);
         s->stats.launches += svk_sel_step(s->sel, s->hist, s->n, s->stream);
         CHECK_LAUNCH();
         s->stats.passes += 1;
@@ -364,8 +425,12 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     if (rc != SV_OK) return rc;
     if (ss.final_count >= s->count) return SV_OK;   // nothing dropped: bitwise no-op (reading R7)
     const int alt = s->cur ^ 1;
+    cudaEvent_t ce0, ce1;
+    prof_slot(s, SV_K_COMPACT, 24.0 * ((double)s->count + (double)ss.final_count), &ce0, &ce1);
+    if (ce0) cudaEventRecord(ce0, s->stream);
     s->stats.launches += svk_compact(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, s->sel,
                                      keymap_of(s), 1, s->status, s->tile_counter, s->d_count, s->stream);
+    if (ce1) cudaEventRecord(ce1, s->stream);
     CHECK_LAUNCH();
     s->stats.passes += 1;
     u64 nout = 0;

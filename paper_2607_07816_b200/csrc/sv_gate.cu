@@ -232,14 +232,16 @@ static int launch_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u3
 }
 
 int svk_move(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, TileDesc* desc,
-             cudaStream_t st) {
+             cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
     if (n == 0) return 0;
     const u32 ntiles = (u32)((n + SV_MOVE_TILE - 1) / SV_MOVE_TILE);
     int l = launch_find_splits(kin, n, p, -1, SV_MOVE_TILE, ntiles, desc, st);
     const size_t smem = (size_t)SV_MOVE_TILE * (16 + 8 + 2) + (SV_MOVE_TILE + 2) * 2;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(move_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    if (e0) cudaEventRecord(e0, st);
     move_kernel<<<ntiles, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, desc);
+    if (e1) cudaEventRecord(e1, st);
     return l + 1;
 }
 
@@ -410,7 +412,7 @@ static void launch_group(const u64* kin, const double2* ain, u64* kout, double2*
 
 int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
               const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count, u64 cap,
-              cudaStream_t st) {
+              cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
     int launches = 0;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 tnom = (u32)((SV_TILE_SLOTS >> ma) - (1 << ma));
@@ -419,6 +421,7 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
     cudaMemsetAsync(tile_counter, 0, sizeof(u32), st);
     const bool mv = p >= 0;
     if (mv) launches += launch_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
+    if (e0) cudaEventRecord(e0, st);
 #define SV_LG(MA_) \
     if (mv) launch_group<MA_, true>(kin, ain, kout, aout, n, p, tab, desc, status, tile_counter, d_count, cap, ntiles, st); \
     else launch_group<MA_, false>(kin, ain, kout, aout, n, p, tab, desc, status, tile_counter, d_count, cap, ntiles, st);
@@ -430,5 +433,6 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
         default: SV_LG(4) break;
     }
 #undef SV_LG
+    if (e1) cudaEventRecord(e1, st);
     return launches + 1;
 }

@@ -59,13 +59,13 @@ struct KeyMap {          // stored (physical) key -> logical key
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
 
 int svk_move(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p,
-             TileDesc* desc, cudaStream_t st);
+             TileDesc* desc, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 
 // Final pass of a group gate.  p < 0: the active bits already sit at the LSBs (no move).
 // Writes the output term count to *d_count (may exceed cap: then nothing past cap is written).
 int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
               const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count,
-              u64 cap, cudaStream_t st);
+              u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 
 int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
 

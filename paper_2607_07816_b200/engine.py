@@ -18,12 +18,17 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
-           "sv_check_invariants", "sv_last_error", "sv_sync"]
+           "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get"]
+KERNELS = ["diag", "move", "group", "sel_hist", "compact"]
 
 
 class SvStats(C.Structure):
     _fields_ = [("gate_class", C.c_int), ("m", C.c_int), ("active_bits", C.c_int), ("passes", C.c_int),
                 ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64)]
+
+
+class SvKernelProf(C.Structure):
+    _fields_ = [("ms", C.c_double), ("launches", C.c_uint64), ("alg_bytes", C.c_double)]
 
 
 class SvError(RuntimeError):
@@ -68,6 +73,10 @@ def load_library(path: str = _LIBPATH):
     lib.sv_last_error.argtypes = [vp]
     lib.sv_sync.restype = i32
     lib.sv_sync.argtypes = [vp]
+    lib.sv_profile.restype = i32
+    lib.sv_profile.argtypes = [vp, i32]
+    lib.sv_profile_get.restype = i32
+    lib.sv_profile_get.argtypes = [vp, i32, C.POINTER(SvKernelProf)]
     return lib
 
 
@@ -174,6 +183,17 @@ class SparseSV:
         ok = C.c_int(0)
         self._chk(lib.sv_check_invariants(self._h, C.byref(ok)))
         return bool(ok.value)
+
+    def profile(self, enable: bool = True):
+        self._chk(lib.sv_profile(self._h, 1 if enable else 0))
+
+    def profile_get(self) -> dict:
+        out = {}
+        for i, name in enumerate(KERNELS):
+            kp = SvKernelProf()
+            self._chk(lib.sv_profile_get(self._h, i, C.byref(kp)))
+            out[name] = {"ms": kp.ms, "launches": int(kp.launches), "alg_bytes": kp.alg_bytes}
+        return out
 
     def sync(self):
         self._chk(lib.sv_sync(self._h))
