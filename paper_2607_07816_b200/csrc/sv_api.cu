@@ -19,7 +19,9 @@ struct sv_state {
     u64* keys[2];
     double2* amps[2];
     int cur;
-    u64 count;
+    u64 count;   // logical number of terms
+    u64 phys;    // stored entries in the current buffers (> count while a truncation is deferred)
+    PendPred defer;   // truncation whose compaction is left to the next reader of the state
     // physical layout: stored bit phys_of_log[q] holds logical qubit q (XOR the lazy X mask)
     int phys_of_log[64];
     u64 xmask;   // in physical positions
@@ -129,7 +131,8 @@ extern "C" size_t sv_arena_bytes(uint64_t capacity) { return layout_for(capacity
 
 static int init_state(sv_state* s) {
     s->cur = 0;
-    s->count = 1;
+    s->count = 1; s->phys = 1;
+    s->defer.active = 0;
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     const u64 k0 = 0;
@@ -238,6 +241,25 @@ static int read_back(sv_state* s, void* dst, const void* dsrc, size_t bytes) {
     return SV_OK;
 }
 
+// Apply a deferred truncation now (one compaction pass).  Readers that cannot fuse the
+// predicate into their own load call this first.
+static int materialize(sv_state* s) {
+    if (!s->defer.active) return SV_OK;
+    const int alt = s->cur ^ 1;
+    cudaEvent_t e0, e1;
+    prof_slot(s, SV_K_COMPACT, 24.0 * ((double)s->phys + (double)s->count), &e0, &e1);
+    if (e0) cudaEventRecord(e0, s->stream);
+    s->stats.launches += svk_compact(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, s->defer,
+                                     s->status, s->tile_counter, s->d_count, s->stream);
+    if (e1) cudaEventRecord(e1, s->stream);
+    CHECK_LAUNCH();
+    s->stats.passes += 1;
+    s->cur = alt;
+    s->phys = s->count;
+    s->defer.active = 0;
+    return SV_OK;
+}
+
 // ---------------------------------------------------------------------------------------
 // sv_apply_gate: classify (row a-1), plan the bit moves, launch
 // ---------------------------------------------------------------------------------------
@@ -303,10 +325,20 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         if (!unit_phase) {
             CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
             cudaEvent_t e0, e1;
-            prof_slot(s, SV_K_DIAG, 40.0 * (double)s->count, &e0, &e1);
-            if (e0) cudaEventRecord(e0, s->stream);
-            s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->count, s->tab, s->stream);
-            if (e1) cudaEventRecord(e1, s->stream);
+            if (s->defer.active) {   // truncate-then-diagonal in one out-of-place pass
+                const int alt = s->cur ^ 1;
+                prof_slot(s, SV_K_DIAG, 24.0 * ((double)s->phys + (double)s->count), &e0, &e1);
+                if (e0) cudaEventRecord(e0, s->stream);
+                s->stats.launches += svk_diag_compact(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys,
+                                                      s->tab, s->defer, s->status, s->tile_counter, s->d_count, s->stream);
+                if (e1) cudaEventRecord(e1, s->stream);
+                s->cur = alt; s->phys = s->count; s->defer.active = 0;
+            } else {
+                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->count, &e0, &e1);
+                if (e0) cudaEventRecord(e0, s->stream);
+                s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->count, s->tab, s->stream);
+                if (e1) cudaEventRecord(e1, s->stream);
+            }
             CHECK_LAUNCH();
             s->stats.passes = 1;
         }
@@ -332,9 +364,12 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         const int alt = s->cur ^ 1;
         cudaEvent_t e0, e1;
         prof_slot(s, SV_K_MOVE, 48.0 * (double)s->count, &e0, &e1);
-        s->stats.launches += svk_move(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, p, s->desc, s->stream, e0, e1);
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, p, 0, nullptr,
+                                         s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, e0, e1);
         CHECK_LAUNCH();
         s->cur = alt;
+        s->phys = s->count;      // a deferred truncation has been applied by the pass
+        s->defer.active = 0;
         layout_move(s, p);
         s->stats.passes += 1;
     }
@@ -369,8 +404,15 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     cudaEvent_t ge0, ge1;
     prof_slot(s, SV_K_GROUP, 0.0, &ge0, &ge1);
     const int gslot = s->npend - 1;
-    s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, plast, ma,
-                                   s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+    if (ma == 1) {   // one active bit: the lean pass (p = 0 when the bit already sits at the LSB)
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, s->tab,
+                                         s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+    } else {
+        if (s->defer.active) { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
+        const int alt2 = s->cur ^ 1;
+        s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt2], s->amps[alt2], s->count, plast, ma,
+                                       s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+    }
     CHECK_LAUNCH();
     s->stats.passes += 1;
     u64 nout = 0;
@@ -382,8 +424,9 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
     }
     if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; }
-    s->cur = alt;
-    s->count = nout;
+    s->cur ^= 1;
+    s->count = nout; s->phys = nout;
+    s->defer.active = 0;
     s->stats.n_out = nout;
     return SV_OK;
 }
@@ -420,32 +463,24 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     if (kept_fraction) *kept_fraction = 1.0;
     const bool needK = max_terms != 0 && max_terms < s->count, needM = min_mass < 1.0;
     if (s->count == 0 || (!needK && !needM)) return SV_OK;
+    int rc = materialize(s);   // a second truncation in a row: apply the first one now
+    if (rc != SV_OK) return rc;
     SelState ss;
-    int rc = run_select(s, max_terms, min_mass, &ss);
+    rc = run_select(s, max_terms, min_mass, &ss);
     if (rc != SV_OK) return rc;
     if (ss.final_count >= s->count) return SV_OK;   // nothing dropped: bitwise no-op (reading R7)
-    const int alt = s->cur ^ 1;
-    cudaEvent_t ce0, ce1;
-    prof_slot(s, SV_K_COMPACT, 24.0 * ((double)s->count + (double)ss.final_count), &ce0, &ce1);
-    if (ce0) cudaEventRecord(ce0, s->stream);
-    s->stats.launches += svk_compact(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->count, s->sel,
-                                     keymap_of(s), 1, s->status, s->tile_counter, s->d_count, s->stream);
-    if (ce1) cudaEventRecord(ce1, s->stream);
-    CHECK_LAUNCH();
-    s->stats.passes += 1;
-    u64 nout = 0;
-    rc = read_back(s, &nout, s->d_count, sizeof(u64));
-    if (rc != SV_OK) return rc;
-    if (nout != ss.final_count) return fail(s, SV_ERR_CUDA, "internal: compaction count differs from select count");
-    s->cur = alt;
-    s->count = nout;
-    s->stats.n_out = nout;
+    // The cut is decided; the compaction + renormalisation is left to the next reader of the
+    // state (the next gate's load applies it for free), or to materialize().
+    s->defer.active = 1; s->defer.PT = ss.PT; s->defer.KT = ss.KT; s->defer.scale = ss.scale; s->defer.km = keymap_of(s);
+    s->count = ss.final_count;
+    s->stats.n_out = ss.final_count;
     if (kept_fraction) *kept_fraction = ss.kept_fraction;
     return SV_OK;
 }
 
 extern "C" int sv_norm(sv_state* s, double* mass) {
     if (!s || !mass) return SV_ERR_INVALID_ARG;
+    { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
     s->stats.launches += svk_norm(s->amps[s->cur], s->count, s->partials, s->d_norm, s->stream);
     CHECK_LAUNCH();
     return read_back(s, mass, s->d_norm, sizeof(double));
@@ -453,6 +488,7 @@ extern "C" int sv_norm(sv_state* s, double* mass) {
 
 extern "C" int sv_check_invariants(sv_state* s, int* ok) {
     if (!s || !ok) return SV_ERR_INVALID_ARG;
+    { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
     s->stats.launches += svk_check(s->keys[s->cur], s->amps[s->cur], s->count, s->n, s->d_bad, s->stream);
     CHECK_LAUNCH();
     int bad = 0;
@@ -474,6 +510,7 @@ struct TmpBuf {
 extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, double* probs, uint64_t* n_written) {
     if (!s) return SV_ERR_INVALID_ARG;
     s->err[0] = 0;
+    { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
     const u64 kk = k < s->count ? k : s->count;
     if (n_written) *n_written = kk;
     if (kk == 0) return SV_OK;
@@ -569,7 +606,8 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
         if (bad) return fail(s, SV_ERR_INVALID_ARG, "sv_load: duplicate key, key >= 2^n or zero amplitude (state unchanged)");
     }
     s->cur = alt;
-    s->count = n;
+    s->count = n; s->phys = n;
+    s->defer.active = 0;
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     s->stats.n_in = n; s->stats.n_out = n; s->stats.gate_class = SV_CLASS_NONE;

@@ -224,8 +224,7 @@ __global__ void __launch_bounds__(SV_THREADS) move_kernel(const u64* __restrict_
     }
 }
 
-static int launch_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc,
-                              cudaStream_t st) {
+int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st) {
     const u32 nb = (ntiles + 1 + 127) / 128;
     find_splits_kernel<<<nb, 128, 0, st>>>(keys, n, p, w, tnom, ntiles, desc);
     return 1;
@@ -235,7 +234,7 @@ int svk_move(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n
              cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
     if (n == 0) return 0;
     const u32 ntiles = (u32)((n + SV_MOVE_TILE - 1) / SV_MOVE_TILE);
-    int l = launch_find_splits(kin, n, p, -1, SV_MOVE_TILE, ntiles, desc, st);
+    int l = svk_find_splits(kin, n, p, -1, SV_MOVE_TILE, ntiles, desc, st);
     const size_t smem = (size_t)SV_MOVE_TILE * (16 + 8 + 2) + (SV_MOVE_TILE + 2) * 2;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(move_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
@@ -420,7 +419,7 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
     cudaMemsetAsync(status, 0, (size_t)ntiles * sizeof(u64), st);
     cudaMemsetAsync(tile_counter, 0, sizeof(u32), st);
     const bool mv = p >= 0;
-    if (mv) launches += launch_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
+    if (mv) launches += svk_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
 #define SV_LG(MA_) \
     if (mv) launch_group<MA_, true>(kin, ain, kout, aout, n, p, tab, desc, status, tile_counter, d_count, cap, ntiles, st); \

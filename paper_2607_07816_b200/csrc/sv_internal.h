@@ -55,6 +55,16 @@ struct KeyMap {          // stored (physical) key -> logical key
     u64 xmask;                        // lazy X mask in physical positions
 };
 
+// A truncation whose compaction has been deferred to the next reader of the state: a term
+// survives iff pat > PT || (pat == PT && (KT == ~0 || logical key <= KT)); survivors are
+// multiplied by `scale`.  active == 0: nothing pending.
+struct PendPred {
+    int active;
+    u64 PT, KT;
+    double scale;
+    KeyMap km;
+};
+
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
 
@@ -67,6 +77,18 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
               const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count,
               u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 
+// Lean single-bit pass (sv_pair.cu): moves physical bit p to the LSB in one streaming pass.
+// pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
+// pair == 0: pure move.  A pending truncation is applied while loading.  Writes the output
+// count to *d_count.
+int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair,
+                const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
+                u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
+int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
+// Diagonal gate fused with a pending truncation (out of place, compacting).
+int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
+                     const PendPred& pend, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
+
 int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
 
 int svk_sel_init(SelState* ss, u64 n, u64 max_terms, double min_mass, cudaStream_t st);
@@ -74,8 +96,7 @@ int svk_sel_hist(const u64* keys, const double2* amps, u64 n, const SelState* ss
                  u64* hist, cudaStream_t st);
 int svk_sel_step(SelState* ss, u64* hist, int nq, cudaStream_t st);
 int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
-                const SelState* ss, KeyMap km, int do_scale, u64* status, u32* tile_counter,
-                u64* d_count, cudaStream_t st);
+                const PendPred& pd, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
 
 int svk_check(const u64* keys, const double2* amps, u64 n, int nq, int* d_bad, cudaStream_t st);
 

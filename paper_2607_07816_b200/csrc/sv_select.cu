@@ -329,19 +329,29 @@ __device__ __forceinline__ bool sel_keep(u64 pat, u64 stored_key, u64 PT, u64 KT
 }
 
 #define SV_CMP_IT 8
+// DIAG: a diagonal gate (phase table in gtab, see diag_kernel) is applied to the survivors
+// in the same pass -- "truncate, then diagonal gate" costs one read and one write.
+template <bool DIAG>
 __global__ void __launch_bounds__(SV_THREADS) compact_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                              u64* __restrict__ kout, double2* __restrict__ aout, u64 n,
-                                                             const SelState* __restrict__ ssp, KeyMap km, int do_scale,
+                                                             PendPred pd, const GateTab* __restrict__ gtab,
                                                              u64* status, u32* tile_counter, u64* d_count, u32 ntiles) {
     __shared__ int wcnt[SV_CMP_IT][SV_THREADS / 32];
     __shared__ u32 s_tile;
     __shared__ u64 s_base;
+    __shared__ double2 sd[16];
+    __shared__ int s_cpos[SV_MAX_M], s_mc;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
+    if (DIAG) {
+        if (tid < 16) sd[tid] = gtab->U[tid];
+        if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
+        if (tid == 0) s_mc = gtab->mc;
+    }
     __syncthreads();
     const u32 tile = s_tile;
-    const u64 PT = ssp->PT, KT = ssp->KT;
-    const double scale = do_scale ? ssp->scale : 1.0;
+    const u64 PT = pd.PT, KT = pd.KT;
+    const double scale = pd.scale;
     const u64 t0 = (u64)tile * (SV_THREADS * SV_CMP_IT);
     u64 k[SV_CMP_IT]; double2 a[SV_CMP_IT]; u32 ball[SV_CMP_IT];
 #pragma unroll
@@ -350,46 +360,71 @@ __global__ void __launch_bounds__(SV_THREADS) compact_kernel(const u64* __restri
         if (i < n) { k[it] = ld_stream_u64(kin + i); a[it] = ld_stream_d2(ain + i); }
         else { k[it] = 0; a[it].x = 0.0; a[it].y = 0.0; }
     }
+    int tot = 0;
 #pragma unroll
     for (int it = 0; it < SV_CMP_IT; ++it) {
         const u64 i = t0 + (u64)it * SV_THREADS + tid;
         bool keep = false;
-        if (i < n) keep = sel_keep((u64)__double_as_longlong(prob_of(a[it])), k[it], PT, KT, km);
+        if (i < n) keep = sel_keep((u64)__double_as_longlong(prob_of(a[it])), k[it], PT, KT, pd.km);
         const u32 b = __ballot_sync(0xffffffffu, keep);
         ball[it] = b;
         if (lane == 0) wcnt[it][warp] = __popc(b);
     }
     __syncthreads();
-    if (tid == 0) {
-        int run = 0;
-        for (int it = 0; it < SV_CMP_IT; ++it)
-            for (int w = 0; w < SV_THREADS / 32; ++w) { const int c = wcnt[it][w]; wcnt[it][w] = run; run += c; }
-        const u64 excl = lookback_exclusive(status, tile, (u64)run);
-        s_base = excl;
-        if (tile == ntiles - 1) *d_count = excl + (u64)run;
+    if (tid < 32) {   // exclusive offsets of the IT x 8 warp counts (one per lane pair), tile total, look-back
+        int c0 = 0, c1 = 0;
+        const int e0 = 2 * lane, e1 = 2 * lane + 1;   // 64 entries, row-major [it][warp]
+        c0 = wcnt[e0 >> 3][e0 & 7]; c1 = wcnt[e1 >> 3][e1 & 7];
+        int inc = c0 + c1;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+        tot = __shfl_sync(0xffffffffu, inc, 31);
+        const int ex = inc - c0 - c1;
+        __syncwarp();
+        wcnt[e0 >> 3][e0 & 7] = ex; wcnt[e1 >> 3][e1 & 7] = ex + c0;
+        const u64 excl = lookback_exclusive_warp(status, tile, (u64)tot);
+        if (lane == 0) { s_base = excl; if (tile == ntiles - 1) *d_count = excl + (u64)tot; }
     }
     __syncthreads();
     const u64 base = s_base;
+    const int mc = DIAG ? s_mc : 0;
 #pragma unroll
     for (int it = 0; it < SV_CMP_IT; ++it) {
         if ((ball[it] >> lane) & 1u) {
             const u64 pos = base + (u64)wcnt[it][warp] + (u64)__popc(ball[it] & ((1u << lane) - 1u));
             st_stream_u64(kout + pos, k[it]);
             double2 o; o.x = __dmul_rn(a[it].x, scale); o.y = __dmul_rn(a[it].y, scale);
+            if (DIAG) {
+                int cx = 0;
+                for (int j = 0; j < mc; ++j) cx |= (int)((k[it] >> s_cpos[j]) & 1ull) << j;
+                const double2 u = sd[cx];
+                double2 r;
+                r.x = __dsub_rn(__dmul_rn(u.x, o.x), __dmul_rn(u.y, o.y));
+                r.y = __dadd_rn(__dmul_rn(u.x, o.y), __dmul_rn(u.y, o.x));
+                o = r;
+            }
             st_stream_d2(aout + pos, o);
         }
     }
 }
 
-int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const SelState* ss, KeyMap km,
-                int do_scale, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st) {
+static int launch_compact(bool diag, const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const PendPred& pd,
+                          const GateTab* tab, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st) {
     if (n == 0) return 0;
     const u32 ntiles = (u32)((n + SV_THREADS * SV_CMP_IT - 1) / (SV_THREADS * SV_CMP_IT));
     cudaMemsetAsync(status, 0, (size_t)ntiles * sizeof(u64), st);
     cudaMemsetAsync(tile_counter, 0, sizeof(u32), st);
-    compact_kernel<<<ntiles, SV_THREADS, 0, st>>>(kin, ain, kout, aout, n, ss, km, do_scale, status, tile_counter,
-                                                  d_count, ntiles);
+    if (diag) compact_kernel<true><<<ntiles, SV_THREADS, 0, st>>>(kin, ain, kout, aout, n, pd, tab, status, tile_counter, d_count, ntiles);
+    else compact_kernel<false><<<ntiles, SV_THREADS, 0, st>>>(kin, ain, kout, aout, n, pd, tab, status, tile_counter, d_count, ntiles);
     return 1;
+}
+int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const PendPred& pd, u64* status,
+                u32* tile_counter, u64* d_count, cudaStream_t st) {
+    return launch_compact(false, kin, ain, kout, aout, n, pd, nullptr, status, tile_counter, d_count, st);
+}
+int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
+                     const PendPred& pend, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st) {
+    return launch_compact(true, kin, ain, kout, aout, n, pend, tab, status, tile_counter, d_count, st);
 }
 
 // ---------------------------------------------------------------------------------------
