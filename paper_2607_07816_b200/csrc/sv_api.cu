@@ -36,6 +36,8 @@ struct sv_state {
     int* d_bad;
     double* partials;
     double* d_norm;
+    u64* lut;          // device, 8 x 256: stored -> logical key tables of the current layout
+    bool lut_valid;
     unsigned char* pinned;   // host, for small read-backs
     sv_stats stats;
     char err[256];
@@ -73,18 +75,19 @@ static void prof_slot(sv_state* s, int id, double bytes, cudaEvent_t* e0, cudaEv
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
 
-struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, total; };
+struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, total; };
 static ArenaLayout layout_for(u64 cap) {
     ArenaLayout L; size_t o = 0;
     for (int i = 0; i < 2; ++i) { L.keys[i] = o; o += align_up(cap * 8); }
     for (int i = 0; i < 2; ++i) { L.amps[i] = o; o += align_up(cap * 16); }
     L.desc = o; o += align_up(desc_entries(cap) * sizeof(TileDesc));
     L.status = o; o += align_up(desc_entries(cap) * 8);
-    L.hist = o; o += align_up(3 * SV_SEL_BINS * 8);
+    L.hist = o; o += align_up(3 * SV_SEL_BINS * 8);   // >= the select's 5 x 2048 + 8 words
     L.sel = o; o += align_up(sizeof(SelState));
     L.tab = o; o += align_up(sizeof(GateTab));
     L.misc = o; o += 256;
     L.partials = o; o += align_up(1024 * 8 + 8);
+    L.lut = o; o += align_up(8 * 256 * 8);
     L.total = o;
     return L;
 }
@@ -108,16 +111,31 @@ static int cuda_fail(sv_state* s, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail(s, e__, "kernel launch"); \
     } while (0)
 
-static KeyMap keymap_of(const sv_state* s) {
-    KeyMap km;
-    memset(km.log_of_phys, 0xff, sizeof(km.log_of_phys));
-    for (int q = 0; q < s->n; ++q) km.log_of_phys[s->phys_of_log[q]] = (unsigned char)q;
-    km.xmask = s->xmask;
+// Builds (if the layout changed) and uploads the stored -> logical key tables.
+static KeyMap keymap_of(sv_state* s) {
+    if (!s->lut_valid) {
+        static thread_local u64 h[8 * 256];
+        u64 col[64];
+        for (int p = 0; p < 64; ++p) col[p] = 0;
+        for (int q = 0; q < s->n; ++q) col[s->phys_of_log[q]] = 1ull << q;
+        u64 xl = 0;
+        for (int p = 0; p < 64; ++p) if ((s->xmask >> p) & 1ull) xl ^= col[p];
+        for (int b = 0; b < 8; ++b)
+            for (int v = 0; v < 256; ++v) {
+                u64 o = (b == 0) ? xl : 0;
+                for (int j = 0; j < 8; ++j) if ((v >> j) & 1) o ^= col[8 * b + j];
+                h[b * 256 + v] = o;
+            }
+        cudaMemcpyAsync(s->lut, h, sizeof(h), cudaMemcpyHostToDevice, s->stream);
+        s->lut_valid = true;
+    }
+    KeyMap km; km.lut = s->lut;
     return km;
 }
 
 // move physical bit p to position 0 (bits below p shift up by one)
 static void layout_move(sv_state* s, int p) {
+    s->lut_valid = false;
     for (int q = 0; q < s->n; ++q) {
         if (s->phys_of_log[q] < p) s->phys_of_log[q] += 1;
         else if (s->phys_of_log[q] == p) s->phys_of_log[q] = 0;
@@ -133,6 +151,8 @@ static int init_state(sv_state* s) {
     s->cur = 0;
     s->count = 1; s->phys = 1;
     s->defer.active = 0;
+    s->lut_valid = false;
+    s->lut_valid = false;
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     const u64 k0 = 0;
@@ -174,6 +194,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->d_bad = (int*)(s->arena + L.misc + 128);
     s->d_norm = (double*)(s->arena + L.misc + 192);
     s->partials = (double*)(s->arena + L.partials);
+    s->lut = (u64*)(s->arena + L.lut);
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
         sv_destroy(s);
@@ -320,7 +341,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
             if (!(z.re == 1.0 && z.im == 0.0)) unit_phase = false;
         }
         if (xor_class)   // flip the lazy mask on the active bits: no data is touched
-            for (int i = 0; i < ma; ++i) s->xmask ^= 1ull << s->phys_of_log[qubits[active[i]]];
+            { for (int i = 0; i < ma; ++i) s->xmask ^= 1ull << s->phys_of_log[qubits[active[i]]]; s->lut_valid = false; }
         s->stats.gate_class = xor_class ? SV_CLASS_XOR : SV_CLASS_DIAGONAL;
         if (!unit_phase) {
             CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
@@ -423,7 +444,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.n_out = nout;
         return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
     }
-    if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; }
+    if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; s->lut_valid = false; }
     s->cur ^= 1;
     s->count = nout; s->phys = nout;
     s->defer.active = 0;
@@ -436,20 +457,29 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
 // ---------------------------------------------------------------------------------------
 static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
     const KeyMap km = keymap_of(s);
-    s->stats.launches += svk_sel_init(s->sel, s->count, max_terms, min_mass, s->stream);
-    const int max_levels = 6 + (s->n + 11) / 12 + 1;
-    for (int it = 0; it < max_levels; ++it) {
+    const u64 n = s->count;                   // callers have materialised any deferred truncation
+    u64* lk = s->keys[s->cur ^ 1];            // the idle buffer holds the extracted tie keys
+    s->stats.launches += svk_sel_init(s->sel, s->hist, n, max_terms, min_mass, s->stream);
+    int phase = 0;
+    u64 ties = 0;
+    for (int it = 0; it < 64; ++it) {
         cudaEvent_t e0, e1;
-        prof_slot(s, SV_K_SELHIST, 16.0 * (double)s->count, &e0, &e1);
+        const double bytes = phase <= 1 ? 16.0 * (double)n : (phase == 2 ? 16.0 * (double)n + 16.0 * (double)ties : 8.0 * (double)ties);
+        prof_slot(s, SV_K_SELHIST, bytes, &e0, &e1);
         if (e0) cudaEventRecord(e0, s->stream);
-        s->stats.launches += svk_sel_hist(s->keys[s->cur], s->amps[s->cur], s->count, s->sel, km, s->n, s->hist, s->stream);
+        if (phase <= 1) s->stats.launches += svk_sel_pass(phase, s->amps[s->cur], nullptr, n, s->sel, s->hist, s->stream);
+        else if (phase == 2) s->stats.launches += svk_sel_extract(s->keys[s->cur], s->amps[s->cur], n, s->sel, km, lk, s->hist, s->stream);
+        else s->stats.launches += svk_sel_pass(2, nullptr, lk, ties, s->sel, s->hist, s->stream);
         if (e1) cudaEventRecord(e1, s->stream);
-        s->stats.launches += svk_sel_step(s->sel, s->hist, s->n, s->stream);
+        s->stats.launches += svk_sel_step(s->sel, s->hist, s->stream);
         CHECK_LAUNCH();
         s->stats.passes += 1;
         int rc = read_back(s, out, s->sel, sizeof(SelState));
         if (rc != SV_OK) return rc;
-        if (out->done) return SV_OK;
+        if (out->done == 1) return SV_OK;
+        if (out->done != 0) return fail(s, SV_ERR_CUDA, "internal: radix select inconsistency");
+        phase = out->phase;
+        ties = out->tie_total;
     }
     return fail(s, SV_ERR_CUDA, "radix select did not converge");
 }
@@ -608,6 +638,7 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
     s->cur = alt;
     s->count = n; s->phys = n;
     s->defer.active = 0;
+    s->lut_valid = false;
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     s->stats.n_in = n; s->stats.n_out = n; s->stats.gate_class = SV_CLASS_NONE;

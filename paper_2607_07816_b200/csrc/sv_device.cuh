@@ -127,13 +127,10 @@ __device__ __forceinline__ double prob_of(double2 a) {  // p = re*re + im*im, no
     return __dadd_rn(__dmul_rn(a.x, a.x), __dmul_rn(a.y, a.y));
 }
 
-// stored (physical) key -> logical key: undo the lazy X mask, then the bit permutation.
+// stored (physical) key -> logical key (see KeyMap): eight cached table reads.
 __device__ __forceinline__ u64 logical_key(u64 stored, const KeyMap& km) {
-    u64 t = stored ^ km.xmask, out = 0;
-    while (t) {
-        int p = __ffsll((long long)t) - 1;
-        t &= t - 1;
-        out |= 1ull << km.log_of_phys[p];
-    }
+    u64 out = 0;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) out ^= __ldg(km.lut + b * 256 + (int)((stored >> (8 * b)) & 0xffull));
     return out;
 }

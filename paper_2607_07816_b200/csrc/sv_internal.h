@@ -31,28 +31,34 @@ struct TileDesc {
     u64 e;    // end of the block
 };
 
-// Radix-select state (device resident; one per handle).
+// Radix-select state (device resident; one per handle).  See sv_radix_select.cu.
 struct SelState {
-    u64 pat_prefix;      // resolved high bits of the cutoff probability pattern
-    u64 key_prefix;      // resolved high bits of the cutoff logical key (tie phase)
-    int level;           // next level to run: 0..5 = p levels, 6.. = key levels
-    int done;            // 1: PT/KT final
+    int phase;           // 0 exponent level, 1 adaptive pattern levels, 2 tie keys to be extracted, 3 key levels
+    int done;            // 1: PT/KT final; 2: internal inconsistency
     int count_active, mass_active;
-    u64 k_rem;           // terms still to take from the candidate bin (count criterion)
-    double mass_rem_hi, mass_rem_lo;   // mass still to collect (mass criterion), double-double
+    int E, pad_;         // exponent field shared by the candidates (mass scale)
+    u64 rmask, rval;     // resolved bits of the cutoff probability pattern
+    u64 dmask;           // bit positions forming the next pattern digit
+    u64 krmask, krval, kdmask;          // the same for the logical key among tied terms
+    u64 k_rem;           // terms still to take from the candidates (count criterion / ties)
+    double mass_rem_hi, mass_rem_lo;    // mass still to collect (mass criterion), double-double
     u64 kept_count;      // terms certainly kept so far
-    double kept_hi, kept_lo;           // their mass, double-double
-    double total_hi, total_lo;         // total mass S
+    double kept_hi, kept_lo;            // their mass, double-double
+    double total_hi, total_lo;          // total mass S
+    double min_mass;
     u64 cand_count;      // size of the current candidate bin
-    u64 PT, KT;          // final predicate: keep iff pat > PT || (pat == PT && lkey <= KT)
+    u64 tie_total;       // terms with pattern == PT when the cut falls among ties
+    u64 PT, KT;          // final predicate: keep iff pat > PT || (pat == PT && (KT == ~0 || lkey <= KT))
     double kept_mass, total_mass, scale, kept_fraction;
     u64 final_count;     // number of terms the predicate keeps
     u64 n_total;
 };
 
-struct KeyMap {          // stored (physical) key -> logical key
-    unsigned char log_of_phys[64];   // logical qubit of physical bit p (0xff = unused)
-    u64 xmask;                        // lazy X mask in physical positions
+// stored (physical) key -> logical key.  The map is a bit permutation plus the lazy X mask,
+// hence linear over GF(2): logical = XOR over the 8 bytes b of lut[b * 256 + byte_b(stored)]
+// (the mask is folded into table 0).  lut: DEVICE memory, 8 x 256 u64, built by the host.
+struct KeyMap {
+    const u64* lut;
 };
 
 // A truncation whose compaction has been deferred to the next reader of the state: a term
@@ -91,10 +97,11 @@ int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aou
 
 int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
 
-int svk_sel_init(SelState* ss, u64 n, u64 max_terms, double min_mass, cudaStream_t st);
-int svk_sel_hist(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, int nq,
-                 u64* hist, cudaStream_t st);
-int svk_sel_step(SelState* ss, u64* hist, int nq, cudaStream_t st);
+int svk_sel_init(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass, cudaStream_t st);
+int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const SelState* ss, u64* hist, cudaStream_t st);
+int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
+                    cudaStream_t st);
+int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st);
 int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
                 const PendPred& pd, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
 

@@ -48,7 +48,7 @@ __device__ __forceinline__ bool pend_keep(const PendPred& pd, u64 stored_key, do
 }
 
 template <bool PAIR>
-__global__ void __launch_bounds__(SV_THREADS, 3) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+__global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
@@ -57,39 +57,48 @@ __global__ void __launch_bounds__(SV_THREADS, 3) bitpass_kernel(const u64* __res
     __shared__ __align__(16) u64 sk[BP_TILE];
     __shared__ u32 W[BP_TILE + 1];
     __shared__ int red[SV_THREADS / 32 + 2];
-    __shared__ u32 s_tile;
     __shared__ u64 s_base;
     __shared__ double2 sU[64];      // [cx][xr][xc], ma = 1: up to 8 control patterns x 4
     __shared__ int s_cpos[SV_MAX_M], s_mc;
     const int tid = threadIdx.x;
 
-    if (tid == 0) s_tile = atomicAdd(tile_counter, 1u);
+    // Tiles are taken in blockIdx order (as CUB's single-pass scan does): a block only ever
+    // waits on lower-numbered blocks, which the hardware scheduler has already started.
+    const u32 tile = blockIdx.x;
     if (PAIR) {
         if (tid < 64) sU[tid] = gtab->U[tid];
         if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
         if (tid == 0) s_mc = gtab->mc;
     }
-    __syncthreads();
-    const u32 tile = s_tile;
     const TileDesc d0 = desc[tile], d1 = desc[tile + 1];
     u64 ps0, ps1, ps2; int l0, l1, l2;
     if (d0.e == d1.e) { ps0 = d0.ia; l0 = (int)(d1.ia - d0.ia); ps1 = d0.ib; l1 = (int)(d1.ib - d0.ib); ps2 = 0; l2 = 0; }
     else { ps0 = d0.ia; l0 = (int)(d0.mid - d0.ia); ps1 = d0.ib; l1 = (int)(d1.ia - d0.ib); ps2 = d1.mid; l2 = (int)(d1.ib - d1.mid); }
     const int cnt = min(BP_TILE, l0 + l1 + l2);
-    // coalesced loads of the (up to three) contiguous pieces; pending truncation applied here
-    for (int pc = 0; pc < 3; ++pc) {
-        const u64 gs = pc == 0 ? ps0 : (pc == 1 ? ps1 : ps2);
-        const int len = pc == 0 ? l0 : (pc == 1 ? l1 : l2);
-        const int off = pc == 0 ? 0 : (pc == 1 ? l0 : l0 + l1);
-        for (int idx = tid; idx < len && off + idx < BP_TILE; idx += SV_THREADS) {
-            const u64 k = ld_stream_u64(kin + gs + idx);
-            double2 a = ld_stream_d2(ain + gs + idx);
-            if (pd.active) {
-                if (pend_keep(pd, k, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
-                else { a.x = 0.0; a.y = 0.0; }
+    {   // coalesced loads of the (up to three) contiguous pieces, all issued before any is used;
+        // a pending truncation is applied here (dropped terms become 0+0i, survivors are scaled)
+        u64 lk[BP_VT]; double2 la[BP_VT];
+#pragma unroll
+        for (int r = 0; r < BP_VT; ++r) {
+            const int e = tid + r * SV_THREADS;
+            if (e < cnt) {
+                const u64 g = e < l0 ? ps0 + e : (e < l0 + l1 ? ps1 + (e - l0) : ps2 + (e - l0 - l1));
+                lk[r] = ld_stream_u64(kin + g);
+                la[r] = ld_stream_d2(ain + g);
             }
-            sk[off + idx] = k;
-            sa[off + idx] = a;
+        }
+#pragma unroll
+        for (int r = 0; r < BP_VT; ++r) {
+            const int e = tid + r * SV_THREADS;
+            if (e < cnt) {
+                double2 a = la[r];
+                if (pd.active) {
+                    if (pend_keep(pd, lk[r], a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
+                    else { a.x = 0.0; a.y = 0.0; }
+                }
+                sk[e] = lk[r];
+                sa[e] = a;
+            }
         }
     }
     __syncthreads();
