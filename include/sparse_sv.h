@@ -52,6 +52,7 @@ typedef struct {
     uint64_t n_in;         /* terms before the last call                                    */
     uint64_t n_out;        /* terms after it (N_pre for a gate, N_kept for a truncate)      */
     uint64_t launches;     /* kernels launched by this handle since creation                */
+    uint64_t fallbacks;    /* truncations whose sampled fast path missed and re-ran the full select */
 } sv_stats;
 
 /* Bytes of device memory a state of this capacity needs (for sv_create_in_arena). */
@@ -106,6 +107,12 @@ int sv_load(sv_state *s, const uint64_t *keys, const sv_c128 *amps, uint64_t n);
 /* Same with DEVICE source arrays (no host copy; used to time device-resident input). */
 int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amps, uint64_t n);
 
+/* Tuning knobs.  SV_OPT_SAMPLE_MIN_TERMS: states with at least this many terms find the
+ * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^18), smaller
+ * ones with the full-state radix select.  Both are exact; tests force either. */
+enum { SV_OPT_SAMPLE_MIN_TERMS = 0 };
+int sv_set_option(sv_state *s, int option, uint64_t value);
+
 /* Statistics of the last call and the launch counter. */
 int sv_get_stats(sv_state *s, sv_stats *out);
 
@@ -114,8 +121,8 @@ int sv_get_stats(sv_state *s, sv_stats *out);
  * sv_profile_get synchronises and returns, for one kernel, the summed device time, the
  * number of launches and the ALGORITHMIC bytes they had to move (DESIGN.md "Kernels":
  * diagonal 40 B/term; bit move 48 B/term; group 24 B x (N_in + N_out); select histogram
- * 16 B/term; compaction 24 B x (N_in + N_kept)). */
-enum { SV_K_DIAG = 0, SV_K_MOVE = 1, SV_K_GROUP = 2, SV_K_SELHIST = 3, SV_K_COMPACT = 4, SV_K_COUNT = 5 };
+ * 16 B/term; compaction 24 B x (N_in + N_kept); sampled classification 16 B/term). */
+enum { SV_K_DIAG = 0, SV_K_MOVE = 1, SV_K_GROUP = 2, SV_K_SELHIST = 3, SV_K_COMPACT = 4, SV_K_CLASSIFY = 5, SV_K_COUNT = 6 };
 typedef struct { double ms; uint64_t launches; double alg_bytes; } sv_kernel_prof;
 int sv_profile(sv_state *s, int enable);
 int sv_profile_get(sv_state *s, int kernel, sv_kernel_prof *out);

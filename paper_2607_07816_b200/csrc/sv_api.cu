@@ -48,7 +48,15 @@ struct sv_state {
     cudaEvent_t evpool[128];
     bool ev_ready;
     sv_kernel_prof prof[SV_K_COUNT];
+    // sampled fast path of the truncation cut
+    SampleCtl* sctl;
+    u64* smp_k[2];
+    u32* smp_v[2];
+    u32* smp_scr;
+    u64 sample_min_terms;   // states with fewer terms use the full-state select
+    double mass_est;        // total mass of the current state if known (NaN: unknown); gates are taken as unitary
 };
+#define SV_SAMPLE_MAX (1u << 17)
 
 static void prof_drain(sv_state* s) {
     if (!s->npend) return;
@@ -75,7 +83,7 @@ static void prof_slot(sv_state* s, int id, double bytes, cudaEvent_t* e0, cudaEv
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
 
-struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, total; };
+struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, sctl, smp_k[2], smp_v[2], smp_scr, total; };
 static ArenaLayout layout_for(u64 cap) {
     ArenaLayout L; size_t o = 0;
     for (int i = 0; i < 2; ++i) { L.keys[i] = o; o += align_up(cap * 8); }
@@ -88,6 +96,10 @@ static ArenaLayout layout_for(u64 cap) {
     L.misc = o; o += 256;
     L.partials = o; o += align_up(1024 * 8 + 8);
     L.lut = o; o += align_up(8 * 256 * 8);
+    L.sctl = o; o += align_up(sizeof(SampleCtl));
+    for (int i = 0; i < 2; ++i) { L.smp_k[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 8); }
+    for (int i = 0; i < 2; ++i) { L.smp_v[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 4); }
+    L.smp_scr = o; o += align_up(svk_sort_scratch_bytes(SV_SAMPLE_MAX));
     L.total = o;
     return L;
 }
@@ -152,7 +164,7 @@ static int init_state(sv_state* s) {
     s->count = 1; s->phys = 1;
     s->defer.active = 0;
     s->lut_valid = false;
-    s->lut_valid = false;
+    s->mass_est = 1.0;
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     const u64 k0 = 0;
@@ -195,6 +207,10 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->d_norm = (double*)(s->arena + L.misc + 192);
     s->partials = (double*)(s->arena + L.partials);
     s->lut = (u64*)(s->arena + L.lut);
+    s->sctl = (SampleCtl*)(s->arena + L.sctl);
+    for (int i = 0; i < 2; ++i) { s->smp_k[i] = (u64*)(s->arena + L.smp_k[i]); s->smp_v[i] = (u32*)(s->arena + L.smp_v[i]); }
+    s->smp_scr = (u32*)(s->arena + L.smp_scr);
+    s->sample_min_terms = 1ull << 18;
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
         sv_destroy(s);
@@ -248,6 +264,11 @@ extern "C" int sv_profile_get(sv_state* s, int kernel, sv_kernel_prof* out) {
     prof_drain(s);
     *out = s->prof[kernel];
     return SV_OK;
+}
+extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
+    return fail(s, SV_ERR_INVALID_ARG, "unknown option");
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
     if (!s || !out) return SV_ERR_INVALID_ARG;
@@ -455,11 +476,12 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
 // ---------------------------------------------------------------------------------------
 // truncation driver (rows a-8, a-9)
 // ---------------------------------------------------------------------------------------
-static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
+// The exact adaptive radix select over (keys, amps)[0..n).  seeded: the select state has been
+// prepared by svk_sel_seed (candidates of the sampled fast path); lk: scratch for tie keys.
+static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 n, u64* lk, bool seeded, u64 max_terms,
+                         double min_mass, SelState* out) {
     const KeyMap km = keymap_of(s);
-    const u64 n = s->count;                   // callers have materialised any deferred truncation
-    u64* lk = s->keys[s->cur ^ 1];            // the idle buffer holds the extracted tie keys
-    s->stats.launches += svk_sel_init(s->sel, s->hist, n, max_terms, min_mass, s->stream);
+    if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n, max_terms, min_mass, s->stream);
     int phase = 0;
     u64 ties = 0;
     for (int it = 0; it < 64; ++it) {
@@ -467,8 +489,8 @@ static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out
         const double bytes = phase <= 1 ? 16.0 * (double)n : (phase == 2 ? 16.0 * (double)n + 16.0 * (double)ties : 8.0 * (double)ties);
         prof_slot(s, SV_K_SELHIST, bytes, &e0, &e1);
         if (e0) cudaEventRecord(e0, s->stream);
-        if (phase <= 1) s->stats.launches += svk_sel_pass(phase, s->amps[s->cur], nullptr, n, s->sel, s->hist, s->stream);
-        else if (phase == 2) s->stats.launches += svk_sel_extract(s->keys[s->cur], s->amps[s->cur], n, s->sel, km, lk, s->hist, s->stream);
+        if (phase <= 1) s->stats.launches += svk_sel_pass(phase, amps, nullptr, n, s->sel, s->hist, s->stream);
+        else if (phase == 2) s->stats.launches += svk_sel_extract(keys, amps, n, s->sel, km, lk, s->hist, s->stream);
         else s->stats.launches += svk_sel_pass(2, nullptr, lk, ties, s->sel, s->hist, s->stream);
         if (e1) cudaEventRecord(e1, s->stream);
         s->stats.launches += svk_sel_step(s->sel, s->hist, s->stream);
@@ -476,12 +498,57 @@ static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out
         s->stats.passes += 1;
         int rc = read_back(s, out, s->sel, sizeof(SelState));
         if (rc != SV_OK) return rc;
-        if (out->done == 1) return SV_OK;
+        if (out->done == 1 || out->done == 3) return SV_OK;
         if (out->done != 0) return fail(s, SV_ERR_CUDA, "internal: radix select inconsistency");
         phase = out->phase;
         ties = out->tie_total;
     }
     return fail(s, SV_ERR_CUDA, "radix select did not converge");
+}
+
+// Sampled fast path (sv_sample_select.cu): one streaming pass over the amplitudes, then the
+// exact select on the few candidates around the cut.  *used = false: band miss, nothing decided.
+static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelState* out, bool* used) {
+    *used = false;
+    const u64 n = s->count;
+    const int alt = s->cur ^ 1;
+    u64 m64 = n / 8;
+    if (m64 > SV_SAMPLE_MAX) m64 = SV_SAMPLE_MAX;
+    if (m64 < 64) return SV_OK;
+    const u32 M = (u32)m64;
+    cudaStream_t st = s->stream;
+    s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st);
+    int in_alt = 0;
+    s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 32, s->smp_scr, st, &in_alt);
+    s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n, max_terms, min_mass, s->mass_est, s->sctl, st);
+    cudaEvent_t e0, e1;
+    prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
+    if (e0) cudaEventRecord(e0, st);
+    s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], st);
+    if (e1) cudaEventRecord(e1, st);
+    s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n, max_terms, min_mass, st);
+    CHECK_LAUNCH();
+    s->stats.passes += 1;
+    int rc = read_back(s, out, s->sel, sizeof(SelState));
+    if (rc != SV_OK) return rc;
+    const u64 cand = out->n_total;
+    if (out->done == 3 || cand > n / 2) return SV_OK;   // band miss, or too many candidates to gain anything
+    rc = select_levels(s, s->keys[alt], s->amps[alt], cand, s->keys[alt] + cand, true, max_terms, min_mass, out);
+    if (rc != SV_OK) return rc;
+    if (out->done == 1) *used = true;
+    return SV_OK;
+}
+
+static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
+    const u64 n = s->count;                   // callers have materialised any deferred truncation
+    if (n >= s->sample_min_terms) {
+        bool used = false;
+        int rc = run_select_sampled(s, max_terms, min_mass, out, &used);
+        if (rc != SV_OK || used) return rc;
+        s->stats.fallbacks += 1;
+    }
+    // full-state select; the idle buffer holds the extracted tie keys
+    return select_levels(s, s->keys[s->cur], s->amps[s->cur], n, s->keys[s->cur ^ 1], false, max_terms, min_mass, out);
 }
 
 extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, double* kept_fraction) {
@@ -498,7 +565,16 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     SelState ss;
     rc = run_select(s, max_terms, min_mass, &ss);
     if (rc != SV_OK) return rc;
+    if (getenv("SV_DEBUG")) {
+        SampleCtl c; cudaMemcpy(&c, s->sctl, sizeof(c), cudaMemcpyDeviceToHost);
+        fprintf(stderr, "[trunc] n=%llu K=%llu seeded=%d PT=%016llx KT=%016llx final=%llu kept=%.17g tot=%.17g | P_hi=%016llx P_lo=%016llx above=%llu below=%llu cand=%llu ovf=%llu Eref=%d\n",
+                (unsigned long long)s->count, (unsigned long long)max_terms, ss.seeded, (unsigned long long)ss.PT, (unsigned long long)ss.KT,
+                (unsigned long long)ss.final_count, ss.kept_mass, ss.total_mass, (unsigned long long)c.P_hi, (unsigned long long)c.P_lo,
+                (unsigned long long)c.above_cnt, (unsigned long long)c.below_cnt, (unsigned long long)c.cand_cnt, (unsigned long long)c.overflow, c.Eref);
+    }
+    s->mass_est = ss.total_mass;
     if (ss.final_count >= s->count) return SV_OK;   // nothing dropped: bitwise no-op (reading R7)
+    s->mass_est = 1.0;                              // renormalised
     // The cut is decided; the compaction + renormalisation is left to the next reader of the
     // state (the next gate's load applies it for free), or to materialize().
     s->defer.active = 1; s->defer.PT = ss.PT; s->defer.KT = ss.KT; s->defer.scale = ss.scale; s->defer.km = keymap_of(s);
@@ -518,7 +594,14 @@ extern "C" int sv_norm(sv_state* s, double* mass) {
 
 extern "C" int sv_check_invariants(sv_state* s, int* ok) {
     if (!s || !ok) return SV_ERR_INVALID_ARG;
+    const bool was_deferred = s->defer.active != 0;
     { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
+    if (was_deferred) {   // the compaction must have kept exactly the number of terms the select decided
+        u64 kept = 0;
+        int rck = read_back(s, &kept, s->d_count, sizeof(u64));
+        if (rck != SV_OK) return rck;
+        if (kept != s->count) { *ok = 0; return SV_OK; }
+    }
     s->stats.launches += svk_check(s->keys[s->cur], s->amps[s->cur], s->count, s->n, s->d_bad, s->stream);
     CHECK_LAUNCH();
     int bad = 0;
@@ -639,6 +722,12 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
     s->count = n; s->phys = n;
     s->defer.active = 0;
     s->lut_valid = false;
+    s->mass_est = nan("");
+    if (n > 0) {   // the total mass steers the sampled truncation path (it is re-measured exactly there)
+        double m = 0.0;
+        s->stats.launches += svk_norm(s->amps[s->cur], n, s->partials, s->d_norm, st);
+        if (read_back(s, &m, s->d_norm, sizeof(double)) == SV_OK) s->mass_est = m;
+    }
     s->xmask = 0;
     for (int q = 0; q < 64; ++q) s->phys_of_log[q] = q;
     s->stats.n_in = n; s->stats.n_out = n; s->stats.gate_class = SV_CLASS_NONE;

@@ -52,6 +52,19 @@ struct SelState {
     double kept_mass, total_mass, scale, kept_fraction;
     u64 final_count;     // number of terms the predicate keeps
     u64 n_total;
+    int seeded, pad2_;   // 1: the select runs on the candidates of the sampled fast path (sv_sample_select.cu)
+    u64 P_lo;            // seeded: every term outside the candidates and not above them has a pattern < P_lo
+    u64 below_cnt;       // seeded: terms certainly below the candidates; a cut that would need them is a band miss (done = 3)
+};
+
+// Sampled fast path of the truncation cut (sv_sample_select.cu): pivots and the results of the
+// classification pass.  tot / abv: 128-bit fixed-point masses (low word, high word) in units of
+// 2^(Eref - 1075 - 41).
+struct SampleCtl {
+    u64 P_hi, P_lo;      // above iff pattern > P_hi; below iff pattern < P_lo; else candidate
+    int Eref, pad_;
+    u64 above_cnt, below_cnt, cand_cnt, overflow;
+    u64 tot[2], abv[2];
 };
 
 // stored (physical) key -> logical key.  The map is a bit permutation plus the lazy X mask,
@@ -102,6 +115,12 @@ int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const S
 int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
                     cudaStream_t st);
 int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st);
+// sampled fast path: sample -> (sort) -> pivots -> classify -> seed the select state
+int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
+int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
+                 cudaStream_t st);
+int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st);
+int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st);
 int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
                 const PendPred& pd, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
 

@@ -263,6 +263,48 @@ int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState*
     return 1;
 }
 
+// Seeds the select state for a run over the candidates of the sampled fast path: what lies
+// above the band is already kept, S is known exactly.  done = 3 reports a band miss.
+__device__ __forceinline__ dd dd_from_fx(const u64* lohi, int Eref) {
+    const dd v = dd_add(dd_scale2(dd_from_u64(lohi[1]), 64), dd_from_u64(lohi[0]));
+    return dd_scale2(v, Eref - 1075 - 41);
+}
+__global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass) {
+    for (int i = threadIdx.x; i < H_TOTAL; i += blockDim.x)
+        hist[i] = ((i >= H_AND && i < H_OR) || i == H_EXT + 1) ? ~0ull : 0ull;
+    if (threadIdx.x != 0) return;
+    const SampleCtl c = *ctl;
+    SelState s;
+    memset(&s, 0, sizeof(s));
+    s.seeded = 1;
+    s.n_total = c.cand_cnt;
+    s.cand_count = c.cand_cnt;
+    s.below_cnt = c.below_cnt;
+    s.P_lo = c.P_lo;
+    s.min_mass = min_mass;
+    const dd tot = dd_from_fx(c.tot, c.Eref), abv = dd_from_fx(c.abv, c.Eref);
+    s.total_hi = tot.hi; s.total_lo = tot.lo;
+    s.kept_hi = abv.hi; s.kept_lo = abv.lo;
+    s.kept_count = c.above_cnt;
+    bool miss = c.overflow != 0 || c.cand_cnt == 0 || c.above_cnt + c.below_cnt + c.cand_cnt != n_orig;
+    s.count_active = (max_terms != 0 && max_terms < n_orig) ? 1 : 0;
+    if (s.count_active) {
+        if (max_terms <= c.above_cnt) miss = true; else s.k_rem = max_terms - c.above_cnt;
+    }
+    s.mass_active = (min_mass < 1.0) ? 1 : 0;
+    if (s.mass_active) {
+        const dd rem = dd_sub(dd_make(__dmul_rn(min_mass, tot.hi)), abv);
+        if (!(rem.hi > 0.0)) miss = true;
+        s.mass_rem_hi = rem.hi; s.mass_rem_lo = rem.lo;
+    }
+    if (miss) s.done = 3;
+    *ss = s;
+}
+int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st) {
+    sel_seed_kernel<<<1, SV_THREADS, 0, st>>>(ss, hist, ctl, n_orig, max_terms, min_mass);
+    return 1;
+}
+
 // ---------------------------------------------------------------------------------------
 // one decision step (one block; thread 0 decides), then the histogram is cleared
 // ---------------------------------------------------------------------------------------
@@ -292,7 +334,7 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
     if (s.phase <= 1) {
         const bool l0 = s.phase == 0;
 #define BIN_E(d) (l0 ? ((((d) & 0x7ff) != 0) ? ((d) & 0x7ff) : 1) : s.E)
-        if (l0) {   // total mass S and the p-mass threshold min_mass * S (reading R5)
+        if (l0 && !s.seeded) {   // total mass S and the p-mass threshold min_mass * S (reading R5)
             dd tot = dd_make(0.0);
             for (int d = 0; d < RS_BINS; ++d)
                 if (cnt[d]) tot = dd_add(tot, bin_mass(shi[d], slo[d], BIN_E(d)));
@@ -311,8 +353,10 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
             if (s.mass_active && dM < 0 && dd_ge(dd_add(cum, m), rem)) { dM = d; aboveC_M = cumc; aboveM_M = cum; }
             cumc += c; cum = dd_add(cum, m);
         }
-        if (dlow < 0) { s.done = 1; s.PT = 0; s.KT = ~0ull; }   // no candidates at all (cannot happen)
-        else {
+        if (dlow < 0) { s.done = s.seeded ? 3 : 1; s.PT = 0; s.KT = ~0ull; }   // no candidates at all
+        else if (s.seeded && s.below_cnt > 0 && (!s.mass_active || dM < 0) && (!s.count_active || dK < 0)) {
+            s.done = 3;             // the cut lies below the sampled band: the caller runs the full select
+        } else {
             // threshold not reached (rounding of min_mass * S): every candidate is needed
             if (s.mass_active && dM < 0) {
                 dM = dlow; aboveC_M = cumc - cnt[dlow];
@@ -346,7 +390,9 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
                 else if (s.mass_active && allK) s.count_active = 0;
             }
             if (take_all) {
-                s.PT = A; s.KT = ~0ull;                  // A <= every member of the bin, > every term below it
+                // A <= every member of the bin, > every term in a lower bin; seeded: the terms below
+                // the band never entered the histograms, P_lo separates them from every candidate
+                s.PT = (s.seeded && A < s.P_lo) ? s.P_lo : A; s.KT = ~0ull;
                 s.kept_count += s.cand_count; kept = dd_add(kept, bm);
                 s.done = 1;
             } else if (diff == 0) {                      // the candidates are exact ties at probability pv

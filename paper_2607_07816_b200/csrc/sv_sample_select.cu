@@ -1,0 +1,227 @@
+// Truncation cut, fast path.
+//
+// The paper sorts all terms by probability; sv_radix_select.cu finds the cut with several
+// histogram passes over the whole state.  Here ONE streaming pass over the amplitudes is
+// enough in the common case:
+//
+//   1. sample     M evenly spaced terms -> the top 32 bits of their probability patterns,
+//                 sorted (a 1 MB LSD radix sort that lives in L2);
+//   2. pivots     from the sorted sample, two patterns P_lo <= P_hi that bracket the cut
+//                 with wide statistical margins, for the top-k criterion (a quantile) and
+//                 for the p-mass criterion (the tail of the sample whose scaled mass is
+//                 the mass to be dropped);
+//   3. classify   one pass: every term is "above" (pattern > P_hi: certainly kept), "below"
+//                 (pattern < P_lo: certainly dropped) or a candidate.  The pass returns the
+//                 EXACT count and mass above, the exact total mass S, the count below, and
+//                 copies the candidates (a few per cent of the state) to the idle buffers;
+//   4. finish     the exact adaptive radix select of sv_radix_select.cu runs on the
+//                 candidates only, seeded with what is already kept.
+//
+// The pivots only steer the work.  The cut itself is exact: if it turns out not to lie
+// among the candidates (or a probability is out of the fixed-point range) the seeded select
+// reports a band miss and the caller falls back to the full-state select.
+//
+// Exact masses (D3): p is converted to a 128-bit fixed-point integer relative to
+// a reference exponent, and integers are added -- the sums do not depend on the order in
+// which threads or blocks add them.
+#include "sv_device.cuh"
+
+typedef unsigned __int128 u128;
+
+__global__ void __launch_bounds__(SV_THREADS) ss_sample_kernel(const double2* __restrict__ amps, u64 n, u32 M,
+                                                               u64* __restrict__ smp) {
+    const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= M) return;
+    const u64 i = (u64)(((u128)j * n) / M);
+    smp[j] = (u64)__double_as_longlong(prob_of(ld_stream_d2(amps + i))) >> 32;
+}
+
+__device__ __forceinline__ double smp_prob(u64 top32) {   // mid-point of the values sharing these top bits
+    return __longlong_as_double((long long)((top32 << 32) | 0x80000000ull));
+}
+
+// One block of 1024 threads.  smp[0..M) ascending.  Warp w owns the contiguous range
+// [w * per, (w + 1) * per) and walks it 32 elements at a time.
+__global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ smp, u32 M, u64 n, u64 max_terms,
+                                                        double min_mass, double mass_est, SampleCtl* __restrict__ ctl) {
+    __shared__ double wsum[32];
+    __shared__ u32 cnt[2][3];   // [sweep][threshold]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const u32 per = (M + 31) / 32;
+    const u32 b0 = min(M, warp * per), b1 = min(M, b0 + per);
+    if (threadIdx.x < 6) cnt[threadIdx.x / 3][threadIdx.x % 3] = 0;
+    double s = 0.0;
+    for (u32 i = b0 + lane; i < b1; i += 32) s += smp_prob(smp[i]);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+    if (lane == 0) wsum[warp] = s;
+    __syncthreads();
+    double pre = 0.0, T = 0.0;
+    for (int w = 0; w < 32; ++w) { if (w < warp) pre += wsum[w]; T += wsum[w]; }
+    const bool mass_on = min_mass < 1.0;
+    // mass to drop, in sample units (the tail is made of small terms, so the scaled sample tail
+    // estimates it well even when a few heavy terms carry most of S)
+    const double S_est = (mass_est == mass_est && mass_est > 0.0) ? mass_est : T * ((double)n / (double)M);
+    const double X0 = (1.0 - min_mass) * S_est * ((double)M / (double)n);
+    // sweep 1: a0 = sample elements in the nominal tail; sweep 2: the band X0 / (1 + eps) .. X0 * (1 + eps)
+    // with eps ~ 10 / sqrt(a0) (the relative noise of a tail sum of a0 sampled terms)
+    double X[3] = {X0, X0, X0};
+    for (int sweep = 0; sweep < 2 && mass_on; ++sweep) {
+        u32 c[3] = {0, 0, 0};
+        double run = pre;
+        for (u32 i0 = b0; i0 < b1; i0 += 32) {
+            const u32 i = i0 + lane;
+            const double v = (i < b1) ? smp_prob(smp[i]) : 0.0;
+            double inc = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+            const double incl = run + inc;   // mass of the sample's i + 1 smallest elements
+            if (i < b1) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k) c[k] += (incl <= X[k]) ? 1u : 0u;
+            }
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            u32 v = c[k];
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            if (lane == 0 && v) atomicAdd(&cnt[sweep][k], v);
+        }
+        __syncthreads();
+        if (sweep == 0) {
+            const double a0 = (double)cnt[0][1];
+            const double eps = fmin(2.0, 10.0 / sqrt(fmax(a0, 1.0)));
+            X[0] = X0 / (1.0 + eps); X[2] = X0 * (1.0 + eps);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    // numbers of (smallest) sample elements certainly / possibly dropped
+    long long lo_idx = 0, hi_idx = 0;
+    if (mass_on) {
+        const long long a0 = cnt[0][1];
+        long long a_lo = (a0 < 128) ? 0 : (long long)cnt[1][0] - 8;
+        long long a_hi = (a0 < 128) ? max((long long)cnt[1][2] + 8, 2 * a0 + 64) : (long long)cnt[1][2] + 8;
+        lo_idx = max(lo_idx, a_lo); hi_idx = max(hi_idx, a_hi);
+    }
+    if (max_terms != 0 && max_terms < n) {
+        const double q = (double)(n - max_terms) / (double)n;
+        const double d = q * (double)M;
+        const double dl = 6.0 * sqrt(fmax(d * (1.0 - q), 0.0)) + 8.0;
+        lo_idx = max(lo_idx, (long long)floor(d - dl));
+        hi_idx = max(hi_idx, (long long)ceil(d + dl));
+    }
+    SampleCtl c;
+    memset(&c, 0, sizeof(c));
+    c.P_lo = (lo_idx <= 0) ? 0ull : (smp[min((long long)M, lo_idx) - 1] << 32);
+    c.P_hi = (hi_idx >= (long long)M) ? ~0ull : ((smp[hi_idx] << 32) | 0xffffffffull);
+    int er = (int)(smp[M - 1] >> 20) + 12;
+    c.Eref = er > 2046 ? 2046 : er;
+    *ctl = c;
+}
+
+// p (as its bit pattern) in units of 2^(Eref - 1075 - 41); exponents above Eref overflow
+__device__ __forceinline__ u128 fx_of(u64 pat, int Eref, u32& ovf) {
+    int e = (int)(pat >> 52);
+    u64 M = pat & ((1ull << 52) - 1);
+    if (e) M |= 1ull << 52; else e = 1;
+    const int sh = e - Eref + 41;
+    if (sh > 41) { ovf = 1; return 0; }
+    if (sh >= 0) return (u128)M << sh;
+    if (sh > -53) return (u128)(M >> (-sh));
+    return 0;
+}
+__device__ __forceinline__ u128 warp_sum_u128(u128 v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        const u64 lo = __shfl_xor_sync(0xffffffffu, (u64)v, d);
+        const u64 hi = __shfl_xor_sync(0xffffffffu, (u64)(v >> 64), d);
+        v += ((u128)hi << 64) | lo;
+    }
+    return v;
+}
+__device__ __forceinline__ void atomic_add_u128(u64* lohi, u128 v) {   // lohi[0] = low word, lohi[1] = high word
+    const u64 lo = (u64)v, hi = (u64)(v >> 64);
+    const u64 old = atomicAdd(&lohi[0], lo);
+    const u64 carry = (old + lo < old) ? 1ull : 0ull;
+    if (hi + carry) atomicAdd(&lohi[1], hi + carry);
+}
+
+#define SC_IT 4
+__global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
+                                                                 u64 n, SampleCtl* __restrict__ ctl, u64* __restrict__ ckeys,
+                                                                 double2* __restrict__ camps) {
+    const u64 P_hi = ctl->P_hi, P_lo = ctl->P_lo;
+    const int Eref = ctl->Eref;
+    const int lane = threadIdx.x & 31;
+    u128 tot = 0, abv = 0;
+    u32 n_abv = 0, n_blw = 0, ovf = 0;
+    const u64 chunk = (u64)SV_THREADS * SC_IT;
+    const u64 nchunks = (n + chunk - 1) / chunk;
+    for (u64 c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        double2 a[SC_IT];
+#pragma unroll
+        for (int r = 0; r < SC_IT; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            a[r] = (i < n) ? ld_stream_d2(amps + i) : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int r = 0; r < SC_IT; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            const bool ok = i < n;
+            const u64 pat = (u64)__double_as_longlong(prob_of(a[r]));
+            const u128 f = ok ? fx_of(pat, Eref, ovf) : (u128)0;
+            tot += f;
+            const bool above = ok && pat > P_hi, below = ok && pat < P_lo;
+            if (above) { abv += f; ++n_abv; }
+            n_blw += below ? 1u : 0u;
+            const bool cand = ok && !above && !below;
+            const u32 grp = __ballot_sync(0xffffffffu, cand);
+            if (grp) {
+                u64 base = 0;
+                const int ldr = __ffs(grp) - 1;
+                if (lane == ldr) base = atomicAdd(&ctl->cand_cnt, (u64)__popc(grp));
+                base = __shfl_sync(0xffffffffu, base, ldr);
+                if (cand) {
+                    const u64 pos = base + __popc(grp & ((1u << lane) - 1u));
+                    ckeys[pos] = keys[i];
+                    camps[pos] = a[r];
+                }
+            }
+        }
+    }
+    tot = warp_sum_u128(tot);
+    abv = warp_sum_u128(abv);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        n_abv += __shfl_xor_sync(0xffffffffu, n_abv, d);
+        n_blw += __shfl_xor_sync(0xffffffffu, n_blw, d);
+        ovf |= __shfl_xor_sync(0xffffffffu, ovf, d);
+    }
+    if (lane == 0) {
+        atomic_add_u128(ctl->tot, tot);
+        atomic_add_u128(ctl->abv, abv);
+        if (n_abv) atomicAdd(&ctl->above_cnt, (u64)n_abv);
+        if (n_blw) atomicAdd(&ctl->below_cnt, (u64)n_blw);
+        if (ovf) atomicOr(&ctl->overflow, 1ull);
+    }
+}
+
+int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st) {
+    ss_sample_kernel<<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(amps, n, M, smp);
+    return 1;
+}
+int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
+                 cudaStream_t st) {
+    ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n, max_terms, min_mass, mass_est, ctl);
+    return 1;
+}
+int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st) {
+    u64 blocks = (n + SV_THREADS * SC_IT - 1) / (SV_THREADS * SC_IT);
+    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    if (blocks < 1) blocks = 1;
+    ss_classify_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps);
+    return 1;
+}

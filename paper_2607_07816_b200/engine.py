@@ -18,13 +18,14 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
-           "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get"]
-KERNELS = ["diag", "move", "group", "sel_hist", "compact"]
+           "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option"]
+KERNELS = ["diag", "move", "group", "sel_hist", "compact", "classify"]
+OPT_SAMPLE_MIN_TERMS = 0
 
 
 class SvStats(C.Structure):
     _fields_ = [("gate_class", C.c_int), ("m", C.c_int), ("active_bits", C.c_int), ("passes", C.c_int),
-                ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64)]
+                ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64), ("fallbacks", C.c_uint64)]
 
 
 class SvKernelProf(C.Structure):
@@ -77,6 +78,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_profile.argtypes = [vp, i32]
     lib.sv_profile_get.restype = i32
     lib.sv_profile_get.argtypes = [vp, i32, C.POINTER(SvKernelProf)]
+    lib.sv_set_option.restype = i32
+    lib.sv_set_option.argtypes = [vp, i32, u64]
     return lib
 
 
@@ -177,7 +180,11 @@ class SparseSV:
         st = SvStats()
         self._chk(lib.sv_get_stats(self._h, C.byref(st)))
         return {"class": CLASS_NAMES.get(st.gate_class, "?"), "m": st.m, "active_bits": st.active_bits,
-                "passes": st.passes, "n_in": int(st.n_in), "n_out": int(st.n_out), "launches": int(st.launches)}
+                "passes": st.passes, "n_in": int(st.n_in), "n_out": int(st.n_out), "launches": int(st.launches),
+                "fallbacks": int(st.fallbacks)}
+
+    def set_option(self, option: int, value: int):
+        self._chk(lib.sv_set_option(self._h, int(option), int(value)))
 
     def check_invariants(self) -> bool:
         ok = C.c_int(0)

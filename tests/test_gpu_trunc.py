@@ -10,10 +10,23 @@ pytestmark = pytest.mark.gpu
 from util_parity import assert_same_state, assert_truncation_parity, step_locked, MASS_TOL  # noqa: E402
 
 
-@pytest.fixture(scope="module")
-def eng():
+class _Eng:
+    """The engine module with the truncation-cut path pinned: 'full' = the full-state radix select,
+    'sampled' = the one-pass sampled path (sv_sample_select.cu) from 512 terms on."""
+
+    def __init__(self, engine, mode):
+        self.engine, self.mode = engine, mode
+
+    def SparseSV(self, n, cap, **kw):
+        sv = self.engine.SparseSV(n, cap, **kw)
+        sv.set_option(self.engine.OPT_SAMPLE_MIN_TERMS, (1 << 62) if self.mode == "full" else 512)
+        return sv
+
+
+@pytest.fixture(scope="module", params=["full", "sampled"])
+def eng(request):
     from paper_2607_07816_b200 import engine
-    return engine
+    return _Eng(engine, request.param)
 
 
 def _oracle(n):
@@ -44,6 +57,41 @@ def test_truncate_random(eng, count, K, f, spread):
     assert_truncation_parity(sv.export()[:2], o.export()[:2])
     assert sv.check_invariants()
     assert abs(sv.norm() - 1.0) <= 1e-13
+    if eng.mode == "sampled" and count >= 50000:
+        assert sv.stats()["fallbacks"] == 0, "the sampled band missed the cut on a generic state"
+
+
+@pytest.mark.parametrize("K,f", [(1 << 20, 1.0), (0, 1 - 1e-4), (3 << 20, 0.9999), (0, 0.5), (16, 1.0)])
+def test_truncate_large_sampled(eng, K, f):
+    """2^22 generic terms: the sampled path with its full-size sample (2^17), vs the oracle."""
+    if eng.mode != "sampled":
+        pytest.skip("covered by the sampled mode")
+    rng = np.random.default_rng(K + 7)
+    keys, amps = W.random_state(rng, 50, 1 << 22, spread=1.5)
+    sv, o = _pair(eng, 50, keys, amps)
+    kg = sv.truncate(K, f)
+    ko = o.truncate(K, f)
+    assert abs(kg - ko) <= MASS_TOL
+    assert abs(sv.num_terms() - o.num_terms()) <= 2
+    assert_truncation_parity(sv.export()[:2], o.export()[:2])
+    assert sv.stats()["fallbacks"] == 0
+    assert sv.check_invariants()
+
+
+def test_truncate_peaked_mass(eng):
+    """One term carries most of the mass (a peaked state): the p-mass pivots must come from the
+    tail, not from the sample's estimate of S."""
+    rng = np.random.default_rng(11)
+    keys, amps = W.random_state(rng, 44, 300000, spread=0.5)
+    amps[12345] *= 3000.0
+    amps /= np.sqrt(np.sum(np.abs(amps) ** 2))
+    sv, o = _pair(eng, 44, keys, amps)
+    for f in (1 - 1e-3, 1 - 1e-4):
+        kg = sv.truncate(0, f)
+        ko = o.truncate(0, f)
+        assert abs(kg - ko) <= MASS_TOL
+        assert abs(sv.num_terms() - o.num_terms()) <= 2
+        assert_truncation_parity(sv.export()[:2], o.export()[:2])
 
 
 def test_truncate_noop_bitwise(eng):
