@@ -80,6 +80,16 @@ static void prof_slot(sv_state* s, int id, double bytes, cudaEvent_t* e0, cudaEv
     s->npend += 1;
 }
 
+int sv_sm_count() {
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    }
+    return n;
+}
+
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
 
@@ -283,10 +293,10 @@ static int read_back(sv_state* s, void* dst, const void* dsrc, size_t bytes) {
     return SV_OK;
 }
 
-// Apply a deferred truncation now (one compaction pass).  Readers that cannot fuse the
-// predicate into their own load call this first.
+// Apply a deferred truncation and squeeze out dead entries now (one compaction pass).  Readers that
+// cannot fuse the predicate into their own load, or that need a dense array, call this first.
 static int materialize(sv_state* s) {
-    if (!s->defer.active) return SV_OK;
+    if (!s->defer.active && s->phys == s->count) return SV_OK;
     const int alt = s->cur ^ 1;
     cudaEvent_t e0, e1;
     prof_slot(s, SV_K_COMPACT, 24.0 * ((double)s->phys + (double)s->count), &e0, &e1);
@@ -301,6 +311,8 @@ static int materialize(sv_state* s) {
     s->defer.active = 0;
     return SV_OK;
 }
+// Dead entries (terms dropped in place) are tolerated up to 1/8 of the live terms.
+static inline bool few_dead(const sv_state* s) { return s->phys - s->count <= s->count / 8; }
 
 // ---------------------------------------------------------------------------------------
 // sv_apply_gate: classify (row a-1), plan the bit moves, launch
@@ -367,7 +379,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         if (!unit_phase) {
             CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
             cudaEvent_t e0, e1;
-            if (s->defer.active) {   // truncate-then-diagonal in one out-of-place pass
+            if (s->defer.active && !few_dead(s)) {   // truncate-then-diagonal in one out-of-place, compacting pass
                 const int alt = s->cur ^ 1;
                 prof_slot(s, SV_K_DIAG, 24.0 * ((double)s->phys + (double)s->count), &e0, &e1);
                 if (e0) cudaEventRecord(e0, s->stream);
@@ -375,10 +387,16 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
                                                       s->tab, s->defer, s->status, s->tile_counter, s->d_count, s->stream);
                 if (e1) cudaEventRecord(e1, s->stream);
                 s->cur = alt; s->phys = s->count; s->defer.active = 0;
-            } else {
-                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->count, &e0, &e1);
+            } else if (s->defer.active) {            // in place: dropped terms become dead entries
+                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &e0, &e1);
                 if (e0) cudaEventRecord(e0, s->stream);
-                s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->count, s->tab, s->stream);
+                s->stats.launches += svk_diag_pend(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, 1, s->defer, s->stream);
+                if (e1) cudaEventRecord(e1, s->stream);
+                s->defer.active = 0;
+            } else {
+                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &e0, &e1);
+                if (e0) cudaEventRecord(e0, s->stream);
+                s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, s->stream);
                 if (e1) cudaEventRecord(e1, s->stream);
             }
             CHECK_LAUNCH();
@@ -404,14 +422,15 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;
         const int alt = s->cur ^ 1;
+        const int fixed = few_dead(s) ? 1 : 0;   // position preserving (dead entries carried) or compacting
         cudaEvent_t e0, e1;
-        prof_slot(s, SV_K_MOVE, 48.0 * (double)s->count, &e0, &e1);
-        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, p, 0, nullptr,
+        prof_slot(s, SV_K_MOVE, 24.0 * ((double)s->phys + (double)(fixed ? s->phys : s->count)), &e0, &e1);
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, p, 0, fixed, nullptr,
                                          s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, e0, e1);
         CHECK_LAUNCH();
         s->cur = alt;
-        s->phys = s->count;      // a deferred truncation has been applied by the pass
-        s->defer.active = 0;
+        if (!fixed) s->phys = s->count;      // dropped terms and dead entries have been squeezed out
+        s->defer.active = 0;                 // a deferred truncation has been applied by the pass
         layout_move(s, p);
         s->stats.passes += 1;
     }
@@ -444,15 +463,37 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
     const int alt = s->cur ^ 1;
     cudaEvent_t ge0, ge1;
+    // one active bit whose 2x2 blocks are all monomial (CNOT, Toffoli, ...): every stored entry maps to
+    // exactly one stored entry, the pass needs no scan and the term count is known without a read-back
+    bool monomial = (ma == 1);
+    for (int cx = 0; cx < (1 << mc) && monomial; ++cx) {
+        const double2* u = &tab.U[cx << 2];
+        const bool z00 = u[0].x == 0.0 && u[0].y == 0.0, z01 = u[1].x == 0.0 && u[1].y == 0.0;
+        const bool z10 = u[2].x == 0.0 && u[2].y == 0.0, z11 = u[3].x == 0.0 && u[3].y == 0.0;
+        monomial = (!z00 && !z11 && z01 && z10) || (z00 && z11 && !z01 && !z10);
+    }
+    if (ma == 1 && monomial && few_dead(s)) {
+        prof_slot(s, SV_K_GROUP, 48.0 * (double)s->phys, &ge0, &ge1);
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 1,
+                                         s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; s->lut_valid = false; }
+        s->cur ^= 1;
+        s->defer.active = 0;
+        s->stats.n_out = s->count;
+        return SV_OK;
+    }
     prof_slot(s, SV_K_GROUP, 0.0, &ge0, &ge1);
     const int gslot = s->npend - 1;
-    if (ma == 1) {   // one active bit: the lean pass (p = 0 when the bit already sits at the LSB)
-        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, s->tab,
-                                         s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+    const u64 n_live_in = s->count;
+    if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 0,
+                                         s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
     } else {
         if (s->defer.active) { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
         const int alt2 = s->cur ^ 1;
-        s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt2], s->amps[alt2], s->count, plast, ma,
+        s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt2], s->amps[alt2], s->phys, plast, ma,
                                        s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
     }
     CHECK_LAUNCH();
@@ -460,7 +501,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     u64 nout = 0;
     int rc = read_back(s, &nout, s->d_count, sizeof(u64));
     if (rc != SV_OK) return rc;
-    if (ge0) s->pend[gslot].bytes = 24.0 * ((double)s->count + (double)(nout > s->cap ? s->cap : nout));
+    if (ge0) s->pend[gslot].bytes = 24.0 * ((double)n_live_in + (double)(nout > s->cap ? s->cap : nout));
     if (nout > s->cap) {
         s->stats.n_out = nout;
         return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
@@ -478,10 +519,10 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
 // ---------------------------------------------------------------------------------------
 // The exact adaptive radix select over (keys, amps)[0..n).  seeded: the select state has been
 // prepared by svk_sel_seed (candidates of the sampled fast path); lk: scratch for tie keys.
-static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 n, u64* lk, bool seeded, u64 max_terms,
+static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 n, u64 n_live, u64* lk, bool seeded, u64 max_terms,
                          double min_mass, SelState* out) {
     const KeyMap km = keymap_of(s);
-    if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n, max_terms, min_mass, s->stream);
+    if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n_live, max_terms, min_mass, s->stream);
     int phase = 0;
     u64 ties = 0;
     for (int it = 0; it < 64; ++it) {
@@ -510,7 +551,7 @@ static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 
 // exact select on the few candidates around the cut.  *used = false: band miss, nothing decided.
 static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelState* out, bool* used) {
     *used = false;
-    const u64 n = s->count;
+    const u64 n = s->phys, n_live = s->count;   // stored entries (dead ones included) / live terms
     const int alt = s->cur ^ 1;
     u64 m64 = n / 8;
     if (m64 > SV_SAMPLE_MAX) m64 = SV_SAMPLE_MAX;
@@ -520,35 +561,35 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st);
     int in_alt = 0;
     s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 32, s->smp_scr, st, &in_alt);
-    s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n, max_terms, min_mass, s->mass_est, s->sctl, st);
+    s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st);
     cudaEvent_t e0, e1;
     prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
     if (e0) cudaEventRecord(e0, st);
     s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], st);
     if (e1) cudaEventRecord(e1, st);
-    s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n, max_terms, min_mass, st);
+    s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st);
     CHECK_LAUNCH();
     s->stats.passes += 1;
     int rc = read_back(s, out, s->sel, sizeof(SelState));
     if (rc != SV_OK) return rc;
     const u64 cand = out->n_total;
-    if (out->done == 3 || cand > n / 2) return SV_OK;   // band miss, or too many candidates to gain anything
-    rc = select_levels(s, s->keys[alt], s->amps[alt], cand, s->keys[alt] + cand, true, max_terms, min_mass, out);
+    if (out->done == 3 || cand > n_live / 2) return SV_OK;   // band miss, or too many candidates to gain anything
+    rc = select_levels(s, s->keys[alt], s->amps[alt], cand, cand, s->keys[alt] + cand, true, max_terms, min_mass, out);
     if (rc != SV_OK) return rc;
     if (out->done == 1) *used = true;
     return SV_OK;
 }
 
 static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
-    const u64 n = s->count;                   // callers have materialised any deferred truncation
-    if (n >= s->sample_min_terms) {
+    const u64 n = s->phys;                    // callers have materialised any deferred truncation; dead entries may remain
+    if (s->count >= s->sample_min_terms) {
         bool used = false;
         int rc = run_select_sampled(s, max_terms, min_mass, out, &used);
         if (rc != SV_OK || used) return rc;
         s->stats.fallbacks += 1;
     }
     // full-state select; the idle buffer holds the extracted tie keys
-    return select_levels(s, s->keys[s->cur], s->amps[s->cur], n, s->keys[s->cur ^ 1], false, max_terms, min_mass, out);
+    return select_levels(s, s->keys[s->cur], s->amps[s->cur], n, s->count, s->keys[s->cur ^ 1], false, max_terms, min_mass, out);
 }
 
 extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, double* kept_fraction) {
@@ -560,7 +601,8 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     if (kept_fraction) *kept_fraction = 1.0;
     const bool needK = max_terms != 0 && max_terms < s->count, needM = min_mass < 1.0;
     if (s->count == 0 || (!needK && !needM)) return SV_OK;
-    int rc = materialize(s);   // a second truncation in a row: apply the first one now
+    int rc = SV_OK;
+    if (s->defer.active) rc = materialize(s);   // a second truncation in a row: apply the first one now
     if (rc != SV_OK) return rc;
     SelState ss;
     rc = run_select(s, max_terms, min_mass, &ss);
@@ -586,8 +628,8 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
 
 extern "C" int sv_norm(sv_state* s, double* mass) {
     if (!s || !mass) return SV_ERR_INVALID_ARG;
-    { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
-    s->stats.launches += svk_norm(s->amps[s->cur], s->count, s->partials, s->d_norm, s->stream);
+    if (s->defer.active) { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
+    s->stats.launches += svk_norm(s->amps[s->cur], s->phys, s->partials, s->d_norm, s->stream);   // dead entries add 0
     CHECK_LAUNCH();
     return read_back(s, mass, s->d_norm, sizeof(double));
 }
@@ -623,7 +665,7 @@ struct TmpBuf {
 extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, double* probs, uint64_t* n_written) {
     if (!s) return SV_ERR_INVALID_ARG;
     s->err[0] = 0;
-    { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
+    if (s->defer.active) { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
     const u64 kk = k < s->count ? k : s->count;
     if (n_written) *n_written = kk;
     if (kk == 0) return SV_OK;
@@ -651,7 +693,7 @@ extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, do
     u32* vb = (u32*)b; b += a4;
     u32* scr = (u32*)b;
     cudaStream_t st = s->stream;
-    s->stats.launches += svk_gather_top(s->keys[s->cur], s->amps[s->cur], s->count, s->sel, use_sel, keymap_of(s), pat, lkey,
+    s->stats.launches += svk_gather_top(s->keys[s->cur], s->amps[s->cur], s->phys, s->sel, use_sel, keymap_of(s), pat, lkey,
                                         amp, s->d_count, kk, st);
     CHECK_LAUNCH();
     u64 got = 0;

@@ -85,6 +85,69 @@ __device__ __forceinline__ u64 lookback_exclusive_warp(u64* status, u32 tile, u6
     return excl;
 }
 
+// Two-level look-back.  A chain of one-warp windows resolves at most 32 tiles per L2 round
+// trip; a pass over 2^28 terms has 2.6e5 tiles of ~9000 cycles on ~600 resident blocks, i.e.
+// one tile every ~15 cycles -- more than such a chain can carry, and the tiles end up waiting
+// on the scan instead of on HBM.  Here tiles are grouped by 32: the last tile of a group to
+// publish its total also publishes the group's total, and a tile adds (a) the totals of the
+// tiles before it in its own group and (b) a windowed look-back over GROUP statuses, 32 groups
+// (1024 tiles) per round trip; both polls are in flight together.
+//   status[t]      AGG | total of tile t (never overwritten)
+//   gstat[g]       AGG | total of group g, later INCL | inclusive prefix through group g
+//   gacc[2g], [2g+1]  running sum / number of published tiles of group g
+// All three arrays must be zero at launch.  Called by all 32 lanes of ONE warp.
+__device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat, u64* gacc, u32 tile, u32 ntiles, u64 total) {
+    const int lane = threadIdx.x & 31;
+    const u32 g = tile >> 5, r = tile & 31u;
+    if (lane == 0) {
+        st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
+        atomicAdd(&gacc[2 * g], total);
+        __threadfence();
+        const u64 done = atomicAdd(&gacc[2 * g + 1], 1ull) + 1ull;
+        const u32 gsize = min(32u, ntiles - (g << 5));
+        if (done == gsize) {
+            __threadfence();
+            const u64 sum = atomicAdd(&gacc[2 * g], 0ull);
+            st_relaxed_u64(&gstat[g], SV_FLAG_AGG | sum);
+        }
+    }
+    u64 excl = 0;
+    bool own_done = (r == 0);
+    long long j = (long long)g - 1;          // newest group of the current window
+    bool groups_done = (g == 0);
+    for (;;) {
+        u64 v1 = SV_FLAG_AGG, v2 = SV_FLAG_INCL;
+        if (!own_done && lane < (int)r) v1 = ld_relaxed_u64(&status[(g << 5) + lane]);
+        const long long idx = j - lane;
+        if (!groups_done && idx >= 0) v2 = ld_relaxed_u64(&gstat[idx]);   // virtual groups < 0: inclusive 0
+        if (!own_done) {
+            if (__all_sync(0xffffffffu, (v1 >> 62) != 0)) {
+                u64 c = (lane < (int)r) ? (v1 & SV_VAL_MASK) : 0;
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+                excl += c;
+                own_done = true;
+            }
+        }
+        if (!groups_done) {
+            const u32 flagged = __ballot_sync(0xffffffffu, (v2 >> 62) != 0);
+            const u32 incl = __ballot_sync(0xffffffffu, (v2 >> 62) == 2);
+            const int first = incl ? (__ffs(incl) - 1) : 32;
+            const u32 need = (first >= 31) ? 0xffffffffu : ((2u << first) - 1u);
+            if ((flagged & need) == need) {
+                u64 c = (lane <= first) ? (v2 & SV_VAL_MASK) : 0;
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+                excl += c;
+                if (first < 32) groups_done = true; else j -= 32;
+            }
+        }
+        if (own_done && groups_done) break;
+    }
+    if (r == 0 && g > 0 && lane == 0) st_relaxed_u64(&gstat[g - 1], SV_FLAG_INCL | excl);   // = inclusive prefix of group g - 1
+    return excl;
+}
+
 // Exclusive block scan of one int per thread (blockDim.x == SV_THREADS).  `red` holds
 // SV_THREADS/32 + 1 ints.  Returns the exclusive prefix; *total gets the block sum.
 __device__ __forceinline__ int block_excl_scan(int v, int* red, int* total) {

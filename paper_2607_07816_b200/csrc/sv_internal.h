@@ -84,6 +84,8 @@ struct PendPred {
     KeyMap km;
 };
 
+int sv_sm_count();   // SMs of the current device (cached)
+
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
 
@@ -100,7 +102,7 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
 // pair == 0: pure move.  A pending truncation is applied while loading.  Writes the output
 // count to *d_count.
-int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair,
+int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
@@ -108,16 +110,19 @@ int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, 
 int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
                      const PendPred& pend, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
 
+// In-place: pending truncation (+ diagonal phases when has_phase) -> dropped terms become dead entries.
+int svk_diag_pend(const u64* keys, double2* amps, u64 n, const GateTab* tab, int has_phase, const PendPred& pend, cudaStream_t st);
+
 int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
 
-int svk_sel_init(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass, cudaStream_t st);
+int svk_sel_init(SelState* ss, u64* hist, u64 n_live, u64 max_terms, double min_mass, cudaStream_t st);
 int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const SelState* ss, u64* hist, cudaStream_t st);
 int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
                     cudaStream_t st);
 int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st);
 // sampled fast path: sample -> (sort) -> pivots -> classify -> seed the select state
 int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
-int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
+int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
                  cudaStream_t st);
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st);
 int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st);

@@ -22,12 +22,16 @@
 //             sorted, unique keys by construction.
 #include "sv_device.cuh"
 
+#ifndef BP_CTAS
+#define BP_CTAS 4
+#endif
 #define BP_VT 4
 #define BP_TILE (SV_THREADS * BP_VT)      // 1024 terms per tile
 #define BP_TNOM (BP_TILE - 2)             // nominal tile (boundaries are pulled back to a tuple start)
 #define BP_WARPS (SV_THREADS / 32)
 
 __device__ __forceinline__ bool pend_keep(const PendPred& pd, u64 stored_key, double2 a) {
+    if (a.x == 0.0 && a.y == 0.0) return false;   // dead entry
     const u64 pat = (u64)__double_as_longlong(prob_of(a));
     if (pat > pd.PT) return true;
     if (pat < pd.PT) return false;
@@ -35,55 +39,117 @@ __device__ __forceinline__ bool pend_keep(const PendPred& pd, u64 stored_key, do
     return logical_key(stored_key, pd.km) <= pd.KT;
 }
 
-template <bool PAIR>
-__global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+__device__ __forceinline__ void cp_async8(void* sdst, const void* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(sdst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* sdst, const void* gsrc) {
+    const unsigned d = (unsigned)__cvta_generic_to_shared(sdst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+struct Pieces3 { u64 ps0, ps1, ps2; int l0, l1, l2, cnt; bool oneblock; };
+__device__ __forceinline__ Pieces3 pieces_of(const u64* w) {   // w: desc[tile] (4 words) followed by desc[tile + 1]
+    Pieces3 q;
+    const u64 ia0 = w[0], ib0 = w[1], mid0 = w[2], e0 = w[3], ia1 = w[4], ib1 = w[5], mid1 = w[6], e1 = w[7];
+    q.oneblock = (e0 == e1);
+    if (q.oneblock) { q.ps0 = ia0; q.l0 = (int)(ia1 - ia0); q.ps1 = ib0; q.l1 = (int)(ib1 - ib0); q.ps2 = 0; q.l2 = 0; }
+    else { q.ps0 = ia0; q.l0 = (int)(mid0 - ia0); q.ps1 = ib0; q.l1 = (int)(ia1 - ib0); q.ps2 = mid1; q.l2 = (int)(ib1 - mid1); }
+    q.cnt = min(BP_TILE, q.l0 + q.l1 + q.l2);
+    return q;
+}
+
+#ifdef BP_X_TIMING
+__device__ unsigned long long g_bp_t[16];
+extern "C" void sv_debug_timing(unsigned long long* out, int reset) {
+    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_bp_t, z, sizeof(z)); return; }
+    cudaMemcpyFromSymbol(out, g_bp_t, sizeof(unsigned long long) * 16);
+}
+#define TSTAMP(k) do { if (tid == TWHO) { const long long t_ = clock64(); tacc[k] += t_ - tlast; tlast = t_; } } while (0)
+#else
+#define TSTAMP(k)
+#endif
+// FIXED: position-preserving variant for passes that map every stored entry to exactly one stored
+// entry (pure moves; gates whose 2x2 blocks are monomial, e.g. CNOT / Toffoli).  Terms dropped by a
+// pending truncation are carried as DEAD entries (amplitude 0+0i) instead of being squeezed out, so
+// the position of every output is known from the tile descriptor alone: no scan, no look-back.
+template <bool PAIR, bool FIXED>
+__global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
-                                                                u64* d_count, u64 cap, u32 ntiles) {
-    constexpr int OUTCAP = PAIR ? 2 * BP_TILE : BP_TILE;
+                                                                u32* tile_counter, u64* d_count, u64 cap, u32 ntiles) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* sta = reinterpret_cast<double2*>(smem_raw);      // staged outputs; its front doubles as the input tile
-    u64* stk = reinterpret_cast<u64*>(sta + OUTCAP);
+    double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer of the asynchronous loads (next tile)
+    double2* sta = La + BP_TILE;                               // work buffer: the partitioned tile, then the staged outputs
+    u64* Lk = reinterpret_cast<u64*>(sta + BP_TILE);
+    u64* stk = Lk + BP_TILE;
     double2* sa = sta;
     u64* sk = stk;
     __shared__ int red[BP_WARPS + 2];
     __shared__ int wc[BP_VT][BP_WARPS];
     __shared__ int s_nA;
+    __shared__ u64 s_desc[2][8];
     __shared__ u64 s_base;
     __shared__ double2 sU[64];      // [cx][xr][xc], ma = 1: up to 8 control patterns x 4
     __shared__ int s_cpos[SV_MAX_M], s_mc;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    // Tiles are taken in blockIdx order: a block only ever waits on lower-numbered blocks,
-    // which the hardware scheduler has already started.
-    const u32 tile = blockIdx.x;
     if (PAIR) {
         if (tid < 64) sU[tid] = gtab->U[tid];
         if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
         if (tid == 0) s_mc = gtab->mc;
     }
-    const TileDesc d0 = desc[tile], d1 = desc[tile + 1];
-    const bool oneblock = (d0.e == d1.e);
-    u64 ps0, ps1, ps2; int l0, l1, l2;
-    if (oneblock) { ps0 = d0.ia; l0 = (int)(d1.ia - d0.ia); ps1 = d0.ib; l1 = (int)(d1.ib - d0.ib); ps2 = 0; l2 = 0; }
-    else { ps0 = d0.ia; l0 = (int)(d0.mid - d0.ia); ps1 = d0.ib; l1 = (int)(d1.ia - d0.ib); ps2 = d1.mid; l2 = (int)(d1.ib - d1.mid); }
-    const int cnt = min(BP_TILE, l0 + l1 + l2);
     const u64 bit = 1ull << p;
+    const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
+    u64* gstat = status + ntiles;                       // group statuses, then the group accumulators
+    u64* gacc = gstat + ((ntiles + 31) >> 5);
+    // Persistent blocks (the grid is sized to be fully resident): tile t is taken by block
+    // t mod gridDim.x, so a block only ever waits on tiles that resident blocks have taken already.
+    // Software pipeline: while a tile is merged, scanned and written, the block's NEXT tile is
+    // already on its way from HBM into the landing buffer (cp.async, one thread per element), so
+    // every block keeps a full tile of loads in flight all the time.  Each thread later picks up
+    // exactly the elements it requested.  Tile descriptors travel one iteration ahead (s_desc).
+    auto issue_loads = [&](const Pieces3& q) {
+#pragma unroll
+        for (int r = 0; r < BP_VT; ++r) {
+            const int e = tid + r * SV_THREADS;
+            if (e < q.cnt) {
+                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
+                cp_async8(Lk + e, kin + g);
+                cp_async16(La + e, ain + g);
+            }
+        }
+        cp_async_commit();
+    };
+    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+    __syncthreads();
+    issue_loads(pieces_of(s_desc[0]));
+#ifdef BP_X_TIMING
+    long long tacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
+#endif
+    int par = 0;
+    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+    const u32 next = tile + gridDim.x;
+    u64 dnext = 0;
+    if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
+    const Pieces3 pc = pieces_of(s_desc[par]);
+    const int cnt = pc.cnt;
     int nA;
-    {   // coalesced loads of the contiguous pieces, all issued before any is used
+    {
+        TSTAMP(0);
+        cp_async_wait_all();      // this thread's own elements have landed
+        TSTAMP(1);
         u64 lk[BP_VT]; double2 la[BP_VT];
 #pragma unroll
         for (int r = 0; r < BP_VT; ++r) {
             const int e = tid + r * SV_THREADS;
             lk[r] = 0; la[r] = make_double2(0.0, 0.0);
-            if (e < cnt) {
-                const u64 g = e < l0 ? ps0 + e : (e < l0 + l1 ? ps1 + (e - l0) : ps2 + (e - l0 - l1));
-                lk[r] = ld_stream_u64(kin + g);
-                la[r] = ld_stream_d2(ain + g);
-            }
+            if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
         }
-        if (pd.active) {
+        if (pd.active) {          // pending truncation: dropped terms become 0+0i, survivors are scaled
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 if (tid + r * SV_THREADS < cnt) {
@@ -92,8 +158,8 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
                 }
             }
         }
-        if (oneblock) {   // piece 0 is all A, piece 1 all B: the load order is already A* | B*
-            nA = l0;
+        if (pc.oneblock) {   // piece 0 is all A, piece 1 all B: the load order is already A* | B*
+            nA = pc.l0;
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
@@ -129,7 +195,12 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
             }
         }
     }
-    __syncthreads();
+    if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+    TSTAMP(2);
+    __syncthreads();       // the work buffer is complete; every thread has emptied its landing slots
+    TSTAMP(3);
+    if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]));
+    TSTAMP(4);
     const int nB = cnt - nA;
     const u64* skB = sk + nA;
     const double2* saB = sa + nA;
@@ -145,9 +216,9 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
         }
         i = lo; j = diag - lo;
     }
+    TSTAMP(5);
     const int endpos = min(diag + BP_VT, cnt);
     int pos = diag;
-    const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
     // keys with bit p cleared never equal ~0: safe sentinels for an exhausted side
     u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
     u64 ok[BP_VT];
@@ -158,6 +229,7 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
         ++j; ++pos;
         kb = (j < nB) ? skB[j] : ~0ull;
     }
+    const int startpos = pos;
 #pragma unroll
     for (int v = 0; v < BP_VT; ++v) {
         ok[v] = 0; o0r[v] = o0i[v] = o1r[v] = o1i[v] = 0.0;
@@ -193,7 +265,10 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
                     cmul_acc(r0, m0, u[1].x, u[1].y, a.x, a.y);
                     cmul_acc(r1, m1, u[3].x, u[3].y, a.x, a.y);
                 }
-                const u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
+                u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
+                if (FIXED) {   // a pair always yields two entries, a lone term one (its nonzero row; row 0 if dead)
+                    if (has_partner) { f0 = 1; f1 = 1; } else { f0 = f1 ^ 1u; }
+                }
                 ok[v] = nk; o0r[v] = r0; o0i[v] = m0; o1r[v] = r1; o1i[v] = m1;
                 fl |= (f0 | (f1 << 1)) << (2 * v);
                 nout += (int)(f0 + f1);
@@ -201,59 +276,90 @@ __global__ void __launch_bounds__(SV_THREADS, 4) bitpass_kernel(const u64* __res
                 const double2 a = takeA ? sa[i] : saB[j];
                 if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
                 ++pos;
-                const u32 f0 = !(a.x == 0.0 && a.y == 0.0);
+                const u32 f0 = FIXED ? 1u : (u32)!(a.x == 0.0 && a.y == 0.0);
                 ok[v] = nk | (takeA ? 0ull : 1ull); o0r[v] = a.x; o0i[v] = a.y;
                 fl |= f0 << (2 * v);
                 nout += (int)f0;
             }
         }
     }
-    int total;
-    const int excl = block_excl_scan(nout, red, &total);   // its barriers also retire every read of the input tile
-    if (tid < 32) {
-        const u64 ex = lookback_exclusive_warp(status, tile, (u64)total);
-        if (tid == 0) {
-            s_base = ex;
-            if (tile == ntiles - 1) *d_count = ex + (u64)total;
-        }
-    }
-    {   // stage the outputs in output order (the staging area aliases the consumed input tile)
-        int off = excl;
+    TSTAMP(6);
+    int total, excl;
+    if (FIXED) { excl = startpos; total = cnt; __syncthreads(); }   // the barrier retires every read of the input tile
+    else excl = block_excl_scan(nout, red, &total);
+    TSTAMP(7);   // its barriers also retire every read of the input tile
+    // stage the outputs in output order (the staging area aliases the consumed input tile and holds
+    // BP_TILE outputs: a gate that doubles the tile is written in two rounds), store them coalesced
+    for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_TILE) {
+        if (h0 > 0) __syncthreads();
+        {
+            int off = excl - h0;
 #pragma unroll
-        for (int v = 0; v < BP_VT; ++v) {
-            const u32 f = (fl >> (2 * v)) & 3u;
-            if (f & 1u) { stk[off] = ok[v]; sta[off] = make_double2(o0r[v], o0i[v]); ++off; }
-            if (PAIR && (f & 2u)) { stk[off] = ok[v] | 1ull; sta[off] = make_double2(o1r[v], o1i[v]); ++off; }
+            for (int v = 0; v < BP_VT; ++v) {
+                const u32 f = (fl >> (2 * v)) & 3u;
+                if (f & 1u) {
+                    if ((unsigned)off < (unsigned)BP_TILE) { stk[off] = ok[v]; sta[off] = make_double2(o0r[v], o0i[v]); }
+                    ++off;
+                }
+                if (PAIR && (f & 2u)) {
+                    if ((unsigned)off < (unsigned)BP_TILE) { stk[off] = ok[v] | 1ull; sta[off] = make_double2(o1r[v], o1i[v]); }
+                    ++off;
+                }
+            }
+        }
+        if (FIXED) {
+            if (tid == 0) s_base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
+        } else if (h0 == 0 && tid < 32) {
+            const u64 ex = lookback_exclusive_2level(status, gstat, gacc, tile, ntiles, (u64)total);
+            if (tid == 0) {
+                s_base = ex;
+                if (tile == ntiles - 1) *d_count = ex + (u64)total;
+            }
+        }
+        TSTAMP(8);
+        __syncthreads();
+        TSTAMP(9);
+        const u64 base = s_base + (u64)h0;
+        const int m = min(total - h0, BP_TILE);
+        for (int idx = tid; idx < m; idx += SV_THREADS) {
+            const u64 g = base + (u64)idx;
+            if (g < cap) { st_stream_u64(kout + g, stk[idx]); st_stream_d2(aout + g, sta[idx]); }
         }
     }
-    __syncthreads();
-    const u64 base = s_base;
-    for (int idx = tid; idx < total; idx += SV_THREADS) {
-        const u64 g = base + (u64)idx;
-        if (g < cap) { st_stream_u64(kout + g, stk[idx]); st_stream_d2(aout + g, sta[idx]); }
+    __syncthreads();   // the staging area is the next tile's input buffer
     }
+#ifdef BP_X_TIMING
+    if (tid == TWHO && blockIdx.x % 37 == 0) for (int k = 0; k < 10; ++k) atomicAdd(&g_bp_t[k], (unsigned long long)tacc[k]);
+#endif
 }
 
-template <bool PAIR>
+template <bool PAIR, bool FIXED>
 static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
-                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
-    const size_t smem = (size_t)(PAIR ? 2 : 1) * BP_TILE * 24;
+                           const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
+    const size_t smem = (size_t)2 * BP_TILE * 24;   // landing buffer + work / staging buffer
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
-    bitpass_kernel<PAIR><<<ntiles, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles);
+    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<PAIR, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    static int per_sm = 0;
+    if (!per_sm) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<PAIR, FIXED>, SV_THREADS, smem);
+        if (per_sm < 1) per_sm = 1;
+    }
+    const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
+    bitpass_kernel<PAIR, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles);
 }
 
-int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair,
+int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
-    (void)tile_counter;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
-    cudaMemsetAsync(status, 0, (size_t)ntiles * sizeof(u64), st);
+    cudaMemsetAsync(status, 0, ((size_t)ntiles + 3 * ((ntiles + 31) / 32) + 8) * sizeof(u64), st);   // tile + group statuses + group accumulators
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
-    if (pair) launch_bitpass<true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st);
-    else launch_bitpass<false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st);
+#define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles, st)
+    if (pair) { if (fixed) SV_BP(true, true); else SV_BP(true, false); }
+    else { if (fixed) SV_BP(false, true); else SV_BP(false, false); }
+#undef SV_BP
     if (e1) cudaEventRecord(e1, st);
     return launches + 1;
 }

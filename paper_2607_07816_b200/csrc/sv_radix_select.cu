@@ -145,7 +145,11 @@ __global__ void __launch_bounds__(SV_THREADS) sel_pass_kernel(const double2* __r
             v[r] = 0;
             if (ok[r]) {
                 if (MODE == 2) v[r] = ld_stream_u64(lkeys + i);
-                else v[r] = (u64)__double_as_longlong(prob_of(ld_stream_d2(amps + i)));
+                else {
+                    const double2 a = ld_stream_d2(amps + i);
+                    v[r] = (u64)__double_as_longlong(prob_of(a));
+                    if (a.x == 0.0 && a.y == 0.0) ok[r] = false;   // dead entry
+                }
             }
         }
 #pragma unroll
@@ -228,7 +232,11 @@ __global__ void __launch_bounds__(SV_THREADS) sel_extract_kernel(const u64* __re
 #pragma unroll
         for (int r = 0; r < SP_IT; ++r) {
             const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
-            pat[r] = (i < n) ? (u64)__double_as_longlong(prob_of(ld_stream_d2(amps + i))) : ~0ull;
+            pat[r] = ~0ull;
+            if (i < n) {
+                const double2 a = ld_stream_d2(amps + i);
+                if (!(a.x == 0.0 && a.y == 0.0)) pat[r] = (u64)__double_as_longlong(prob_of(a));   // dead entries never tie
+            }
         }
 #pragma unroll
         for (int r = 0; r < SP_IT; ++r) {

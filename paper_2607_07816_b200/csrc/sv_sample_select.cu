@@ -33,36 +33,49 @@ __global__ void __launch_bounds__(SV_THREADS) ss_sample_kernel(const double2* __
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= M) return;
     const u64 i = (u64)(((u128)j * n) / M);
-    smp[j] = (u64)__double_as_longlong(prob_of(ld_stream_d2(amps + i))) >> 32;
+    const double2 a = ld_stream_d2(amps + i);
+    // dead entries (0+0i) sort to the front as key 0; live terms get their pattern's top bits + 1
+    smp[j] = (a.x == 0.0 && a.y == 0.0) ? 0ull : (((u64)__double_as_longlong(prob_of(a)) >> 32) + 1ull);
 }
 
 __device__ __forceinline__ double smp_prob(u64 top32) {   // mid-point of the values sharing these top bits
     return __longlong_as_double((long long)((top32 << 32) | 0x80000000ull));
 }
 
-// One block of 1024 threads.  smp[0..M) ascending.  Warp w owns the contiguous range
-// [w * per, (w + 1) * per) and walks it 32 elements at a time.
-__global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ smp, u32 M, u64 n, u64 max_terms,
+// One block of 1024 threads.  smp[0..M) ascending; the first z entries are 0 (dead sample points),
+// the live ones hold (top 32 pattern bits) + 1.  Warp w owns a contiguous range of the live part
+// and walks it 32 elements at a time.
+__global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ smp, u32 M, u64 n_live, u64 max_terms,
                                                         double min_mass, double mass_est, SampleCtl* __restrict__ ctl) {
     __shared__ double wsum[32];
     __shared__ u32 cnt[2][3];   // [sweep][threshold]
+    __shared__ u32 s_z;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const u32 per = (M + 31) / 32;
-    const u32 b0 = min(M, warp * per), b1 = min(M, b0 + per);
+    if (threadIdx.x == 0) {   // z = number of dead sample points (lower bound of 1)
+        u32 lo = 0, hi = M;
+        while (lo < hi) { const u32 mid = (lo + hi) >> 1; if (smp[mid] == 0) lo = mid + 1; else hi = mid; }
+        s_z = lo;
+    }
     if (threadIdx.x < 6) cnt[threadIdx.x / 3][threadIdx.x % 3] = 0;
+    __syncthreads();
+    const u32 z = s_z, Ml = M - z;
+    const u64* live = smp + z;
+    const u32 per = (Ml + 31) / 32;
+    const u32 b0 = min(Ml, warp * per), b1 = min(Ml, b0 + per);
     double s = 0.0;
-    for (u32 i = b0 + lane; i < b1; i += 32) s += smp_prob(smp[i]);
+    for (u32 i = b0 + lane; i < b1; i += 32) s += smp_prob(live[i] - 1);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
     if (lane == 0) wsum[warp] = s;
     __syncthreads();
     double pre = 0.0, T = 0.0;
     for (int w = 0; w < 32; ++w) { if (w < warp) pre += wsum[w]; T += wsum[w]; }
-    const bool mass_on = min_mass < 1.0;
+    const bool mass_on = min_mass < 1.0 && Ml > 0;
     // mass to drop, in sample units (the tail is made of small terms, so the scaled sample tail
     // estimates it well even when a few heavy terms carry most of S)
-    const double S_est = (mass_est == mass_est && mass_est > 0.0) ? mass_est : T * ((double)n / (double)M);
-    const double X0 = (1.0 - min_mass) * S_est * ((double)M / (double)n);
+    const double per_sample = (double)n_live / (double)max(Ml, 1u);
+    const double S_est = (mass_est == mass_est && mass_est > 0.0) ? mass_est : T * per_sample;
+    const double X0 = (1.0 - min_mass) * S_est / per_sample;
     // sweep 1: a0 = sample elements in the nominal tail; sweep 2: the band X0 / (1 + eps) .. X0 * (1 + eps)
     // with eps ~ 10 / sqrt(a0) (the relative noise of a tail sum of a0 sampled terms)
     double X[3] = {X0, X0, X0};
@@ -71,11 +84,11 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
         double run = pre;
         for (u32 i0 = b0; i0 < b1; i0 += 32) {
             const u32 i = i0 + lane;
-            const double v = (i < b1) ? smp_prob(smp[i]) : 0.0;
+            const double v = (i < b1) ? smp_prob(live[i] - 1) : 0.0;
             double inc = v;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-            const double incl = run + inc;   // mass of the sample's i + 1 smallest elements
+            const double incl = run + inc;   // mass of the sample's i + 1 smallest live elements
             if (i < b1) {
 #pragma unroll
                 for (int k = 0; k < 3; ++k) c[k] += (incl <= X[k]) ? 1u : 0u;
@@ -98,7 +111,7 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
     }
     __syncthreads();
     if (threadIdx.x != 0) return;
-    // numbers of (smallest) sample elements certainly / possibly dropped
+    // numbers of (smallest) live sample elements certainly / possibly dropped
     long long lo_idx = 0, hi_idx = 0;
     if (mass_on) {
         const long long a0 = cnt[0][1];
@@ -106,18 +119,18 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
         long long a_hi = (a0 < 128) ? max((long long)cnt[1][2] + 8, 2 * a0 + 64) : (long long)cnt[1][2] + 8;
         lo_idx = max(lo_idx, a_lo); hi_idx = max(hi_idx, a_hi);
     }
-    if (max_terms != 0 && max_terms < n) {
-        const double q = (double)(n - max_terms) / (double)n;
-        const double d = q * (double)M;
+    if (max_terms != 0 && max_terms < n_live) {
+        const double q = (double)(n_live - max_terms) / (double)n_live;
+        const double d = q * (double)Ml;
         const double dl = 6.0 * sqrt(fmax(d * (1.0 - q), 0.0)) + 8.0;
         lo_idx = max(lo_idx, (long long)floor(d - dl));
         hi_idx = max(hi_idx, (long long)ceil(d + dl));
     }
     SampleCtl c;
     memset(&c, 0, sizeof(c));
-    c.P_lo = (lo_idx <= 0) ? 0ull : (smp[min((long long)M, lo_idx) - 1] << 32);
-    c.P_hi = (hi_idx >= (long long)M) ? ~0ull : ((smp[hi_idx] << 32) | 0xffffffffull);
-    int er = (int)(smp[M - 1] >> 20) + 12;
+    c.P_lo = (lo_idx <= 0 || Ml == 0) ? 0ull : ((live[min((long long)Ml, lo_idx) - 1] - 1) << 32);
+    c.P_hi = (hi_idx >= (long long)Ml) ? ~0ull : (((live[hi_idx] - 1) << 32) | 0xffffffffull);
+    int er = (Ml ? (int)((live[Ml - 1] - 1) >> 20) : 1023) + 12;
     c.Eref = er > 2046 ? 2046 : er;
     *ctl = c;
 }
@@ -170,7 +183,7 @@ __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __re
 #pragma unroll
         for (int r = 0; r < SC_IT; ++r) {
             const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
-            const bool ok = i < n;
+            const bool ok = i < n && !(a[r].x == 0.0 && a[r].y == 0.0);   // dead entries take no part
             const u64 pat = (u64)__double_as_longlong(prob_of(a[r]));
             const u128 f = ok ? fx_of(pat, Eref, ovf) : (u128)0;
             tot += f;
@@ -213,9 +226,9 @@ int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st) 
     ss_sample_kernel<<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(amps, n, M, smp);
     return 1;
 }
-int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
+int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
                  cudaStream_t st) {
-    ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n, max_terms, min_mass, mass_est, ctl);
+    ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n_live, max_terms, min_mass, mass_est, ctl);
     return 1;
 }
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st) {

@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(SV_THREADS) compact_kernel(const u64* __restri
     __syncthreads();
     const u32 tile = s_tile;
     const u64 PT = pd.PT, KT = pd.KT;
-    const double scale = pd.scale;
+    const double scale = pd.active ? pd.scale : 1.0;
     const u64 t0 = (u64)tile * (SV_THREADS * SV_CMP_IT);
     u64 k[SV_CMP_IT]; double2 a[SV_CMP_IT]; u32 ball[SV_CMP_IT];
 #pragma unroll
@@ -90,7 +90,8 @@ __global__ void __launch_bounds__(SV_THREADS) compact_kernel(const u64* __restri
     for (int it = 0; it < SV_CMP_IT; ++it) {
         const u64 i = t0 + (u64)it * SV_THREADS + tid;
         bool keep = false;
-        if (i < n) keep = sel_keep((u64)__double_as_longlong(prob_of(a[it])), k[it], PT, KT, pd.km);
+        if (i < n && !(a[it].x == 0.0 && a[it].y == 0.0))   // dead entries (0+0i) are squeezed out
+            keep = !pd.active || sel_keep((u64)__double_as_longlong(prob_of(a[it])), k[it], PT, KT, pd.km);
         const u32 b = __ballot_sync(0xffffffffu, keep);
         ball[it] = b;
         if (lane == 0) wcnt[it][warp] = __popc(b);
@@ -152,6 +153,59 @@ int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aou
     return launch_compact(true, kin, ain, kout, aout, n, pend, tab, status, tile_counter, d_count, st);
 }
 
+// Diagonal gate fused with a pending truncation, IN PLACE: survivors are scaled and multiplied by
+// their phase, dropped terms become dead entries (0+0i) that later passes skip or squeeze out.
+// 40 B per term (key read, amplitude read + write), no scan.
+__global__ void __launch_bounds__(SV_THREADS) diag_pend_kernel(const u64* __restrict__ keys, double2* __restrict__ amps, u64 n,
+                                                               PendPred pd, const GateTab* __restrict__ gtab, int has_phase) {
+    __shared__ double2 sd[16];
+    __shared__ int s_cpos[SV_MAX_M], s_mc;
+    if (threadIdx.x < 16) sd[threadIdx.x] = gtab->U[threadIdx.x];
+    if (threadIdx.x < SV_MAX_M) s_cpos[threadIdx.x] = gtab->ctrl_pos[threadIdx.x];
+    if (threadIdx.x == 0) s_mc = gtab->mc;
+    __syncthreads();
+    const int mc = has_phase ? s_mc : 0;
+    const u64 PT = pd.PT, KT = pd.KT;
+    const double scale = pd.scale;
+    const u64 chunk = (u64)SV_THREADS * 4;
+    const u64 nchunks = (n + chunk - 1) / chunk;
+    for (u64 c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        u64 k[4]; double2 a[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            k[r] = 0; a[r] = make_double2(0.0, 0.0);
+            if (i < n) { k[r] = ld_stream_u64(keys + i); a[r] = amps[i]; }
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            if (i >= n || (a[r].x == 0.0 && a[r].y == 0.0)) continue;   // dead stays dead (nothing to write)
+            double2 o = make_double2(0.0, 0.0);
+            if (sel_keep((u64)__double_as_longlong(prob_of(a[r])), k[r], PT, KT, pd.km)) {
+                o.x = __dmul_rn(a[r].x, scale); o.y = __dmul_rn(a[r].y, scale);
+                if (has_phase) {
+                    int cx = 0;
+                    for (int j = 0; j < mc; ++j) cx |= (int)((k[r] >> s_cpos[j]) & 1ull) << j;
+                    const double2 u = sd[cx];
+                    double2 t;
+                    t.x = __dsub_rn(__dmul_rn(u.x, o.x), __dmul_rn(u.y, o.y));
+                    t.y = __dadd_rn(__dmul_rn(u.x, o.y), __dmul_rn(u.y, o.x));
+                    o = t;
+                }
+            }
+            amps[i] = o;
+        }
+    }
+}
+int svk_diag_pend(const u64* keys, double2* amps, u64 n, const GateTab* tab, int has_phase, const PendPred& pend, cudaStream_t st) {
+    if (n == 0) return 0;
+    u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
+    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    diag_pend_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, pend, tab, has_phase);
+    return 1;
+}
+
 // ---------------------------------------------------------------------------------------
 // readout support: gather the selected terms as (p pattern, logical key, amplitude)
 // ---------------------------------------------------------------------------------------
@@ -165,6 +219,7 @@ __global__ void __launch_bounds__(SV_THREADS) gather_top_kernel(const u64* __res
         const u64 k = keys[i];
         const double2 a = amps[i];
         const u64 pat = (u64)__double_as_longlong(prob_of(a));
+        if (a.x == 0.0 && a.y == 0.0) continue;   // dead entry
         if (!use_sel || sel_keep(pat, k, PT, KT, km)) {
             const u64 pos = atomicAdd(d_count, 1ull);
             if (pos < kmax) { o_pat[pos] = pat; o_lkey[pos] = logical_key(k, km); o_amp[pos] = a; }
@@ -193,7 +248,7 @@ __global__ void check_kernel(const u64* __restrict__ keys, const double2* __rest
         bool b = false;
         if (i > 0 && keys[i - 1] >= k) b = true;
         if (nq < 64 && (k >> nq) != 0) b = true;
-        if (a.x == 0.0 && a.y == 0.0) b = true;
+        if (a.x == 0.0 && a.y == 0.0) b = true;   // callers compact dead entries away first
         if (b) atomicExch(bad, 1);
     }
 }
