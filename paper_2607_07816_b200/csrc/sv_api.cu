@@ -474,7 +474,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     }
     if (ma == 1 && monomial && few_dead(s)) {
         prof_slot(s, SV_K_GROUP, 48.0 * (double)s->phys, &ge0, &ge1);
-        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 1,
+        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 2, 1,
                                          s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
         CHECK_LAUNCH();
         s->stats.passes += 1;

@@ -75,12 +75,17 @@ extern "C" void sv_debug_timing(unsigned long long* out, int reset) {
 // entry (pure moves; gates whose 2x2 blocks are monomial, e.g. CNOT / Toffoli).  Terms dropped by a
 // pending truncation are carried as DEAD entries (amplitude 0+0i) instead of being squeezed out, so
 // the position of every output is known from the tile descriptor alone: no scan, no look-back.
-template <bool PAIR, bool FIXED>
+// MODE 0: pure move.  MODE 1: gate with one active bit (2x2 mat-vec per tuple).  MODE 2 (FIXED only):
+// the same for MONOMIAL 2x2 blocks: every entry maps to one entry (its bit kept or flipped, times a
+// phase), so the pass is a move whose partners may trade places -- no tuple arithmetic.
+template <int MODE, bool FIXED>
 __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
                                                                 u32* tile_counter, u64* d_count, u64 cap, u32 ntiles) {
+    constexpr bool PAIR = (MODE == 1);
+    constexpr bool PERM = (MODE == 2);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer of the asynchronous loads (next tile)
     double2* sta = La + BP_TILE;                               // work buffer: the partitioned tile, then the staged outputs
@@ -97,10 +102,22 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     __shared__ int s_cpos[SV_MAX_M], s_mc;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    if (PAIR) {
+    __shared__ int s_sw[8], s_unit;   // PERM: block cx swaps the bit; every nonzero entry is exactly 1
+    if (PAIR || PERM) {
         if (tid < 64) sU[tid] = gtab->U[tid];
         if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
         if (tid == 0) s_mc = gtab->mc;
+        if (PERM && tid == 0) {
+            int unit = 1;
+            for (int cx = 0; cx < 8; ++cx) {
+                const double2* u = &gtab->U[cx << 2];
+                const int sw = (u[0].x == 0.0 && u[0].y == 0.0) ? 1 : 0;
+                s_sw[cx] = sw;
+                const double2 x = sw ? u[1] : u[0], y = sw ? u[2] : u[3];
+                if (cx < (1 << gtab->mc) && !(x.x == 1.0 && x.y == 0.0 && y.x == 1.0 && y.y == 0.0)) unit = 0;
+            }
+            s_unit = unit;
+        }
     }
     const u64 bit = 1ull << p;
     const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
@@ -230,14 +247,34 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
         kb = (j < nB) ? skB[j] : ~0ull;
     }
     const int startpos = pos;
+    u64 lastA = (PERM && i > 0) ? sk[i - 1] : ~0ull;   // PERM: a B term's partner is the A term merged just before it
+    int opos[BP_VT];
 #pragma unroll
     for (int v = 0; v < BP_VT; ++v) {
-        ok[v] = 0; o0r[v] = o0i[v] = o1r[v] = o1i[v] = 0.0;
+        ok[v] = 0; o0r[v] = o0i[v] = o1r[v] = o1i[v] = 0.0; opos[v] = -1;
         if (pos < endpos) {
             const bool takeA = ka <= kb;
             const u64 k = takeA ? ka : kb;
             const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
-            if (PAIR) {
+            if (PERM) {
+                const int c = takeA ? 0 : 1;
+                const bool partner = takeA ? (kb == k) : (lastA == k);
+                double2 a = takeA ? sa[i] : saB[j];
+                if (takeA) { ++i; lastA = k; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
+                int cx = 0;
+                const int mc = s_mc;
+                for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
+                const int sw = s_sw[cx], row = c ^ sw;
+                if (!s_unit) {
+                    const double2 u = sU[(cx << 2) | (row << 1) | c];
+                    const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
+                    const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
+                    a.x = __dadd_rn(0.0, pr); a.y = __dadd_rn(0.0, pi);
+                }
+                ok[v] = nk | (u64)row; o0r[v] = a.x; o0i[v] = a.y;
+                opos[v] = pos + ((partner && sw) ? (c ? -1 : 1) : 0);   // partners that swap rows trade places
+                ++pos;
+            } else if (PAIR) {
                 double2 a, pa = make_double2(0.0, 0.0);
                 bool has_partner = false;
                 if (takeA) {
@@ -292,7 +329,11 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     // BP_TILE outputs: a gate that doubles the tile is written in two rounds), store them coalesced
     for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_TILE) {
         if (h0 > 0) __syncthreads();
-        {
+        if (PERM) {
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (opos[v] >= 0) { stk[opos[v]] = ok[v]; sta[opos[v]] = make_double2(o0r[v], o0i[v]); }
+        } else {
             int off = excl - h0;
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v) {
@@ -333,19 +374,19 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
 #endif
 }
 
-template <bool PAIR, bool FIXED>
+template <int MODE, bool FIXED>
 static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                            const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
     const size_t smem = (size_t)2 * BP_TILE * 24;   // landing buffer + work / staging buffer
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<PAIR, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
     if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<PAIR, FIXED>, SV_THREADS, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<MODE, FIXED>, SV_THREADS, smem);
         if (per_sm < 1) per_sm = 1;
     }
     const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    bitpass_kernel<PAIR, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles);
+    bitpass_kernel<MODE, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles);
 }
 
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
@@ -357,8 +398,9 @@ int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u6
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
 #define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles, st)
-    if (pair) { if (fixed) SV_BP(true, true); else SV_BP(true, false); }
-    else { if (fixed) SV_BP(false, true); else SV_BP(false, false); }
+    if (pair == 2) SV_BP(2, true);                       // monomial blocks: always position preserving
+    else if (pair) { if (fixed) SV_BP(1, true); else SV_BP(1, false); }
+    else { if (fixed) SV_BP(0, true); else SV_BP(0, false); }
 #undef SV_BP
     if (e1) cudaEventRecord(e1, st);
     return launches + 1;
