@@ -87,30 +87,21 @@ __device__ __forceinline__ u64 lookback_exclusive_warp(u64* status, u32 tile, u6
 
 // Two-level look-back.  A chain of one-warp windows resolves at most 32 tiles per L2 round
 // trip; a pass over 2^28 terms has 2.6e5 tiles of ~9000 cycles on ~600 resident blocks, i.e.
-// one tile every ~15 cycles -- more than such a chain can carry, and the tiles end up waiting
-// on the scan instead of on HBM.  Here tiles are grouped by 32: the last tile of a group to
-// publish its total also publishes the group's total, and a tile adds (a) the totals of the
-// tiles before it in its own group and (b) a windowed look-back over GROUP statuses, 32 groups
-// (1024 tiles) per round trip; both polls are in flight together.
-//   status[t]      AGG | total of tile t (never overwritten)
-//   gstat[g]       AGG | total of group g, later INCL | inclusive prefix through group g
-//   gacc[2g], [2g+1]  running sum / number of published tiles of group g
-// All three arrays must be zero at launch.  Called by all 32 lanes of ONE warp.
-__device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat, u64* gacc, u32 tile, u32 ntiles, u64 total) {
+// one tile every ~15 cycles -- more than such a chain can carry.  Here tiles are grouped by
+// 32.  A tile adds (a) the totals of the tiles before it in its own group and (b) a windowed
+// look-back over GROUP statuses, 32 groups (1024 tiles) per round trip; both polls are in
+// flight together.  The last tile of a group (by index) knows the group's total once (a) is
+// complete and publishes it; the first tile of the next group later upgrades it to the
+// inclusive prefix.  No atomics, one store to publish, one or two polls to resolve.
+//   status[t]   AGG | total of tile t (never overwritten)
+//   gstat[g]    AGG | total of group g, later INCL | inclusive prefix through group g
+// Both arrays must be zero at launch.  Called by all 32 lanes of ONE warp.
+__device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat, u32 tile, u32 ntiles, u64 total) {
     const int lane = threadIdx.x & 31;
     const u32 g = tile >> 5, r = tile & 31u;
-    if (lane == 0) {
-        st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
-        atomicAdd(&gacc[2 * g], total);
-        __threadfence();
-        const u64 done = atomicAdd(&gacc[2 * g + 1], 1ull) + 1ull;
-        const u32 gsize = min(32u, ntiles - (g << 5));
-        if (done == gsize) {
-            __threadfence();
-            const u64 sum = atomicAdd(&gacc[2 * g], 0ull);
-            st_relaxed_u64(&gstat[g], SV_FLAG_AGG | sum);
-        }
-    }
+    if (lane == 0) st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
+    const bool closes_group = (r == 31u) || (tile == ntiles - 1);
+    if (r == 0 && closes_group && lane == 0) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | total);   // a group of one tile
     u64 excl = 0;
     bool own_done = (r == 0);
     long long j = (long long)g - 1;          // newest group of the current window
@@ -127,6 +118,7 @@ __device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat
                 for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
                 excl += c;
                 own_done = true;
+                if (closes_group && lane == 0) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | (c + total));
             }
         }
         if (!groups_done) {
@@ -144,7 +136,7 @@ __device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat
         }
         if (own_done && groups_done) break;
     }
-    if (r == 0 && g > 0 && lane == 0) st_relaxed_u64(&gstat[g - 1], SV_FLAG_INCL | excl);   // = inclusive prefix of group g - 1
+    if (r == 0 && g > 0 && lane == 0) st_relaxed_u64(&gstat[g - 1], SV_FLAG_INCL | excl);   // = inclusive prefix through group g - 1
     return excl;
 }
 

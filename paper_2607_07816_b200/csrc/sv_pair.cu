@@ -121,8 +121,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     }
     const u64 bit = 1ull << p;
     const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
-    u64* gstat = status + ntiles;                       // group statuses, then the group accumulators
-    u64* gacc = gstat + ((ntiles + 31) >> 5);
+    u64* gstat = status + ntiles;                       // group statuses follow the tile statuses
     // Persistent blocks (the grid is sized to be fully resident): tile t is taken by block
     // t mod gridDim.x, so a block only ever waits on tiles that resident blocks have taken already.
     // Software pipeline: while a tile is merged, scanned and written, the block's NEXT tile is
@@ -351,7 +350,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
         if (FIXED) {
             if (tid == 0) s_base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
         } else if (h0 == 0 && tid < 32) {
-            const u64 ex = lookback_exclusive_2level(status, gstat, gacc, tile, ntiles, (u64)total);
+            const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
             if (tid == 0) {
                 s_base = ex;
                 if (tile == ntiles - 1) *d_count = ex + (u64)total;
@@ -394,7 +393,7 @@ int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u6
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
-    cudaMemsetAsync(status, 0, ((size_t)ntiles + 3 * ((ntiles + 31) / 32) + 8) * sizeof(u64), st);   // tile + group statuses + group accumulators
+    cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
 #define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles, st)

@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(SV_THREADS) compact_kernel(const u64* __restri
         const int ex = inc - c0 - c1;
         __syncwarp();
         wcnt[e0 >> 3][e0 & 7] = ex; wcnt[e1 >> 3][e1 & 7] = ex + c0;
-        const u64 excl = lookback_exclusive_warp(status, tile, (u64)tot);
+        const u64 excl = lookback_exclusive_2level(status, status + ntiles, tile, ntiles, (u64)tot);
         if (lane == 0) { s_base = excl; if (tile == ntiles - 1) *d_count = excl + (u64)tot; }
     }
     __syncthreads();
@@ -138,7 +138,7 @@ static int launch_compact(bool diag, const u64* kin, const double2* ain, u64* ko
                           const GateTab* tab, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st) {
     if (n == 0) return 0;
     const u32 ntiles = (u32)((n + SV_THREADS * SV_CMP_IT - 1) / (SV_THREADS * SV_CMP_IT));
-    cudaMemsetAsync(status, 0, (size_t)ntiles * sizeof(u64), st);
+    cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
     cudaMemsetAsync(tile_counter, 0, sizeof(u32), st);
     if (diag) compact_kernel<true><<<ntiles, SV_THREADS, 0, st>>>(kin, ain, kout, aout, n, pd, tab, status, tile_counter, d_count, ntiles);
     else compact_kernel<false><<<ntiles, SV_THREADS, 0, st>>>(kin, ain, kout, aout, n, pd, tab, status, tile_counter, d_count, ntiles);
