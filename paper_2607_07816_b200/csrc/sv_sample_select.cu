@@ -163,12 +163,32 @@ __device__ __forceinline__ void atomic_add_u128(u64* lohi, u128 v) {   // lohi[0
 }
 
 #define SC_IT 4
+#define SC_WBUF 96       // candidate slots per warp (flushed when more than 64 are waiting)
+// Candidates are rare (a few per cent) but almost every warp meets one every few iterations.  They
+// are parked in a warp-private shared-memory buffer (amplitude + index) and flushed 64+ at a
+// time: one global atomic and one batch of key loads per flush instead of one per iteration.
 __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
                                                                  u64 n, SampleCtl* __restrict__ ctl, u64* __restrict__ ckeys,
                                                                  double2* __restrict__ camps) {
+    __shared__ double2 s_ba[SV_THREADS / 32][SC_WBUF];
+    __shared__ u64 s_bi[SV_THREADS / 32][SC_WBUF];
     const u64 P_hi = ctl->P_hi, P_lo = ctl->P_lo;
     const int Eref = ctl->Eref;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double2* ba = s_ba[warp];
+    u64* bi = s_bi[warp];
+    int nbuf = 0;            // warp-uniform
+    auto flush = [&]() {
+        u64 base = 0;
+        if (lane == 0) base = atomicAdd(&ctl->cand_cnt, (u64)nbuf);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        for (int q = lane; q < nbuf; q += 32) {
+            ckeys[base + q] = keys[bi[q]];
+            camps[base + q] = ba[q];
+        }
+        __syncwarp();
+        nbuf = 0;
+    };
     u128 tot = 0, abv = 0;
     u32 n_abv = 0, n_blw = 0, ovf = 0;
     const u64 chunk = (u64)SV_THREADS * SC_IT;
@@ -193,18 +213,17 @@ __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __re
             const bool cand = ok && !above && !below;
             const u32 grp = __ballot_sync(0xffffffffu, cand);
             if (grp) {
-                u64 base = 0;
-                const int ldr = __ffs(grp) - 1;
-                if (lane == ldr) base = atomicAdd(&ctl->cand_cnt, (u64)__popc(grp));
-                base = __shfl_sync(0xffffffffu, base, ldr);
                 if (cand) {
-                    const u64 pos = base + __popc(grp & ((1u << lane) - 1u));
-                    ckeys[pos] = keys[i];
-                    camps[pos] = a[r];
+                    const int q = nbuf + __popc(grp & ((1u << lane) - 1u));
+                    ba[q] = a[r]; bi[q] = i;
                 }
+                nbuf += __popc(grp);
+                __syncwarp();
+                if (nbuf > SC_WBUF - 32) flush();
             }
         }
     }
+    if (nbuf) flush();
     tot = warp_sum_u128(tot);
     abv = warp_sum_u128(abv);
 #pragma unroll
@@ -232,8 +251,13 @@ int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double
     return 1;
 }
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st) {
+    static int per_sm = 0;   // one wave of resident blocks: a grid-stride loop has no tail
+    if (!per_sm) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_classify_kernel, SV_THREADS, 0);
+        if (per_sm < 1) per_sm = 1;
+    }
     u64 blocks = (n + SV_THREADS * SC_IT - 1) / (SV_THREADS * SC_IT);
-    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
     if (blocks < 1) blocks = 1;
     ss_classify_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps);
     return 1;
