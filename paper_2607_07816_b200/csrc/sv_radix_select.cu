@@ -330,36 +330,64 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
         hist[i] = ((i >= H_AND && i < H_OR) || i == H_EXT + 1) ? ~0ull : 0ull;
     }
     __syncthreads();
-    if (threadIdx.x != 0) return;
     SelState s = *ssp;
     const u64* cnt = h + H_CNT;
     const u64* shi = h + H_SHI;
     const u64* slo = h + H_SLO;
     const u64* band = h + H_AND;
     const u64* bor = h + H_OR;
+    // per-bin masses and per-segment (8 bins per thread) sums, in parallel; the cut is then found by
+    // one thread that skips whole segments and walks only the segment(s) a cut can fall in
+    double* mh = reinterpret_cast<double*>(h + H_TOTAL);
+    double* ml = mh + RS_BINS;
+    double* sgh = ml + RS_BINS;
+    double* sgl = sgh + SV_THREADS;
+    u64* sgc = reinterpret_cast<u64*>(sgl + SV_THREADS);
+    constexpr int SEG = RS_BINS / SV_THREADS;
+    const bool l0 = s.phase == 0;
+#define BIN_E(d) (l0 ? ((((d) & 0x7ff) != 0) ? ((d) & 0x7ff) : 1) : s.E)
+    if (s.phase <= 1) {
+        dd sm = dd_make(0.0); u64 sc = 0;
+        for (int d = threadIdx.x * SEG + SEG - 1; d >= (int)threadIdx.x * SEG; --d) {
+            dd m = dd_make(0.0);
+            if (cnt[d]) { m = bin_mass(shi[d], slo[d], BIN_E(d)); sm = dd_add(sm, m); sc += cnt[d]; }
+            mh[d] = m.hi; ml[d] = m.lo;
+        }
+        sgh[threadIdx.x] = sm.hi; sgl[threadIdx.x] = sm.lo; sgc[threadIdx.x] = sc;
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
     dd kept; kept.hi = s.kept_hi; kept.lo = s.kept_lo;
     dd rem; rem.hi = s.mass_rem_hi; rem.lo = s.mass_rem_lo;
     if (s.phase <= 1) {
-        const bool l0 = s.phase == 0;
-#define BIN_E(d) (l0 ? ((((d) & 0x7ff) != 0) ? ((d) & 0x7ff) : 1) : s.E)
         if (l0 && !s.seeded) {   // total mass S and the p-mass threshold min_mass * S (reading R5)
             dd tot = dd_make(0.0);
-            for (int d = 0; d < RS_BINS; ++d)
-                if (cnt[d]) tot = dd_add(tot, bin_mass(shi[d], slo[d], BIN_E(d)));
+            for (int t = 0; t < SV_THREADS; ++t)
+                if (sgc[t]) { dd x; x.hi = sgh[t]; x.lo = sgl[t]; tot = dd_add(tot, x); }
             s.total_hi = tot.hi; s.total_lo = tot.lo;
             rem = dd_make(__dmul_rn(s.min_mass, tot.hi));
         }
         u64 cumc = 0; dd cum = dd_make(0.0);
         int dK = -1, dM = -1, dlow = -1;
         u64 aboveC_K = 0, aboveC_M = 0; dd aboveM_K = dd_make(0.0), aboveM_M = dd_make(0.0);
-        for (int d = RS_BINS - 1; d >= 0; --d) {
-            const u64 c = cnt[d];
-            if (!c) continue;
-            dlow = d;
-            const dd m = bin_mass(shi[d], slo[d], BIN_E(d));
-            if (s.count_active && dK < 0 && cumc + c >= s.k_rem) { dK = d; aboveC_K = cumc; aboveM_K = cum; }
-            if (s.mass_active && dM < 0 && dd_ge(dd_add(cum, m), rem)) { dM = d; aboveC_M = cumc; aboveM_M = cum; }
-            cumc += c; cum = dd_add(cum, m);
+        int lowest_seg = -1;
+        for (int t = 0; t < SV_THREADS && lowest_seg < 0; ++t) if (sgc[t]) lowest_seg = t;
+        for (int t = SV_THREADS - 1; t >= 0; --t) {
+            if (!sgc[t]) continue;
+            dd sgm; sgm.hi = sgh[t]; sgm.lo = sgl[t];
+            bool walk = (t == lowest_seg);                         // the lowest non-empty segment holds dlow
+            if (s.count_active && dK < 0 && cumc + sgc[t] >= s.k_rem) walk = true;
+            if (s.mass_active && dM < 0 && dd_add(cum, sgm).hi >= rem.hi - fabs(rem.hi) * 1e-12) walk = true;
+            if (!walk) { cumc += sgc[t]; cum = dd_add(cum, sgm); continue; }
+            for (int d = t * SEG + SEG - 1; d >= t * SEG; --d) {
+                const u64 c = cnt[d];
+                if (!c) continue;
+                dlow = d;
+                dd m; m.hi = mh[d]; m.lo = ml[d];
+                if (s.count_active && dK < 0 && cumc + c >= s.k_rem) { dK = d; aboveC_K = cumc; aboveM_K = cum; }
+                if (s.mass_active && dM < 0 && dd_ge(dd_add(cum, m), rem)) { dM = d; aboveC_M = cumc; aboveM_M = cum; }
+                cumc += c; cum = dd_add(cum, m);
+            }
         }
         if (dlow < 0) { s.done = s.seeded ? 3 : 1; s.PT = 0; s.KT = ~0ull; }   // no candidates at all
         else if (s.seeded && s.below_cnt > 0 && (!s.mass_active || dM < 0) && (!s.count_active || dK < 0)) {
@@ -470,7 +498,7 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
     *ssp = s;
 }
 int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st) {
-    const size_t smem = (size_t)H_TOTAL * 8;
+    const size_t smem = (size_t)H_TOTAL * 8 + (size_t)RS_BINS * 16 + (size_t)SV_THREADS * 24;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(sel_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     sel_step_kernel<<<1, SV_THREADS, smem, st>>>(ss, hist);

@@ -63,6 +63,7 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
     const u32 per = (Ml + 31) / 32;
     const u32 b0 = min(Ml, warp * per), b1 = min(Ml, b0 + per);
     double s = 0.0;
+#pragma unroll 8
     for (u32 i = b0 + lane; i < b1; i += 32) s += smp_prob(live[i] - 1);
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
@@ -82,18 +83,26 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
     for (int sweep = 0; sweep < 2 && mass_on; ++sweep) {
         u32 c[3] = {0, 0, 0};
         double run = pre;
-        for (u32 i0 = b0; i0 < b1; i0 += 32) {
-            const u32 i = i0 + lane;
-            const double v = (i < b1) ? smp_prob(live[i] - 1) : 0.0;
-            double inc = v;
+        for (u32 ib = b0; ib < b1; ib += 32 * 8) {   // 8 rows of 32 per batch: the loads of a batch are in flight together
+            double vv[8];
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-            const double incl = run + inc;   // mass of the sample's i + 1 smallest live elements
-            if (i < b1) {
-#pragma unroll
-                for (int k = 0; k < 3; ++k) c[k] += (incl <= X[k]) ? 1u : 0u;
+            for (int u = 0; u < 8; ++u) {
+                const u32 i = ib + u * 32 + lane;
+                vv[u] = (i < b1) ? smp_prob(live[i] - 1) : 0.0;
             }
-            run += __shfl_sync(0xffffffffu, inc, 31);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const u32 i = ib + u * 32 + lane;
+                double inc = vv[u];
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                const double incl = run + inc;   // mass of the sample's i + 1 smallest live elements
+                if (i < b1) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) c[k] += (incl <= X[k]) ? 1u : 0u;
+                }
+                run += __shfl_sync(0xffffffffu, inc, 31);
+            }
         }
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
