@@ -491,16 +491,15 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 0,
                                          s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
     } else {
-        if (s->defer.active) { int rcm = materialize(s); if (rcm != SV_OK) return rcm; }
-        const int alt2 = s->cur ^ 1;
-        s->stats.launches += svk_group(s->keys[s->cur], s->amps[s->cur], s->keys[alt2], s->amps[alt2], s->phys, plast, ma,
-                                       s->tab, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
+        s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
+                                           s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1);
     }
     CHECK_LAUNCH();
     s->stats.passes += 1;
-    u64 nout = 0;
-    int rc = read_back(s, &nout, s->d_count, sizeof(u64));
+    u64 cnts[2] = {0, 0};   // stored outputs, dead ones among them (exact cancellations of a multi-bit gate)
+    int rc = read_back(s, cnts, s->d_count, ma == 1 ? sizeof(u64) : 2 * sizeof(u64));
     if (rc != SV_OK) return rc;
+    const u64 nout = cnts[0], ndead = (ma == 1) ? 0 : cnts[1];
     if (ge0) s->pend[gslot].bytes = 24.0 * ((double)n_live_in + (double)(nout > s->cap ? s->cap : nout));
     if (nout > s->cap) {
         s->stats.n_out = nout;
@@ -508,9 +507,9 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     }
     if (plast > 0) { memcpy(s->phys_of_log, after.phys_of_log, sizeof(s->phys_of_log)); s->xmask = after.xmask; s->lut_valid = false; }
     s->cur ^= 1;
-    s->count = nout; s->phys = nout;
+    s->count = nout - ndead; s->phys = nout;
     s->defer.active = 0;
-    s->stats.n_out = nout;
+    s->stats.n_out = s->count;
     return SV_OK;
 }
 

@@ -1,0 +1,314 @@
+// Final pass of a gate with MA >= 2 active bits (SURVEY.md rows a-4 .. a-7).
+//
+// Same tile pipeline as the single-bit pass (sv_pair.cu): persistent blocks, the next tile landing
+// through cp.async while the current one is processed, A* | B* partition, one merge-path split per
+// thread.  Phase 1 moves the last missing active bit to the LSB (skipped when the active bits
+// already sit at physical positions 0 .. MA-1) and leaves the tile in shared memory in its NEW
+// order, where the <= 2^MA terms of a tuple are neighbours.  Phase 2:
+//   * every term that opens a tuple collects the tuple's presence mask and, from the zero pattern
+//     of U, the set of output rows that can be nonzero: the tile's output count is known before
+//     any arithmetic, so one scan + look-back fixes every output position;
+//   * the outputs are then computed ONE PER THREAD (thread t takes outputs t, t + 256, ...: it finds
+//     the tuple by a search over the per-term output offsets; column contributions are added in
+//     ascending logical column index, every operation rounded separately: DESIGN.md D1) and stored
+//     directly, consecutive threads writing consecutive entries.  A row that cancels to exactly 0+0i is written as a dead entry
+//     (counted, so the term count stays exact) instead of forcing a second scan.
+#include "sv_tile.cuh"
+
+template <int MA>
+__global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+                                                                  u64* __restrict__ kout, double2* __restrict__ aout, int p,
+                                                                  const GateTab* __restrict__ gtab, PendPred pd,
+                                                                  const TileDesc* __restrict__ desc, u64* status,
+                                                                  u64* d_count, u64 cap, u32 ntiles) {
+    constexpr int NP = 1 << MA;
+    constexpr u64 AM = (u64)NP - 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
+    double2* sa = La + BP_TILE;                                // work buffer: partitioned tile, then the tile in its new order
+    u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
+    u64* sk = Lk + BP_TILE;
+    u64* s_info = sk + BP_TILE;                                // per term: the tuple it opens (rows, masks, control block)
+    int* s_offs = reinterpret_cast<int*>(s_info + BP_TILE);    // per term: outputs of the tile before it
+    __shared__ int red[BP_WARPS + 2];
+    __shared__ int wc[BP_VT][BP_WARPS];
+    __shared__ int s_nA;
+    __shared__ u64 s_desc[2][8];
+    __shared__ u64 s_base;
+    __shared__ double2 sU[256];
+    __shared__ unsigned short s_nzr[16][16];   // [cx][xc]: rows r with U[r][xc] != 0 in control block cx
+    __shared__ int s_cpos[SV_MAX_M], s_col[16], s_mc;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool mv = p >= 0;
+
+    for (int i = tid; i < 256; i += SV_THREADS) sU[i] = gtab->U[i];
+    if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
+    if (tid < 16) s_col[tid] = gtab->colorder[tid];
+    if (tid == 0) s_mc = gtab->mc;
+    __syncthreads();
+    {
+        const int cx = tid >> 4, xc = tid & 15;
+        unsigned short m = 0;
+        if (cx < (1 << s_mc) && xc < NP)
+            for (int r = 0; r < NP; ++r) {
+                const double2 u = sU[(((cx << MA) | r) << MA) | xc];
+                if (!(u.x == 0.0 && u.y == 0.0)) m |= (unsigned short)(1u << r);
+            }
+        s_nzr[cx][xc] = m;
+    }
+    const u64 bit = mv ? (1ull << p) : 0ull;
+    const u64 himask = (!mv || p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
+    u64* gstat = status + ntiles;
+    u32 n_dead = 0;
+
+    auto issue_loads = [&](const Pieces3& q) {
+#pragma unroll
+        for (int r = 0; r < BP_VT; ++r) {
+            const int e = tid + r * SV_THREADS;
+            if (e < q.cnt) {
+                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
+                cp_async8(Lk + e, kin + g);
+                cp_async16(La + e, ain + g);
+            }
+        }
+        cp_async_commit();
+    };
+    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+    __syncthreads();
+    issue_loads(pieces_of(s_desc[0]));
+    int par = 0;
+    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+        const u32 next = tile + gridDim.x;
+        u64 dnext = 0;
+        if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
+        const Pieces3 pc = pieces_of(s_desc[par]);
+        const int cnt = pc.cnt;
+        int nA;
+        {   // pick up this thread's landed elements, apply a pending truncation, partition into A* | B*
+            cp_async_wait_all();
+            u64 lk[BP_VT]; double2 la[BP_VT];
+#pragma unroll
+            for (int r = 0; r < BP_VT; ++r) {
+                const int e = tid + r * SV_THREADS;
+                lk[r] = 0; la[r] = make_double2(0.0, 0.0);
+                if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
+            }
+            if (pd.active) {
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    if (tid + r * SV_THREADS < cnt) {
+                        if (pend_keep(pd, lk[r], la[r])) { la[r].x = __dmul_rn(la[r].x, pd.scale); la[r].y = __dmul_rn(la[r].y, pd.scale); }
+                        else { la[r].x = 0.0; la[r].y = 0.0; }
+                    }
+                }
+            }
+            if (!mv || pc.oneblock) {   // load order = A* | B* already (no move: everything is "A", keys unchanged)
+                nA = mv ? pc.l0 : cnt;
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const int e = tid + r * SV_THREADS;
+                    if (e < cnt) { sk[e] = lk[r] & ~bit; sa[e] = la[r]; }
+                }
+            } else {
+                u32 balA[BP_VT];
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const bool isA = (tid + r * SV_THREADS < cnt) && !(lk[r] & bit);
+                    balA[r] = __ballot_sync(0xffffffffu, isA);
+                    if (lane == 0) wc[r][warp] = __popc(balA[r]);
+                }
+                __syncthreads();
+                if (warp == 0) {
+                    const int c = wc[lane >> 3][lane & 7];
+                    int inc = c;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                    wc[lane >> 3][lane & 7] = inc - c;
+                    if (lane == 31) s_nA = inc;
+                }
+                __syncthreads();
+                nA = s_nA;
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const int e = tid + r * SV_THREADS;
+                    if (e < cnt) {
+                        const int aBefore = wc[r][warp] + __popc(balA[r] & ((1u << lane) - 1u));
+                        const int slot = (lk[r] & bit) ? nA + (e - aBefore) : aBefore;
+                        sk[slot] = lk[r] & ~bit; sa[slot] = la[r];
+                    }
+                }
+            }
+        }
+        if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+        __syncthreads();
+        if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]));
+
+        // ---- phase 1: bring the tile into its new order (moved bit at the LSB) ----
+        if (mv) {
+            const int nB = cnt - nA;
+            const u64* skB = sk + nA;
+            const double2* saB = sa + nA;
+            const int diag = min(tid * BP_VT, cnt);
+            int i, j;
+            {
+                int lo = max(0, diag - nB), hi = min(diag, nA);
+                while (lo < hi) {   // A first on ties
+                    const int mid = (lo + hi) >> 1;
+                    if (sk[mid] <= skB[diag - 1 - mid]) lo = mid + 1; else hi = mid;
+                }
+                i = lo; j = diag - lo;
+            }
+            const int endpos = min(diag + BP_VT, cnt);
+            u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
+            u64 mk[BP_VT]; double2 ma_[BP_VT];
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v) {
+                mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
+                if (diag + v < endpos) {
+                    const bool takeA = ka <= kb;
+                    const u64 k = takeA ? ka : kb;
+                    ma_[v] = takeA ? sa[i] : saB[j];
+                    mk[v] = (k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull);
+                    if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
+                }
+            }
+            __syncthreads();   // every read of the partitioned tile is done
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (diag + v < endpos) { sk[diag + v] = mk[v]; sa[diag + v] = ma_[v]; }
+            __syncthreads();
+        }
+
+        // ---- phase 2a: tuples, presence masks, possible output rows -> output counts ----
+        const int e0 = min(tid * BP_VT, cnt);
+        const int mc = s_mc;
+        u64 t_info[BP_VT];   // rows | pm << 16 | pk << 32 | cx << 48 of the tuple a term opens (0: it opens none)
+        int mycount = 0;
+#pragma unroll
+        for (int v = 0; v < BP_VT; ++v) {
+            t_info[v] = 0;
+            const int e = e0 + v;
+            if (e < cnt) {
+                const u64 k = sk[e];
+                if (e == 0 || (sk[e - 1] >> MA) != (k >> MA)) {   // this term opens a tuple
+                    int cx = 0;
+                    for (int q = 0; q < mc; ++q) cx |= (int)((k >> s_cpos[q]) & 1ull) << q;
+                    u32 pk = 0, pm = 0, rows = 0;
+                    for (int w = 0; w < NP && e + w < cnt; ++w) {
+                        const u64 kw = sk[e + w];
+                        if ((kw >> MA) != (k >> MA)) break;
+                        const int x = (int)(kw & AM);
+                        pk |= 1u << x;
+                        const double2 a = sa[e + w];
+                        if (!(a.x == 0.0 && a.y == 0.0)) { pm |= 1u << x; rows |= s_nzr[cx][x]; }
+                    }
+                    t_info[v] = (u64)rows | ((u64)pm << 16) | ((u64)pk << 32) | ((u64)cx << 48);
+                    mycount += __popc(rows);
+                }
+            }
+        }
+        int total;
+        const int excl = block_excl_scan(mycount, red, &total);
+        {
+            int run = excl;
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (e0 + v < cnt) { s_offs[e0 + v] = run; s_info[e0 + v] = t_info[v]; run += __popc((u32)(t_info[v] & 0xffffu)); }
+        }
+        if (tid < 32) {
+            const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
+            if (tid == 0) {
+                s_base = ex;
+                if (tile == ntiles - 1) d_count[0] = ex + (u64)total;
+            }
+        }
+        __syncthreads();
+        // ---- phase 2b: one thread per OUTPUT: consecutive threads write consecutive entries ----
+        const u64 base = s_base;
+        for (int o = tid; o < total; o += SV_THREADS) {
+            int lo = o >> MA, hi = min(o, cnt - 1);        // the opening term L: last element with offs <= o
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) >> 1;
+                if (s_offs[mid] <= o) lo = mid; else hi = mid - 1;
+            }
+            const int e = lo;
+            const u64 info = s_info[e];
+            const u32 rows = (u32)(info & 0xffffu), pm = (u32)((info >> 16) & 0xffffu), pk = (u32)((info >> 32) & 0xffffu);
+            const int cx = (int)(info >> 48);
+            const int r = __fns(rows, 0, o - s_offs[e] + 1);   // the (o - offs + 1)-th possible row
+            const u64 k = sk[e];
+            const double2* urow = &sU[((cx << MA) | r) << MA];
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int t = 0; t < NP; ++t) {                 // ascending LOGICAL column index (D1)
+                const int x = s_col[t];
+                if ((pm >> x) & 1u) {
+                    const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+                    const double2 u = urow[x];
+                    cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+                }
+            }
+            if (sr == 0.0 && si == 0.0) ++n_dead;          // exact cancellation: a dead entry
+            const u64 g = base + (u64)o;
+            if (g < cap) { st_stream_u64(kout + g, (k & ~AM) | (u64)r); st_stream_d2(aout + g, make_double2(sr, si)); }
+        }
+        __syncthreads();   // the work buffer and the tuple tables are reused by the next tile
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) n_dead += __shfl_xor_sync(0xffffffffu, n_dead, d);
+    if (lane == 0 && n_dead) atomicAdd(&d_count[1], (u64)n_dead);
+}
+
+// Tile boundaries when no bit has to move (the active bits already sit at positions 0 .. ma-1): nominal
+// starts pulled back to the start of a tuple, encoded as one-block descriptors without a B run.
+__global__ void find_starts_kernel(const u64* __restrict__ keys, u64 n, int ma, u32 tnom, u32 ntiles, TileDesc* __restrict__ desc) {
+    const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > ntiles) return;
+    u64 t = (u64)j * tnom;
+    if (t >= n) t = n;
+    else if (t > 0) {
+        const u64 v = keys[t] >> ma;
+        while (t > 0 && (keys[t - 1] >> ma) == v) --t;
+    }
+    TileDesc d;
+    d.ia = t; d.ib = n; d.mid = n; d.e = n;
+    desc[j] = d;
+}
+
+template <int MA>
+static void launch_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
+                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
+    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 12;   // landing + work + tuple tables
+    static bool attr = false;
+    if (!attr) { cudaFuncSetAttribute(grouppass_kernel<MA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    static int per_sm = 0;
+    if (!per_sm) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grouppass_kernel<MA>, SV_THREADS, smem);
+        if (per_sm < 1) per_sm = 1;
+    }
+    const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
+    grouppass_kernel<MA><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles);
+}
+
+// Final pass of a gate with ma >= 2 active bits.  p < 0: no bit has to move.  Writes the number of
+// stored outputs to d_count[0] and the number of dead ones among them (exact cancellations) to d_count[1].
+int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
+                  const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
+                  u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
+    cudaMemsetAsync(d_count, 0, 2 * sizeof(u64), st);
+    if (n == 0) return 0;
+    const u32 tnom = (u32)(BP_TILE - (1 << ma));
+    const u32 ntiles = (u32)((n + tnom - 1) / tnom);
+    cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);
+    int launches = 1;
+    if (p >= 0) launches += svk_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
+    else { find_starts_kernel<<<(ntiles + 1 + 127) / 128, 128, 0, st>>>(kin, n, ma, tnom, ntiles, desc); launches += 1; }
+    if (e0) cudaEventRecord(e0, st);
+    switch (ma) {
+        case 2: launch_grouppass<2>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+        case 3: launch_grouppass<3>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+        default: launch_grouppass<4>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+    }
+    if (e1) cudaEventRecord(e1, st);
+    return launches;
+}

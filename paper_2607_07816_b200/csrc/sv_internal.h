@@ -98,6 +98,12 @@ int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 
               const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count,
               u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 
+// Final pass of a gate with ma >= 2 active bits (sv_group.cu).  p < 0: the active bits already sit at the
+// LSBs.  A pending truncation is applied while loading.  d_count[0] = stored outputs, d_count[1] = dead ones.
+int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
+                  const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
+                  u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
+
 // Lean single-bit pass (sv_pair.cu): moves physical bit p to the LSB in one streaming pass.
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
 // pair == 0: pure move.  A pending truncation is applied while loading.  Writes the output
