@@ -127,6 +127,14 @@ static int cuda_fail(sv_state* s, cudaError_t e, const char* where) {
         cudaError_t e__ = (call);                                          \
         if (e__ != cudaSuccess) return cuda_fail(s, e__, #call);           \
     } while (0)
+static bool dbg_sync_on() { static int v = -1; if (v < 0) v = getenv("SV_DEBUG_SYNC") ? 1 : 0; return v == 1; }
+#define DBG_SYNC(tag)                                                                            \
+    do {                                                                                         \
+        if (dbg_sync_on()) {                                                                     \
+            cudaError_t e__ = cudaStreamSynchronize(s->stream);                                  \
+            if (e__ != cudaSuccess) { fprintf(stderr, "[sv debug] %s: %s\n", tag, cudaGetErrorString(e__)); return cuda_fail(s, e__, tag); } \
+        }                                                                                        \
+    } while (0)
 #define CHECK_LAUNCH()                                                     \
     do {                                                                   \
         cudaError_t e__ = cudaGetLastError();                              \
@@ -533,7 +541,9 @@ static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 
         else if (phase == 2) s->stats.launches += svk_sel_extract(keys, amps, n, s->sel, km, lk, s->hist, s->stream);
         else s->stats.launches += svk_sel_pass(2, nullptr, lk, ties, s->sel, s->hist, s->stream);
         if (e1) cudaEventRecord(e1, s->stream);
+        DBG_SYNC(phase <= 1 ? "sel_pass" : (phase == 2 ? "sel_extract" : "sel_pass_keys"));
         s->stats.launches += svk_sel_step(s->sel, s->hist, s->stream);
+        DBG_SYNC("sel_step");
         CHECK_LAUNCH();
         s->stats.passes += 1;
         int rc = read_back(s, out, s->sel, sizeof(SelState));
@@ -558,15 +568,19 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     const u32 M = (u32)m64;
     cudaStream_t st = s->stream;
     s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st);
+    DBG_SYNC("ss_sample");
     int in_alt = 0;
     s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 32, s->smp_scr, st, &in_alt);
     s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st);
+    DBG_SYNC("ss_sort+pivot");
     cudaEvent_t e0, e1;
     prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
     if (e0) cudaEventRecord(e0, st);
     s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], st);
     if (e1) cudaEventRecord(e1, st);
+    DBG_SYNC("ss_classify");
     s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st);
+    DBG_SYNC("sel_seed");
     CHECK_LAUNCH();
     s->stats.passes += 1;
     int rc = read_back(s, out, s->sel, sizeof(SelState));
@@ -603,6 +617,7 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     int rc = SV_OK;
     if (s->defer.active) rc = materialize(s);   // a second truncation in a row: apply the first one now
     if (rc != SV_OK) return rc;
+    if (dbg_sync_on()) { DBG_SYNC("before select"); fprintf(stderr, "[sv debug] truncate: count=%llu phys=%llu cap=%llu cur=%d defer=%d\n", (unsigned long long)s->count, (unsigned long long)s->phys, (unsigned long long)s->cap, s->cur, s->defer.active); }
     SelState ss;
     rc = run_select(s, max_terms, min_mass, &ss);
     if (rc != SV_OK) return rc;

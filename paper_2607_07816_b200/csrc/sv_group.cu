@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
         // ---- phase 2b: one thread per OUTPUT: consecutive threads write consecutive entries ----
         const u64 base = s_base;
         for (int o = tid; o < total; o += SV_THREADS) {
-            int lo = o >> MA, hi = min(o, cnt - 1);        // the opening term L: last element with offs <= o
+            int lo = o >> MA, hi = cnt - 1;                // the opening term L: last element with offs <= o (L >= o / 2^MA)
             while (lo < hi) {
                 const int mid = (lo + hi + 1) >> 1;
                 if (s_offs[mid] <= o) lo = mid; else hi = mid - 1;

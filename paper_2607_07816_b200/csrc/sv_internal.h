@@ -8,8 +8,6 @@ typedef unsigned long long u64;
 typedef unsigned int u32;
 
 #define SV_MAX_M 4
-#define SV_TILE_SLOTS 2048      // outputs one group tile may produce (8 per thread at 256 threads)
-#define SV_MOVE_TILE 2048       // elements per tile of a pure bit-move pass
 #define SV_THREADS 256
 #define SV_SEL_BINS 4096        // 12-bit digits for the radix select
 
@@ -88,15 +86,6 @@ int sv_sm_count();   // SMs of the current device (cached)
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
-
-int svk_move(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p,
-             TileDesc* desc, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
-
-// Final pass of a group gate.  p < 0: the active bits already sit at the LSBs (no move).
-// Writes the output term count to *d_count (may exceed cap: then nothing past cap is written).
-int svk_group(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
-              const GateTab* tab, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count,
-              u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
 
 // Final pass of a gate with ma >= 2 active bits (sv_group.cu).  p < 0: the active bits already sit at the
 // LSBs.  A pending truncation is applied while loading.  d_count[0] = stored outputs, d_count[1] = dead ones.

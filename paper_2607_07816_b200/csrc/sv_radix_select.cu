@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(SV_THREADS) sel_pass_kernel(const double2* __r
             const u64 x = v[r];
             bool valid = ok[r];
             u32 bin;
-            if (MODE == 0) bin = (u32)(x >> 52);
+            if (MODE == 0) bin = (u32)(x >> 52) & (RS_BINS - 1);   // (p >= 0: the sign bit is clear)
             else { valid = valid && ((x & rmask) == rval); bin = valid ? pext_desc(x, dmask) : 0; }
             const u64 mant = x & ((1ull << 52) - 1);
             const u64 M = ((x >> 52) & 0x7ff) ? (mant | (1ull << 52)) : mant;

@@ -187,3 +187,31 @@ def test_config3_small_peak(eng):
     assert int(k[0]) == c.secret
     assert_same_state(sv.export()[:2], o.export()[:2], strict_keys=False)
     assert abs(sv.norm() - 1.0) <= 1e-12
+
+
+def test_pending_cut_and_dead_entries_twin(eng):
+    """The hot loop as the bench runs it: the truncation stays PENDING (and dead entries stay in place)
+    when the next gate arrives -- no export in between.  A twin engine fed the same calls is exported
+    before every gate to give the oracle the pre-gate state; the first engine's result must match."""
+    c = W.config5(num_gates=220, max_terms=1 << 13)
+    sv = eng.SparseSV(c.n, 1 << 17)
+    twin = eng.SparseSV(c.n, 1 << 17)
+    seen = set()
+    for g in c.gates:
+        k0, a0, _ = twin.export()            # (materialises the twin only)
+        o = _oracle(c.n)
+        o.load(k0, a0)
+        sv.apply_gate(g.qubits, g.U)
+        twin.apply_gate(g.qubits, g.U)
+        o.apply_gate(g.qubits, g.U)
+        assert sv.num_terms() == o.num_terms(), "term count after %s %r" % (g.name, g.qubits)
+        kg = sv.truncate(c.max_terms, c.min_mass)
+        kt = twin.truncate(c.max_terms, c.min_mass)
+        ko = o.truncate(c.max_terms, c.min_mass)
+        assert abs(kg - ko) <= MASS_TOL and abs(kt - ko) <= MASS_TOL
+        assert sv.num_terms() == twin.num_terms()
+        seen.add(g.klass)
+    assert {"diag", "perm", "gen1", "gen2", "gen3"} <= seen
+    assert_truncation_parity(sv.export()[:2], twin.export()[:2])
+    assert sv.check_invariants()
+    assert abs(sv.norm() - 1.0) <= 1e-12
