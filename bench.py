@@ -247,8 +247,19 @@ def run_ours(args):
     dom = max(prof, key=lambda k: prof[k]["ms"])
     dk = prof[dom]
     ach = dk["alg_bytes"] / (dk["ms"] * 1e-3) / 1e9 if dk["ms"] > 0 else 0.0
+    # dram__bytes_read + dram__bytes_write of one captured launch of that kernel at this workload
+    # (ncu --set full, see profiles/): traffic well above the algorithmic bytes would mean re-reads
+    traffic, traffic_note = None, None
+    tp = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    if os.path.exists(tp):
+        try:
+            t = json.load(open(tp)).get(dom)
+            if t:
+                traffic, traffic_note = t["dram_bytes_per_launch"], t.get("note")
+        except Exception:
+            pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm,
-                "traffic": None, "peak_kind": peak_kind, "launches": dk["launches"],
+                "traffic": traffic, "traffic_note": traffic_note, "peak_kind": peak_kind, "launches": dk["launches"],
                 "avg_launch_ms": dk["ms"] / max(dk["launches"], 1),
                 "alg_bytes_per_launch": dk["alg_bytes"] / max(dk["launches"], 1),
                 "kernels": {k: {"ms": v["ms"], "launches": v["launches"],

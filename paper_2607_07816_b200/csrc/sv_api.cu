@@ -481,7 +481,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         monomial = (!z00 && !z11 && z01 && z10) || (z00 && z11 && !z01 && !z10);
     }
     if (ma == 1 && monomial && few_dead(s)) {
-        prof_slot(s, SV_K_GROUP, 48.0 * (double)s->phys, &ge0, &ge1);
+        prof_slot(s, SV_K_BITPASS, 48.0 * (double)s->phys, &ge0, &ge1);
         s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 2, 1,
                                          s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
         CHECK_LAUNCH();
@@ -492,7 +492,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.n_out = s->count;
         return SV_OK;
     }
-    prof_slot(s, SV_K_GROUP, 0.0, &ge0, &ge1);
+    prof_slot(s, ma == 1 ? SV_K_BITPASS : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
     const int gslot = s->npend - 1;
     const u64 n_live_in = s->count;
     if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)
