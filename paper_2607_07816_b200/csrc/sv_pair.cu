@@ -8,54 +8,48 @@
 // stored order, are ascending in the key with bit p cleared, and so are the B terms: the
 // pass is ONE two-way merge of two sorted sequences A* and B* per tile.
 //
-//   load      the tile's (up to three) contiguous pieces; a truncation left pending by
-//             sv_truncate is applied here (dropped terms load as 0+0i, survivors are scaled);
-//             terms are placed in shared memory partitioned into A* | B*;
-//   split     every thread finds where its VT consecutive OUTPUT positions start in A* and
-//             B* (merge path: one binary search per thread, not per term);
-//   merge     VT sequential merge steps per thread.  Partners (the terms
-//             that differ only in the gate's qubit) meet as neighbours: the A member leads,
-//             the 2x2 mat-vec runs on the spot, exact zeros are dropped
-//             (PAPER.md:13);
-//   write     block scan + decoupled look-back give the output offsets; the outputs are
-//             staged in shared memory in output order and stored with coalesced writes:
-//             sorted, unique keys by construction.
-#include "sv_device.cuh"
-
+// The pass is bound by the shared-memory pipe, not by HBM (profiles/r1_b_pipeline.md), so the
+// data flow keeps shared-memory traffic low: ONLY KEYS are partitioned, searched and merged;
+// an amplitude lands once (cp.async, double buffered) and is read once, by index, where it is
+// needed.
+//
+//   land      the tile's (up to three) contiguous pieces arrive through cp.async one tile ahead;
+//   prepare   every thread files the keys it requested into A* | B* (bit p cleared) together with
+//             their landing slot;
+//   split     every thread finds where its VT consecutive OUTPUT positions start in A* and B*
+//             (merge path: one binary search per thread, not per term);
+//   merge     VT sequential merge steps per thread over keys.  Partners (the
+//             terms that differ only in the gate's qubit) meet as neighbours;
+//   write     MODE 0 / 2 (position preserving, see FIXED below): output keys and source slots are
+//             staged by output position; the copy-out gathers each amplitude from the landing
+//             buffer, applies a pending truncation (dropped -> dead entry 0+0i, survivors scaled)
+//             and the gate's phase, and stores coalesced.
+//             MODE 1 (general 2x2 blocks): the tuple mat-vec runs in the merge,
+//             exact zeros are dropped, block scan + two-level look-back give the
+//             offsets, outputs are staged and stored coalesced: sorted, unique keys by construction.
 #include "sv_tile.cuh"
 
-#ifdef BP_X_TIMING
-__device__ unsigned long long g_bp_t[16];
-extern "C" void sv_debug_timing(unsigned long long* out, int reset) {
-    if (reset) { unsigned long long z[16] = {0}; cudaMemcpyToSymbol(g_bp_t, z, sizeof(z)); return; }
-    cudaMemcpyFromSymbol(out, g_bp_t, sizeof(unsigned long long) * 16);
-}
-#define TSTAMP(k) do { if (tid == TWHO) { const long long t_ = clock64(); tacc[k] += t_ - tlast; tlast = t_; } } while (0)
-#else
-#define TSTAMP(k)
-#endif
-// FIXED: position-preserving variant for passes that map every stored entry to exactly one stored
-// entry (pure moves; gates whose 2x2 blocks are monomial, e.g. CNOT / Toffoli).  Terms dropped by a
-// pending truncation are carried as DEAD entries (amplitude 0+0i) instead of being squeezed out, so
-// the position of every output is known from the tile descriptor alone: no scan, no look-back.
 // MODE 0: pure move.  MODE 1: gate with one active bit (2x2 mat-vec per tuple).  MODE 2 (FIXED only):
 // the same for MONOMIAL 2x2 blocks: every entry maps to one entry (its bit kept or flipped, times a
 // phase), so the pass is a move whose partners may trade places -- no tuple arithmetic.
+// FIXED: position-preserving variant for passes that map every stored entry to exactly one stored
+// entry (pure moves, monomial blocks).  Terms dropped by a pending truncation are carried as DEAD
+// entries (amplitude 0+0i) instead of being squeezed out, so the position of every output is known
+// from the tile descriptor alone: no scan, no look-back.
 template <int MODE, bool FIXED>
 __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
-                                                                u32* tile_counter, u64* d_count, u64 cap, u32 ntiles) {
+                                                                u64* d_count, u64 cap, u32 ntiles) {
     constexpr bool PAIR = (MODE == 1);
     constexpr bool PERM = (MODE == 2);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer of the asynchronous loads (next tile)
-    double2* sta = La + BP_TILE;                               // work buffer: the partitioned tile, then the staged outputs
-    u64* Lk = reinterpret_cast<u64*>(sta + BP_TILE);
-    u64* stk = Lk + BP_TILE;
-    double2* sa = sta;
-    u64* sk = stk;
+    double2* La0 = reinterpret_cast<double2*>(smem_raw);       // landing amplitudes, double buffered
+    double2* La1 = La0 + BP_TILE;
+    u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);           // landing keys (consumed by prepare)
+    u64* Wk = Lk + BP_TILE;                                    // A* | B* keys with bit p cleared; later the staged output keys
+    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk + BP_TILE);   // their landing slots; later the staged source slots
     __shared__ int red[BP_WARPS + 2];
     __shared__ int wc[BP_VT][BP_WARPS];
     __shared__ int s_nA;
@@ -63,9 +57,9 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     __shared__ u64 s_base;
     __shared__ double2 sU[64];      // [cx][xr][xc], ma = 1: up to 8 control patterns x 4
     __shared__ int s_cpos[SV_MAX_M], s_mc;
+    __shared__ int s_sw[8], s_unit; // PERM: block cx swaps the bit; every nonzero entry is exactly 1
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    __shared__ int s_sw[8], s_unit;   // PERM: block cx swaps the bit; every nonzero entry is exactly 1
     if (PAIR || PERM) {
         if (tid < 64) sU[tid] = gtab->U[tid];
         if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
@@ -85,13 +79,12 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     const u64 bit = 1ull << p;
     const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
     u64* gstat = status + ntiles;                       // group statuses follow the tile statuses
-    // Persistent blocks (the grid is sized to be fully resident): tile t is taken by block
-    // t mod gridDim.x, so a block only ever waits on tiles that resident blocks have taken already.
-    // Software pipeline: while a tile is merged, scanned and written, the block's NEXT tile is
-    // already on its way from HBM into the landing buffer (cp.async, one thread per element), so
-    // every block keeps a full tile of loads in flight all the time.  Each thread later picks up
-    // exactly the elements it requested.  Tile descriptors travel one iteration ahead (s_desc).
-    auto issue_loads = [&](const Pieces3& q) {
+    // Persistent blocks (the grid is sized to be fully resident): tile t is taken by block t mod gridDim.x,
+    // so a block only ever waits on tiles that resident blocks have taken already.  While a tile is
+    // merged and written, the block's NEXT tile is already on its way from HBM (cp.async, one thread per
+    // element): every block keeps a full tile of loads in flight.  Each thread later files exactly the
+    // keys it requested.  Tile descriptors travel one iteration ahead (s_desc).
+    auto issue_loads = [&](const Pieces3& q, double2* La) {
 #pragma unroll
         for (int r = 0; r < BP_VT; ++r) {
             const int e = tid + r * SV_THREADS;
@@ -105,241 +98,259 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     };
     if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
     __syncthreads();
-    issue_loads(pieces_of(s_desc[0]));
-#ifdef BP_X_TIMING
-    long long tacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
-#endif
+    issue_loads(pieces_of(s_desc[0]), La0);
     int par = 0;
     for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
-    const u32 next = tile + gridDim.x;
-    u64 dnext = 0;
-    if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
-    const Pieces3 pc = pieces_of(s_desc[par]);
-    const int cnt = pc.cnt;
-    int nA;
-    {
-        TSTAMP(0);
-        cp_async_wait_all();      // this thread's own elements have landed
-        TSTAMP(1);
-        u64 lk[BP_VT]; double2 la[BP_VT];
-#pragma unroll
-        for (int r = 0; r < BP_VT; ++r) {
-            const int e = tid + r * SV_THREADS;
-            lk[r] = 0; la[r] = make_double2(0.0, 0.0);
-            if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
-        }
-        if (pd.active) {          // pending truncation: dropped terms become 0+0i, survivors are scaled
-#pragma unroll
-            for (int r = 0; r < BP_VT; ++r) {
-                if (tid + r * SV_THREADS < cnt) {
-                    if (pend_keep(pd, lk[r], la[r])) { la[r].x = __dmul_rn(la[r].x, pd.scale); la[r].y = __dmul_rn(la[r].y, pd.scale); }
-                    else { la[r].x = 0.0; la[r].y = 0.0; }
-                }
-            }
-        }
-        if (pc.oneblock) {   // piece 0 is all A, piece 1 all B: the load order is already A* | B*
-            nA = pc.l0;
+        double2* La = par ? La1 : La0;          // this tile's amplitudes (by landing slot)
+        double2* Lnext = par ? La0 : La1;
+        const u32 next = tile + gridDim.x;
+        u64 dnext = 0;
+        if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
+        const Pieces3 pc = pieces_of(s_desc[par]);
+        const int cnt = pc.cnt;
+        int nA;
+        {   // ---- prepare: keys only ----
+            cp_async_wait_all();      // this thread's own elements have landed
+            u64 lk[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
-                if (e < cnt) { sk[e] = lk[r] & ~bit; sa[e] = la[r]; }
+                lk[r] = (e < cnt) ? Lk[e] : 0;
             }
-        } else {          // stable partition by bit p (the load order is the stored order)
-            u32 balA[BP_VT];
+            if (pc.oneblock) {   // piece 0 is all A, piece 1 all B: the load order is already A* | B*
+                nA = pc.l0;
 #pragma unroll
-            for (int r = 0; r < BP_VT; ++r) {
-                const bool isA = (tid + r * SV_THREADS < cnt) && !(lk[r] & bit);
-                balA[r] = __ballot_sync(0xffffffffu, isA);
-                if (lane == 0) wc[r][warp] = __popc(balA[r]);
-            }
-            __syncthreads();
-            if (warp == 0) {   // lane = r * 8 + warp: exclusive scan of the 32 counts in load order
-                const int c = wc[lane >> 3][lane & 7];
-                int inc = c;
+                for (int r = 0; r < BP_VT; ++r) {
+                    const int e = tid + r * SV_THREADS;
+                    if (e < cnt) { Wk[e] = lk[r] & ~bit; Wi[e] = (unsigned short)e; }
+                }
+            } else {             // stable partition by bit p (the load order is the stored order)
+                u32 balA[BP_VT];
 #pragma unroll
-                for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
-                wc[lane >> 3][lane & 7] = inc - c;
-                if (lane == 31) s_nA = inc;
-            }
-            __syncthreads();
-            nA = s_nA;
+                for (int r = 0; r < BP_VT; ++r) {
+                    const bool isA = (tid + r * SV_THREADS < cnt) && !(lk[r] & bit);
+                    balA[r] = __ballot_sync(0xffffffffu, isA);
+                    if (lane == 0) wc[r][warp] = __popc(balA[r]);
+                }
+                __syncthreads();
+                if (warp == 0) {   // lane = r * 8 + warp: exclusive scan of the 32 counts in load order
+                    const int c = wc[lane >> 3][lane & 7];
+                    int inc = c;
 #pragma unroll
-            for (int r = 0; r < BP_VT; ++r) {
-                const int e = tid + r * SV_THREADS;
-                if (e < cnt) {
-                    const int aBefore = wc[r][warp] + __popc(balA[r] & ((1u << lane) - 1u));
-                    const int slot = (lk[r] & bit) ? nA + (e - aBefore) : aBefore;
-                    sk[slot] = lk[r] & ~bit; sa[slot] = la[r];
+                    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                    wc[lane >> 3][lane & 7] = inc - c;
+                    if (lane == 31) s_nA = inc;
+                }
+                __syncthreads();
+                nA = s_nA;
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const int e = tid + r * SV_THREADS;
+                    if (e < cnt) {
+                        const int aBefore = wc[r][warp] + __popc(balA[r] & ((1u << lane) - 1u));
+                        const int slot = (lk[r] & bit) ? nA + (e - aBefore) : aBefore;
+                        Wk[slot] = lk[r] & ~bit; Wi[slot] = (unsigned short)e;
+                    }
                 }
             }
         }
-    }
-    if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
-    TSTAMP(2);
-    __syncthreads();       // the work buffer is complete; every thread has emptied its landing slots
-    TSTAMP(3);
-    if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]));
-    TSTAMP(4);
-    const int nB = cnt - nA;
-    const u64* skB = sk + nA;
-    const double2* saB = sa + nA;
+        if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+        __syncthreads();       // A* | B* complete, every landed amplitude visible, landing keys consumed
+        if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]), Lnext);
+        const int nB = cnt - nA;
+        const u64* WkB = Wk + nA;
+        const unsigned short* WiB = Wi + nA;
 
-    // merge-path split of this thread's first output position
-    const int diag = min(tid * BP_VT, cnt);
-    int i, j;
-    {
-        int lo = max(0, diag - nB), hi = min(diag, nA);
-        while (lo < hi) {   // A first on ties
-            const int mid = (lo + hi) >> 1;
-            if (sk[mid] <= skB[diag - 1 - mid]) lo = mid + 1; else hi = mid;
+        // ---- merge-path split of this thread's first output position ----
+        const int diag = min(tid * BP_VT, cnt);
+        int i, j;
+        {
+            int lo = max(0, diag - nB), hi = min(diag, nA);
+            while (lo < hi) {   // A first on ties
+                const int mid = (lo + hi) >> 1;
+                if (Wk[mid] <= WkB[diag - 1 - mid]) lo = mid + 1; else hi = mid;
+            }
+            i = lo; j = diag - lo;
         }
-        i = lo; j = diag - lo;
-    }
-    TSTAMP(5);
-    const int endpos = min(diag + BP_VT, cnt);
-    int pos = diag;
-    // keys with bit p cleared never equal ~0: safe sentinels for an exhausted side
-    u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
-    u64 ok[BP_VT];
-    double o0r[BP_VT], o0i[BP_VT], o1r[BP_VT], o1i[BP_VT];
-    u32 fl = 0;     // two flag bits per step
-    int nout = 0;
-    if (PAIR && pos < endpos && j < nB && i > 0 && sk[i - 1] == kb) {   // this B belongs to the previous thread's tuple
-        ++j; ++pos;
-        kb = (j < nB) ? skB[j] : ~0ull;
-    }
-    const int startpos = pos;
-    u64 lastA = (PERM && i > 0) ? sk[i - 1] : ~0ull;   // PERM: a B term's partner is the A term merged just before it
-    int opos[BP_VT];
+        const int endpos = min(diag + BP_VT, cnt);
+        int pos = diag;
+        // keys with bit p cleared never equal ~0: safe sentinels for an exhausted side
+        u64 ka = (i < nA) ? Wk[i] : ~0ull, kb = (j < nB) ? WkB[j] : ~0ull;
+        if (FIXED) {
+            // ---- keys only: output key, source slot and output position of VT merged terms ----
+            u64 okey[BP_VT]; int osrc[BP_VT], opos[BP_VT];
+            u64 lastA = (PERM && i > 0) ? Wk[i - 1] : ~0ull;   // PERM: a B term's partner is the A term merged just before it
 #pragma unroll
-    for (int v = 0; v < BP_VT; ++v) {
-        ok[v] = 0; o0r[v] = o0i[v] = o1r[v] = o1i[v] = 0.0; opos[v] = -1;
-        if (pos < endpos) {
-            const bool takeA = ka <= kb;
-            const u64 k = takeA ? ka : kb;
-            const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
-            if (PERM) {
-                const int c = takeA ? 0 : 1;
-                const bool partner = takeA ? (kb == k) : (lastA == k);
-                double2 a = takeA ? sa[i] : saB[j];
-                if (takeA) { ++i; lastA = k; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
-                int cx = 0;
-                const int mc = s_mc;
-                for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
-                const int sw = s_sw[cx], row = c ^ sw;
-                if (!s_unit) {
+            for (int v = 0; v < BP_VT; ++v) {
+                okey[v] = 0; osrc[v] = 0; opos[v] = -1;
+                if (pos < endpos) {
+                    const bool takeA = ka <= kb;
+                    const u64 k = takeA ? ka : kb;
+                    const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
+                    osrc[v] = takeA ? Wi[i] : WiB[j];
+                    int row = takeA ? 0 : 1, shift = 0;
+                    if (PERM) {
+                        const bool partner = takeA ? (kb == k) : (lastA == k);
+                        int cx = 0;
+                        const int mc = s_mc;
+                        for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
+                        const int sw = s_sw[cx];
+                        if (partner && sw) shift = row ? -1 : 1;           // partners that swap rows trade places
+                        row ^= sw;
+                    }
+                    okey[v] = nk | (u64)row;
+                    opos[v] = pos + shift;
+                    if (takeA) { ++i; lastA = k; ka = (i < nA) ? Wk[i] : ~0ull; } else { ++j; kb = (j < nB) ? WkB[j] : ~0ull; }
+                    ++pos;
+                }
+            }
+            __syncthreads();   // every read of A* | B* is done: stage by output position in the same arrays
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (opos[v] >= 0) { Wk[opos[v]] = okey[v]; Wi[opos[v]] = (unsigned short)osrc[v]; }
+            __syncthreads();
+            // ---- copy-out: gather the amplitude, apply a pending truncation and the phase, store coalesced ----
+            const u64 base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
+            const int mc = PERM ? s_mc : 0;
+            const bool phase = PERM && !s_unit;
+            for (int idx = tid; idx < cnt; idx += SV_THREADS) {
+                const u64 key = Wk[idx];
+                double2 a = La[Wi[idx]];
+                const int row = (int)(key & 1ull);
+                int cx = 0, c = row;
+                if (PERM) {
+                    for (int q = 0; q < mc; ++q) cx |= (int)((key >> s_cpos[q]) & 1ull) << q;
+                    c = row ^ s_sw[cx];
+                }
+                if (pd.active) {
+                    const u64 old = (key & himask) | ((key >> 1) & lowmask) | (c ? bit : 0ull);   // the stored key it came from
+                    if (pend_keep(pd, old, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
+                    else { a.x = 0.0; a.y = 0.0; }
+                }
+                if (phase) {
                     const double2 u = sU[(cx << 2) | (row << 1) | c];
                     const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
                     const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
                     a.x = __dadd_rn(0.0, pr); a.y = __dadd_rn(0.0, pi);
                 }
-                ok[v] = nk | (u64)row; o0r[v] = a.x; o0i[v] = a.y;
-                opos[v] = pos + ((partner && sw) ? (c ? -1 : 1) : 0);   // partners that swap rows trade places
-                ++pos;
-            } else if (PAIR) {
-                double2 a, pa = make_double2(0.0, 0.0);
-                bool has_partner = false;
-                if (takeA) {
-                    a = sa[i]; ++i; ++pos;
-                    has_partner = (kb == k);
-                    if (has_partner) { pa = saB[j]; ++j; ++pos; kb = (j < nB) ? skB[j] : ~0ull; }
-                    ka = (i < nA) ? sk[i] : ~0ull;
-                } else {
-                    a = saB[j]; ++j; ++pos;
-                    kb = (j < nB) ? skB[j] : ~0ull;
-                }
-                int cx = 0;
-                const int mc = s_mc;
-                for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
-                const double2* u = &sU[cx << 2];                    // u[xr * 2 + xc]
-                double r0 = 0.0, m0 = 0.0, r1 = 0.0, m1 = 0.0;
-                if (takeA) {
-                    cmul_acc(r0, m0, u[0].x, u[0].y, a.x, a.y);
-                    cmul_acc(r1, m1, u[2].x, u[2].y, a.x, a.y);
-                    if (has_partner) {
-                        cmul_acc(r0, m0, u[1].x, u[1].y, pa.x, pa.y);
-                        cmul_acc(r1, m1, u[3].x, u[3].y, pa.x, pa.y);
+                const u64 g = base + (u64)idx;
+                if (g < cap) { st_stream_u64(kout + g, key); st_stream_d2(aout + g, a); }
+            }
+            __syncthreads();   // A* | B* and this landing buffer are reused
+            continue;
+        }
+
+        // ---- compacting variants: amplitudes are read (by landing slot) in the merge ----
+        auto amp_at = [&](int slot, u64 stored_key) {
+            double2 a = La[slot];
+            if (pd.active) {
+                if (pend_keep(pd, stored_key, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
+                else { a.x = 0.0; a.y = 0.0; }
+            }
+            return a;
+        };
+        u64 ok[BP_VT];
+        double o0r[BP_VT], o0i[BP_VT], o1r[BP_VT], o1i[BP_VT];
+        u32 fl = 0;     // two flag bits per step
+        int nout = 0;
+        if (PAIR && pos < endpos && j < nB && i > 0 && Wk[i - 1] == kb) {   // this B belongs to the previous thread's tuple
+            ++j; ++pos;
+            kb = (j < nB) ? WkB[j] : ~0ull;
+        }
+#pragma unroll
+        for (int v = 0; v < BP_VT; ++v) {
+            ok[v] = 0; o0r[v] = o0i[v] = o1r[v] = o1i[v] = 0.0;
+            if (pos < endpos) {
+                const bool takeA = ka <= kb;
+                const u64 k = takeA ? ka : kb;
+                const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
+                if (PAIR) {
+                    double2 a, pa = make_double2(0.0, 0.0);
+                    bool has_partner = false;
+                    if (takeA) {
+                        a = amp_at(Wi[i], k); ++i; ++pos;
+                        has_partner = (kb == k);
+                        if (has_partner) { pa = amp_at(WiB[j], k | bit); ++j; ++pos; kb = (j < nB) ? WkB[j] : ~0ull; }
+                        ka = (i < nA) ? Wk[i] : ~0ull;
+                    } else {
+                        a = amp_at(WiB[j], k | bit); ++j; ++pos;
+                        kb = (j < nB) ? WkB[j] : ~0ull;
                     }
-                } else {
-                    cmul_acc(r0, m0, u[1].x, u[1].y, a.x, a.y);
-                    cmul_acc(r1, m1, u[3].x, u[3].y, a.x, a.y);
+                    int cx = 0;
+                    const int mc = s_mc;
+                    for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
+                    const double2* u = &sU[cx << 2];                    // u[xr * 2 + xc]
+                    double r0 = 0.0, m0 = 0.0, r1 = 0.0, m1 = 0.0;
+                    if (takeA) {
+                        cmul_acc(r0, m0, u[0].x, u[0].y, a.x, a.y);
+                        cmul_acc(r1, m1, u[2].x, u[2].y, a.x, a.y);
+                        if (has_partner) {
+                            cmul_acc(r0, m0, u[1].x, u[1].y, pa.x, pa.y);
+                            cmul_acc(r1, m1, u[3].x, u[3].y, pa.x, pa.y);
+                        }
+                    } else {
+                        cmul_acc(r0, m0, u[1].x, u[1].y, a.x, a.y);
+                        cmul_acc(r1, m1, u[3].x, u[3].y, a.x, a.y);
+                    }
+                    const u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
+                    ok[v] = nk; o0r[v] = r0; o0i[v] = m0; o1r[v] = r1; o1i[v] = m1;
+                    fl |= (f0 | (f1 << 1)) << (2 * v);
+                    nout += (int)(f0 + f1);
+                } else {   // compacting move
+                    const double2 a = takeA ? amp_at(Wi[i], k) : amp_at(WiB[j], k | bit);
+                    if (takeA) { ++i; ka = (i < nA) ? Wk[i] : ~0ull; } else { ++j; kb = (j < nB) ? WkB[j] : ~0ull; }
+                    ++pos;
+                    const u32 f0 = !(a.x == 0.0 && a.y == 0.0);
+                    ok[v] = nk | (takeA ? 0ull : 1ull); o0r[v] = a.x; o0i[v] = a.y;
+                    fl |= f0 << (2 * v);
+                    nout += (int)f0;
                 }
-                u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
-                if (FIXED) {   // a pair always yields two entries, a lone term one (its nonzero row; row 0 if dead)
-                    if (has_partner) { f0 = 1; f1 = 1; } else { f0 = f1 ^ 1u; }
-                }
-                ok[v] = nk; o0r[v] = r0; o0i[v] = m0; o1r[v] = r1; o1i[v] = m1;
-                fl |= (f0 | (f1 << 1)) << (2 * v);
-                nout += (int)(f0 + f1);
-            } else {
-                const double2 a = takeA ? sa[i] : saB[j];
-                if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
-                ++pos;
-                const u32 f0 = FIXED ? 1u : (u32)!(a.x == 0.0 && a.y == 0.0);
-                ok[v] = nk | (takeA ? 0ull : 1ull); o0r[v] = a.x; o0i[v] = a.y;
-                fl |= f0 << (2 * v);
-                nout += (int)f0;
             }
         }
-    }
-    TSTAMP(6);
-    int total, excl;
-    if (FIXED) { excl = startpos; total = cnt; __syncthreads(); }   // the barrier retires every read of the input tile
-    else excl = block_excl_scan(nout, red, &total);
-    TSTAMP(7);   // its barriers also retire every read of the input tile
-    // stage the outputs in output order (the staging area aliases the consumed input tile and holds
-    // BP_TILE outputs: a gate that doubles the tile is written in two rounds), store them coalesced
-    for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_TILE) {
-        if (h0 > 0) __syncthreads();
-        if (PERM) {
+        int total;
+        const int excl = block_excl_scan(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
+        // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
+        // BP_TILE outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
+        for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_TILE) {
+            if (h0 > 0) __syncthreads();
+            {
+                int off = excl - h0;
 #pragma unroll
-            for (int v = 0; v < BP_VT; ++v)
-                if (opos[v] >= 0) { stk[opos[v]] = ok[v]; sta[opos[v]] = make_double2(o0r[v], o0i[v]); }
-        } else {
-            int off = excl - h0;
-#pragma unroll
-            for (int v = 0; v < BP_VT; ++v) {
-                const u32 f = (fl >> (2 * v)) & 3u;
-                if (f & 1u) {
-                    if ((unsigned)off < (unsigned)BP_TILE) { stk[off] = ok[v]; sta[off] = make_double2(o0r[v], o0i[v]); }
-                    ++off;
-                }
-                if (PAIR && (f & 2u)) {
-                    if ((unsigned)off < (unsigned)BP_TILE) { stk[off] = ok[v] | 1ull; sta[off] = make_double2(o1r[v], o1i[v]); }
-                    ++off;
+                for (int v = 0; v < BP_VT; ++v) {
+                    const u32 f = (fl >> (2 * v)) & 3u;
+                    if (f & 1u) {
+                        if ((unsigned)off < (unsigned)BP_TILE) { Wk[off] = ok[v]; La[off] = make_double2(o0r[v], o0i[v]); }
+                        ++off;
+                    }
+                    if (PAIR && (f & 2u)) {
+                        if ((unsigned)off < (unsigned)BP_TILE) { Wk[off] = ok[v] | 1ull; La[off] = make_double2(o1r[v], o1i[v]); }
+                        ++off;
+                    }
                 }
             }
-        }
-        if (FIXED) {
-            if (tid == 0) s_base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
-        } else if (h0 == 0 && tid < 32) {
-            const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
-            if (tid == 0) {
-                s_base = ex;
-                if (tile == ntiles - 1) *d_count = ex + (u64)total;
+            if (h0 == 0 && tid < 32) {
+                const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
+                if (tid == 0) {
+                    s_base = ex;
+                    if (tile == ntiles - 1) *d_count = ex + (u64)total;
+                }
+            }
+            __syncthreads();
+            const u64 base = s_base + (u64)h0;
+            const int m = min(total - h0, BP_TILE);
+            for (int idx = tid; idx < m; idx += SV_THREADS) {
+                const u64 g = base + (u64)idx;
+                if (g < cap) { st_stream_u64(kout + g, Wk[idx]); st_stream_d2(aout + g, La[idx]); }
             }
         }
-        TSTAMP(8);
-        __syncthreads();
-        TSTAMP(9);
-        const u64 base = s_base + (u64)h0;
-        const int m = min(total - h0, BP_TILE);
-        for (int idx = tid; idx < m; idx += SV_THREADS) {
-            const u64 g = base + (u64)idx;
-            if (g < cap) { st_stream_u64(kout + g, stk[idx]); st_stream_d2(aout + g, sta[idx]); }
-        }
+        __syncthreads();   // A* | B* and this landing buffer are reused
     }
-    __syncthreads();   // the staging area is the next tile's input buffer
-    }
-#ifdef BP_X_TIMING
-    if (tid == TWHO && blockIdx.x % 37 == 0) for (int k = 0; k < 10; ++k) atomicAdd(&g_bp_t[k], (unsigned long long)tacc[k]);
-#endif
 }
 
 template <int MODE, bool FIXED>
 static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
-                           const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
-    const size_t smem = (size_t)2 * BP_TILE * 24;   // landing buffer + work / staging buffer
+                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
+    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8 + 8 + 2);   // amplitudes x 2, landing keys, A* | B* keys, slots
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
@@ -348,20 +359,21 @@ static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double
         if (per_sm < 1) per_sm = 1;
     }
     const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    bitpass_kernel<MODE, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles);
+    bitpass_kernel<MODE, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles);
 }
 
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
+    (void)tile_counter;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
     cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
-#define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, tile_counter, d_count, cap, ntiles, st)
+#define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st)
     if (pair == 2) SV_BP(2, true);                       // monomial blocks: always position preserving
-    else if (pair) { if (fixed) SV_BP(1, true); else SV_BP(1, false); }
+    else if (pair) SV_BP(1, false);
     else { if (fixed) SV_BP(0, true); else SV_BP(0, false); }
 #undef SV_BP
     if (e1) cudaEventRecord(e1, st);
