@@ -8,13 +8,14 @@
 //   * every term that opens a tuple collects the tuple's presence mask and, from the zero pattern
 //     of U, the set of output rows that can be nonzero: the tile's output count is known before
 //     any arithmetic, so one scan + look-back fixes every output position;
-//   * the outputs are then computed ONE PER THREAD (thread t takes outputs t, t + 256, ...: it finds
-//     the tuple by a search over the per-term output offsets; column contributions are added in
+//   * the outputs are then computed ONE PER THREAD (thread t takes outputs t, t + 256, ... of a round
+//     of 2048; the opening terms post (term, row) per output first; column contributions are added in
 //     ascending logical column index, every operation rounded separately: DESIGN.md D1) and stored
 //     directly, consecutive threads writing consecutive entries.  A row that cancels to exactly 0+0i is written as a dead entry
 //     (counted, so the term count stays exact) instead of forcing a second scan.
 #include "sv_tile.cuh"
 
+#define GP_ROUND 2048
 template <int MA>
 __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                   u64* __restrict__ kout, double2* __restrict__ aout, int p,
@@ -29,7 +30,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
     u64* sk = Lk + BP_TILE;
     u64* s_info = sk + BP_TILE;                                // per term: the tuple it opens (rows, masks, control block)
-    int* s_offs = reinterpret_cast<int*>(s_info + BP_TILE);    // per term: outputs of the tile before it
+    unsigned short* s_owner = reinterpret_cast<unsigned short*>(s_info + BP_TILE);   // per output of a round: (term << 4) | row
     __shared__ int red[BP_WARPS + 2];
     __shared__ int wc[BP_VT][BP_WARPS];
     __shared__ int s_nA;
@@ -209,12 +210,9 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
         }
         int total;
         const int excl = block_excl_scan(mycount, red, &total);
-        {
-            int run = excl;
 #pragma unroll
-            for (int v = 0; v < BP_VT; ++v)
-                if (e0 + v < cnt) { s_offs[e0 + v] = run; s_info[e0 + v] = t_info[v]; run += __popc((u32)(t_info[v] & 0xffffu)); }
-        }
+        for (int v = 0; v < BP_VT; ++v)
+            if (e0 + v < cnt) s_info[e0 + v] = t_info[v];
         if (tid < 32) {
             const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
             if (tid == 0) {
@@ -223,34 +221,56 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
             }
         }
         __syncthreads();
-        // ---- phase 2b: one thread per OUTPUT: consecutive threads write consecutive entries ----
+        // ---- phase 2b: one thread per OUTPUT: consecutive threads write consecutive entries.  Outputs are
+        // taken GP_ROUND at a time: the opening terms first post (term, row) for each of their outputs of
+        // the round in s_owner, then every thread computes the outputs t, t + 256, ... of the round ----
         const u64 base = s_base;
-        for (int o = tid; o < total; o += SV_THREADS) {
-            int lo = o >> MA, hi = cnt - 1;                // the opening term L: last element with offs <= o (L >= o / 2^MA)
-            while (lo < hi) {
-                const int mid = (lo + hi + 1) >> 1;
-                if (s_offs[mid] <= o) lo = mid; else hi = mid - 1;
-            }
-            const int e = lo;
-            const u64 info = s_info[e];
-            const u32 rows = (u32)(info & 0xffffu), pm = (u32)((info >> 16) & 0xffffu), pk = (u32)((info >> 32) & 0xffffu);
-            const int cx = (int)(info >> 48);
-            const int r = __fns(rows, 0, o - s_offs[e] + 1);   // the (o - offs + 1)-th possible row
-            const u64 k = sk[e];
-            const double2* urow = &sU[((cx << MA) | r) << MA];
-            double sr = 0.0, si = 0.0;
+        for (int h0 = 0; h0 < total; h0 += GP_ROUND) {
+            if (excl < h0 + GP_ROUND && excl + mycount > h0) {
+                int off = excl - h0;
 #pragma unroll
-            for (int t = 0; t < NP; ++t) {                 // ascending LOGICAL column index (D1)
-                const int x = s_col[t];
-                if ((pm >> x) & 1u) {
+                for (int v = 0; v < BP_VT; ++v) {
+                    u32 rows = (u32)(t_info[v] & 0xffffu);
+                    while (rows) {
+                        const int r = __ffs(rows) - 1;
+                        rows &= rows - 1;
+                        if ((unsigned)off < (unsigned)GP_ROUND) s_owner[off] = (unsigned short)(((e0 + v) << 4) | r);
+                        ++off;
+                    }
+                }
+            }
+            __syncthreads();
+            const int m = min(total - h0, GP_ROUND);
+            for (int q = tid; q < m; q += SV_THREADS) {
+                const u32 code = s_owner[q];
+                const int e = (int)(code >> 4), r = (int)(code & 15u);
+                const u64 info = s_info[e];
+                const u32 pm = (u32)((info >> 16) & 0xffffu), pk = (u32)((info >> 32) & 0xffffu);
+                const int cx = (int)(info >> 48);
+                const u64 k = sk[e];
+                const double2* urow = &sU[((cx << MA) | r) << MA];
+                double sr = 0.0, si = 0.0;
+                if ((pm & (pm - 1)) == 0) {                    // a single live member: one product
+                    const int x = __ffs(pm) - 1;
                     const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
                     const double2 u = urow[x];
                     cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+                } else {
+#pragma unroll
+                    for (int t = 0; t < NP; ++t) {             // ascending LOGICAL column index (D1)
+                        const int x = s_col[t];
+                        if ((pm >> x) & 1u) {
+                            const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+                            const double2 u = urow[x];
+                            cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+                        }
+                    }
                 }
+                if (sr == 0.0 && si == 0.0) ++n_dead;          // exact cancellation: a dead entry
+                const u64 g = base + (u64)(h0 + q);
+                if (g < cap) { st_stream_u64(kout + g, (k & ~AM) | (u64)r); st_stream_d2(aout + g, make_double2(sr, si)); }
             }
-            if (sr == 0.0 && si == 0.0) ++n_dead;          // exact cancellation: a dead entry
-            const u64 g = base + (u64)o;
-            if (g < cap) { st_stream_u64(kout + g, (k & ~AM) | (u64)r); st_stream_d2(aout + g, make_double2(sr, si)); }
+            if (h0 + GP_ROUND < total) __syncthreads();        // s_owner is rewritten by the next round
         }
         __syncthreads();   // the work buffer and the tuple tables are reused by the next tile
     }
@@ -278,7 +298,7 @@ __global__ void find_starts_kernel(const u64* __restrict__ keys, u64 n, int ma, 
 template <int MA>
 static void launch_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                              const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 12;   // landing + work + tuple tables
+    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 8 + (size_t)GP_ROUND * 2;   // landing + work + tuple table + owners
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(grouppass_kernel<MA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
