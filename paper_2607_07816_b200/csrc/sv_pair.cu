@@ -36,6 +36,13 @@
 // entry (pure moves, monomial blocks).  Terms dropped by a pending truncation are carried as DEAD
 // entries (amplitude 0+0i) instead of being squeezed out, so the position of every output is known
 // from the tile descriptor alone: no scan, no look-back.
+// Staged outputs are written by threads that each own a few CONSECUTIVE output positions: without a
+// skew all lanes of a warp would hit the same banks (stride 4..8 entries).  One pad entry per 16 keys
+// (8 B) / per 8 amplitudes (16 B) makes those writes conflict free; the copy-out reads stay almost linear.
+#define BP_SWK(x) ((x) + ((x) >> 4))
+#define BP_SWA(x) ((x) + ((x) >> 3))
+#define BP_WKN (BP_TILE + BP_TILE / 16)        // entries of the key / slot work arrays
+#define BP_ROUND (BP_TILE - BP_TILE / 8)       // outputs staged per round when amplitudes are staged too (896 + 112 pads)
 template <int MODE, bool FIXED>
 __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
@@ -49,7 +56,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     double2* La1 = La0 + BP_TILE;
     u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);           // landing keys (consumed by prepare)
     u64* Wk = Lk + BP_TILE;                                    // A* | B* keys with bit p cleared; later the staged output keys
-    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk + BP_TILE);   // their landing slots; later the staged source slots
+    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk + BP_WKN);   // their landing slots; later the staged source slots
     __shared__ int red[BP_WARPS + 2];
     __shared__ int wc[BP_VT][BP_WARPS];
     __shared__ int s_nA;
@@ -207,15 +214,15 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
             __syncthreads();   // every read of A* | B* is done: stage by output position in the same arrays
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v)
-                if (opos[v] >= 0) { Wk[opos[v]] = okey[v]; Wi[opos[v]] = (unsigned short)osrc[v]; }
+                if (opos[v] >= 0) { Wk[BP_SWK(opos[v])] = okey[v]; Wi[BP_SWK(opos[v])] = (unsigned short)osrc[v]; }
             __syncthreads();
             // ---- copy-out: gather the amplitude, apply a pending truncation and the phase, store coalesced ----
             const u64 base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
             const int mc = PERM ? s_mc : 0;
             const bool phase = PERM && !s_unit;
             for (int idx = tid; idx < cnt; idx += SV_THREADS) {
-                const u64 key = Wk[idx];
-                double2 a = La[Wi[idx]];
+                const u64 key = Wk[BP_SWK(idx)];
+                double2 a = La[Wi[BP_SWK(idx)]];
                 const int row = (int)(key & 1ull);
                 int cx = 0, c = row;
                 if (PERM) {
@@ -310,8 +317,8 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
         int total;
         const int excl = block_excl_scan(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
-        // BP_TILE outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
-        for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_TILE) {
+        // BP_ROUND outputs per round, a gate that doubles the tile is written in up to three rounds), store coalesced
+        for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {
             if (h0 > 0) __syncthreads();
             {
                 int off = excl - h0;
@@ -319,17 +326,21 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                 for (int v = 0; v < BP_VT; ++v) {
                     const u32 f = (fl >> (2 * v)) & 3u;
                     if (f & 1u) {
-                        if ((unsigned)off < (unsigned)BP_TILE) { Wk[off] = ok[v]; La[off] = make_double2(o0r[v], o0i[v]); }
+                        if ((unsigned)off < (unsigned)BP_ROUND) { Wk[BP_SWK(off)] = ok[v]; La[BP_SWA(off)] = make_double2(o0r[v], o0i[v]); }
                         ++off;
                     }
                     if (PAIR && (f & 2u)) {
-                        if ((unsigned)off < (unsigned)BP_TILE) { Wk[off] = ok[v] | 1ull; La[off] = make_double2(o1r[v], o1i[v]); }
+                        if ((unsigned)off < (unsigned)BP_ROUND) { Wk[BP_SWK(off)] = ok[v] | 1ull; La[BP_SWA(off)] = make_double2(o1r[v], o1i[v]); }
                         ++off;
                     }
                 }
             }
             if (h0 == 0 && tid < 32) {
+#ifdef BP_X_NOLOOKBACK
+                const u64 ex = (u64)tile * BP_TNOM * 2;
+#else
                 const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
+#endif
                 if (tid == 0) {
                     s_base = ex;
                     if (tile == ntiles - 1) *d_count = ex + (u64)total;
@@ -337,10 +348,10 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
             }
             __syncthreads();
             const u64 base = s_base + (u64)h0;
-            const int m = min(total - h0, BP_TILE);
+            const int m = min(total - h0, BP_ROUND);
             for (int idx = tid; idx < m; idx += SV_THREADS) {
                 const u64 g = base + (u64)idx;
-                if (g < cap) { st_stream_u64(kout + g, Wk[idx]); st_stream_d2(aout + g, La[idx]); }
+                if (g < cap) { st_stream_u64(kout + g, Wk[BP_SWK(idx)]); st_stream_d2(aout + g, La[BP_SWA(idx)]); }
             }
         }
         __syncthreads();   // A* | B* and this landing buffer are reused
@@ -350,7 +361,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
 template <int MODE, bool FIXED>
 static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                            const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
-    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8 + 8 + 2);   // amplitudes x 2, landing keys, A* | B* keys, slots
+    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2);   // amplitudes x 2, landing keys, A* | B* keys, slots
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
