@@ -1,0 +1,129 @@
+"""GPU checks at BASELINE.json's full sizes, where the oracle cannot run the whole state: structural
+invariants, norm preservation, and SAMPLED outputs recomputed one by one on the host from the
+downloaded pre-gate state with the oracle's arithmetic (D1)."""
+import numpy as np
+import pytest
+
+from paper_2607_07816_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _recompute(keys_sorted, amps_sorted, qubits, U, out_keys):
+    """out amplitude of each key in out_keys: sum over columns c (ascending) of U[r, c] * a[base | scatter(c)],
+    absent members skipped, every product and sum rounded separately (numpy scalar float64 arithmetic)."""
+    m = len(qubits)
+    mask = 0
+    for q in qubits:
+        mask |= 1 << q
+    res = []
+    for k in out_keys:
+        k = int(k)
+        base = k & ~mask
+        r = sum(((k >> q) & 1) << j for j, q in enumerate(qubits))
+        sr, si = np.float64(0.0), np.float64(0.0)
+        for c in range(1 << m):
+            kc = base
+            for j, q in enumerate(qubits):
+                if (c >> j) & 1:
+                    kc |= 1 << q
+            i = int(np.searchsorted(keys_sorted, np.uint64(kc)))
+            if i < keys_sorted.size and int(keys_sorted[i]) == kc:
+                a = amps_sorted[i]
+                ur, ui = np.float64(U[r, c].real), np.float64(U[r, c].imag)
+                ar, ai = np.float64(a.real), np.float64(a.imag)
+                sr = sr + (ur * ar - ui * ai)
+                si = si + (ur * ai + ui * ar)
+        res.append(complex(sr, si))
+    return np.array(res)
+
+
+@pytest.mark.parametrize("log2n", [25])
+def test_gates_at_scale_sampled_recompute(log2n):
+    import torch
+    from paper_2607_07816_b200 import engine
+    n, nq = 1 << log2n, 52
+    g = torch.Generator(device="cuda"); g.manual_seed(7)
+    keys = torch.randint(0, 1 << nq, (int(n * 1.01),), device="cuda", dtype=torch.int64, generator=g).unique()[:n].contiguous()
+    n = int(keys.numel())
+    # make partners common: half of the keys get their qubit-40 partner stored as well
+    keys = torch.cat([keys[: n // 2], keys[: n // 2] ^ (1 << 40)]).unique().contiguous()
+    n = int(keys.numel())
+    amps = torch.randn(n, 2, device="cuda", dtype=torch.float64, generator=g).view(torch.complex128).reshape(n).contiguous()
+    amps /= amps.abs().pow(2).sum().sqrt()
+    sv = engine.SparseSV(nq, 4 * n + 1024)
+    rng = np.random.default_rng(3)
+    gates = [([40], W.mat_h()), ([11, 40], W.mat_mcx(2)), ([3, 40, 17], W.mat_mcx(3)), ([40], W.mat_rz(0.37)),
+             ([40, 9], W.haar_unitary(rng, 4, special=True)), ([45], W.haar_unitary(rng, 2))]
+    for qubits, U in gates:
+        sv.load_device(keys, amps)
+        k0, a0, _ = sv.export()
+        o = np.argsort(k0)
+        k0, a0 = k0[o], a0[o]
+        sv.apply_gate(qubits, U)
+        assert sv.check_invariants()
+        assert abs(sv.norm() - 1.0) <= 1e-12
+        k1, a1, _ = sv.export()
+        pick = rng.choice(k1.size, size=300, replace=False)
+        want = _recompute(k0, a0, qubits, U, k1[pick])
+        assert np.max(np.abs(want - a1[pick])) <= 1e-13, "sampled outputs differ from the definition"
+        # every pre-gate term must have at least one image: spot-check that images of sampled inputs exist
+        o1 = np.sort(k1)
+        mask = 0
+        for q in qubits:
+            mask |= 1 << q
+        pin = rng.choice(k0.size, size=300, replace=False)
+        got = 0
+        for k in k0[pin]:
+            base = int(k) & ~mask
+            lo = int(np.searchsorted(o1, np.uint64(base)))
+            # some key of the tuple (base | pattern) must be present in the output
+            hit = False
+            for c in range(1 << len(qubits)):
+                kc = base
+                for j, q in enumerate(qubits):
+                    if (c >> j) & 1:
+                        kc |= 1 << q
+                i = int(np.searchsorted(o1, np.uint64(kc)))
+                hit = hit or (i < o1.size and int(o1[i]) == kc)
+            got += hit
+        assert got == 300
+
+
+def test_config3_full_size_peak():
+    """BASELINE.json configs[2] at its full size: n = 26, 2^26 terms from the first H layer on (1.6 GB),
+    cap 2^26 never binding.  The most probable bit string must be the secret; the norm must stay 1."""
+    from paper_2607_07816_b200 import engine
+    c = W.config3()
+    sv = engine.SparseSV(c.n, (1 << c.n) + 1024)
+    for g in c.gates:
+        sv.apply_gate(g.qubits, g.U)
+        sv.truncate(c.max_terms, 1.0)
+    assert sv.num_terms() <= 1 << c.n
+    k, a, p = sv.top(4)
+    assert int(k[0]) == c.secret, "top bit string is not the secret"
+    assert p[0] > 0.2 and p[0] > 10 * p[1]
+    assert abs(sv.norm() - 1.0) <= 1e-10
+    assert sv.check_invariants()
+
+
+def test_config5_at_2e24_properties():
+    """BASELINE.json configs[4] (n = 56 mix, mass 1 - 1e-4) at K = 2^24: per-gate structural properties the
+    method fixes at any size -- kept count <= K, kept fraction >= the threshold when the cap does not bind,
+    norm 1 after every cut, strictly ascending unique keys."""
+    from paper_2607_07816_b200 import engine
+    K = 1 << 24
+    c = W.config5(num_gates=170, max_terms=K)
+    sv = engine.SparseSV(c.n, 8 * K)
+    for i, g in enumerate(c.gates):
+        sv.apply_gate(g.qubits, g.U)
+        n_pre = sv.num_terms()
+        kept = sv.truncate(c.max_terms, c.min_mass)
+        assert sv.num_terms() <= K
+        if n_pre <= K:
+            assert kept >= c.min_mass - 1e-12
+        assert 0.0 < kept <= 1.0 + 1e-15
+        if i % 10 == 9:
+            assert abs(sv.norm() - 1.0) <= 1e-11
+    assert sv.check_invariants()
+    assert sv.stats()["fallbacks"] <= 40
