@@ -53,6 +53,10 @@ struct sv_state {
     u64* smp_k[2];
     u32* smp_v[2];
     u32* smp_scr;
+    unsigned char* seg_cnt;  // per 32-entry segment: entries not below the sampled band (band compaction)
+    u32* chunk_cnt;          // per 1024-entry chunk: their sum, then the exclusive scan
+    bool band_valid;         // the last select ran through the sampled path: seg_cnt / sctl describe the current arrays
+    u64 band_above, band_cand;
     u64 sample_min_terms;   // states with fewer terms use the full-state select
     double mass_est;        // total mass of the current state if known (NaN: unknown); gates are taken as unitary
 };
@@ -93,7 +97,7 @@ int sv_sm_count() {
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
 
-struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, sctl, smp_k[2], smp_v[2], smp_scr, total; };
+struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, sctl, smp_k[2], smp_v[2], smp_scr, seg_cnt, chunk_cnt, total; };
 static ArenaLayout layout_for(u64 cap) {
     ArenaLayout L; size_t o = 0;
     for (int i = 0; i < 2; ++i) { L.keys[i] = o; o += align_up(cap * 8); }
@@ -110,6 +114,8 @@ static ArenaLayout layout_for(u64 cap) {
     for (int i = 0; i < 2; ++i) { L.smp_k[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 8); }
     for (int i = 0; i < 2; ++i) { L.smp_v[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 4); }
     L.smp_scr = o; o += align_up(svk_sort_scratch_bytes(SV_SAMPLE_MAX));
+    L.seg_cnt = o; o += align_up(cap / 32 + 256);
+    L.chunk_cnt = o; o += align_up((cap / 1024 + 8) * 4);
     L.total = o;
     return L;
 }
@@ -228,6 +234,8 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->sctl = (SampleCtl*)(s->arena + L.sctl);
     for (int i = 0; i < 2; ++i) { s->smp_k[i] = (u64*)(s->arena + L.smp_k[i]); s->smp_v[i] = (u32*)(s->arena + L.smp_v[i]); }
     s->smp_scr = (u32*)(s->arena + L.smp_scr);
+    s->seg_cnt = s->arena + L.seg_cnt;
+    s->chunk_cnt = (u32*)(s->arena + L.chunk_cnt);
     s->sample_min_terms = 1ull << 18;
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
@@ -561,6 +569,8 @@ static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 
 static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelState* out, bool* used) {
     *used = false;
     const u64 n = s->phys, n_live = s->count;   // stored entries (dead ones included) / live terms
+    // a band compaction can only follow when the cap will drop more than 1/8 of the stored entries
+    const bool want_band = max_terms != 0 && n > max_terms + max_terms / 8;
     const int alt = s->cur ^ 1;
     u64 m64 = n / 8;
     if (m64 > SV_SAMPLE_MAX) m64 = SV_SAMPLE_MAX;
@@ -576,7 +586,7 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     cudaEvent_t e0, e1;
     prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
     if (e0) cudaEventRecord(e0, st);
-    s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], st);
+    s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], want_band ? s->seg_cnt : nullptr, st);
     if (e1) cudaEventRecord(e1, st);
     DBG_SYNC("ss_classify");
     s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st);
@@ -586,14 +596,16 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     int rc = read_back(s, out, s->sel, sizeof(SelState));
     if (rc != SV_OK) return rc;
     const u64 cand = out->n_total;
+    s->band_above = out->kept_count; s->band_cand = cand;
     if (out->done == 3 || cand > n_live / 2) return SV_OK;   // band miss, or too many candidates to gain anything
     rc = select_levels(s, s->keys[alt], s->amps[alt], cand, cand, s->keys[alt] + cand, true, max_terms, min_mass, out);
     if (rc != SV_OK) return rc;
-    if (out->done == 1) *used = true;
+    if (out->done == 1) { *used = true; s->band_valid = want_band; }
     return SV_OK;
 }
 
 static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out) {
+    s->band_valid = false;
     const u64 n = s->phys;                    // callers have materialised any deferred truncation; dead entries may remain
     if (s->count >= s->sample_min_terms) {
         bool used = false;
@@ -637,6 +649,24 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     s->count = ss.final_count;
     s->stats.n_out = ss.final_count;
     if (kept_fraction) *kept_fraction = ss.kept_fraction;
+    // A cut that drops a large part of the stored entries (the cap after an expanding gate): the entries
+    // below the sampled band are squeezed out now, in one scan-free streaming pass, so that the following
+    // passes run on a dense array in their position-preserving variants.  The cut proper stays pending
+    // (the rejected candidates become dead entries); small cuts ride entirely on the next pass.
+    if (s->band_valid && !few_dead(s) && s->phys < (1ull << 32)) {
+        const int alt = s->cur ^ 1;
+        cudaEvent_t e0, e1;
+        prof_slot(s, SV_K_COMPACT, 24.0 * ((double)s->phys + (double)(s->band_above + s->band_cand)), &e0, &e1);
+        if (e0) cudaEventRecord(e0, s->stream);
+        s->stats.launches += svk_ss_band_compact(s->keys[s->cur], s->amps[s->cur], s->phys, s->sctl, s->seg_cnt, s->chunk_cnt,
+                                                 s->status, s->tile_counter, s->keys[alt], s->amps[alt], s->stream);
+        if (e1) cudaEventRecord(e1, s->stream);
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        s->cur = alt;
+        s->phys = s->band_above + s->band_cand;
+        s->band_valid = false;
+    }
     return SV_OK;
 }
 

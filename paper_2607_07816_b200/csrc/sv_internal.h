@@ -119,7 +119,12 @@ int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st);
 int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
                  cudaStream_t st);
-int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st);
+int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
+                    cudaStream_t st);
+// squeeze out the entries below the sampled band (uses the classify pass's per-segment counts)
+int svk_ss_band_compact(const u64* keys, const double2* amps, u64 n, const SampleCtl* ctl, const unsigned char* seg_cnt,
+                        u32* chunk_cnt, u64* scan_status, u32* tile_counter, u64* kout, double2* aout, cudaStream_t st);
+int svk_scan_u32(u32* data, u64 n, u64* status, u32* tile_counter, cudaStream_t st);
 int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st);
 int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
                 const PendPred& pd, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);

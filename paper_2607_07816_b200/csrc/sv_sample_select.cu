@@ -178,7 +178,7 @@ __device__ __forceinline__ void atomic_add_u128(u64* lohi, u128 v) {   // lohi[0
 // time: one global atomic and one batch of key loads per flush instead of one per iteration.
 __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
                                                                  u64 n, SampleCtl* __restrict__ ctl, u64* __restrict__ ckeys,
-                                                                 double2* __restrict__ camps) {
+                                                                 double2* __restrict__ camps, unsigned char* __restrict__ seg_cnt) {
     __shared__ double2 s_ba[SV_THREADS / 32][SC_WBUF];
     __shared__ u64 s_bi[SV_THREADS / 32][SC_WBUF];
     const u64 P_hi = ctl->P_hi, P_lo = ctl->P_lo;
@@ -221,6 +221,10 @@ __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __re
             n_blw += below ? 1u : 0u;
             const bool cand = ok && !above && !below;
             const u32 grp = __ballot_sync(0xffffffffu, cand);
+            if (seg_cnt) {   // entries of this 32-entry segment that a band compaction would keep (above or candidate)
+                const u32 nb = __ballot_sync(0xffffffffu, ok && !below);
+                if (lane == 0 && (c * chunk + (u64)r * SV_THREADS + (threadIdx.x & ~31)) < n) seg_cnt[(c * chunk + (u64)r * SV_THREADS + threadIdx.x) >> 5] = (unsigned char)__popc(nb);
+            }
             if (grp) {
                 if (cand) {
                     const int q = nbuf + __popc(grp & ((1u << lane) - 1u));
@@ -259,7 +263,8 @@ int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double
     ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n_live, max_terms, min_mass, mass_est, ctl);
     return 1;
 }
-int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, cudaStream_t st) {
+int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
+                    cudaStream_t st) {
     static int per_sm = 0;   // one wave of resident blocks: a grid-stride loop has no tail
     if (!per_sm) {
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_classify_kernel, SV_THREADS, 0);
@@ -268,6 +273,76 @@ int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl,
     u64 blocks = (n + SV_THREADS * SC_IT - 1) / (SV_THREADS * SC_IT);
     if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
     if (blocks < 1) blocks = 1;
-    ss_classify_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps);
+    ss_classify_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps, seg_cnt);
     return 1;
+}
+
+// ---------------------------------------------------------------------------------------
+// Band compaction: after a cut that drops a large part of the state (the cap after an expanding gate)
+// the entries BELOW the sampled band are squeezed out at once.  The classify pass has left, per
+// 32-entry segment, the number of entries that stay (above or candidate); a 1024-entry chunk sums
+// its 32 segments, an exclusive scan over the chunk sums gives every chunk its output offset, and
+// the scatter pass below needs neither a scan of its own nor a look-back: it streams like the
+// classify pass.  Rejected candidates stay behind as (few) dead entries for the pending cut.
+// ---------------------------------------------------------------------------------------
+__global__ void ss_chunk_sum_kernel(const unsigned char* __restrict__ seg_cnt, u64 nseg, u32 nchunks, u32* __restrict__ chunk_cnt) {
+    const u32 c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= nchunks) return;
+    u32 sum = 0;
+    for (int q = 0; q < 32; ++q) { const u64 sidx = (u64)c * 32 + q; if (sidx < nseg) sum += seg_cnt[sidx]; }
+    chunk_cnt[c] = sum;
+}
+__global__ void __launch_bounds__(SV_THREADS) ss_band_compact_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps, u64 n,
+                                                                    const SampleCtl* __restrict__ ctl,
+                                                                    const unsigned char* __restrict__ seg_cnt, const u32* __restrict__ chunk_off,
+                                                                    u64* __restrict__ kout, double2* __restrict__ aout) {
+    const u64 P_lo = ctl->P_lo;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const u64 chunk = (u64)SV_THREADS * SC_IT;
+    const u64 nchunks = (n + chunk - 1) / chunk;
+    const u64 nseg = (n + 31) >> 5;
+    for (u64 c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        double2 a[SC_IT];
+#pragma unroll
+        for (int r = 0; r < SC_IT; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            a[r] = (i < n) ? ld_stream_d2(amps + i) : make_double2(0.0, 0.0);
+        }
+        const u64 sidx = c * 32 + lane;                       // lane l holds segment l of the chunk
+        const u32 sc = (sidx < nseg) ? seg_cnt[sidx] : 0u;
+        u32 inc = sc;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const u32 t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+        const u32 segoff = inc - sc;
+        const u64 cbase = chunk_off[c];
+#pragma unroll
+        for (int r = 0; r < SC_IT; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            const bool alive = i < n && !(a[r].x == 0.0 && a[r].y == 0.0);
+            const bool keep = alive && (u64)__double_as_longlong(prob_of(a[r])) >= P_lo;
+            const u32 bal = __ballot_sync(0xffffffffu, keep);
+            const u32 off = __shfl_sync(0xffffffffu, segoff, r * (SV_THREADS / 32) + warp);
+            if (keep) {
+                const u64 pos = cbase + off + __popc(bal & ((1u << lane) - 1u));
+                st_stream_u64(kout + pos, ld_stream_u64(keys + i));
+                st_stream_d2(aout + pos, a[r]);
+            }
+        }
+    }
+}
+int svk_ss_band_compact(const u64* keys, const double2* amps, u64 n, const SampleCtl* ctl, const unsigned char* seg_cnt,
+                        u32* chunk_cnt, u64* scan_status, u32* tile_counter, u64* kout, double2* aout, cudaStream_t st) {
+    const u64 chunk = (u64)SV_THREADS * SC_IT;
+    const u32 nchunks = (u32)((n + chunk - 1) / chunk);
+    ss_chunk_sum_kernel<<<(nchunks + 255) / 256, 256, 0, st>>>(seg_cnt, (n + 31) >> 5, nchunks, chunk_cnt);
+    int launches = 1 + svk_scan_u32(chunk_cnt, nchunks, scan_status, tile_counter, st);
+    static int per_sm = 0;
+    if (!per_sm) {
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_band_compact_kernel, SV_THREADS, 0);
+        if (per_sm < 1) per_sm = 1;
+    }
+    u64 blocks = nchunks;
+    if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
+    ss_band_compact_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, seg_cnt, chunk_cnt, kout, aout);
+    return launches + 1;
 }

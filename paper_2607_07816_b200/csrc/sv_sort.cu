@@ -92,6 +92,16 @@ __global__ void __launch_bounds__(SV_THREADS) rs_scatter_kernel(const u64* __res
     }
 }
 
+// In-place exclusive scan of n u32 values.  status: (n / 2048 + 2) u64 words of scratch.
+int svk_scan_u32(u32* data, u64 n, u64* status, u32* tile_counter, cudaStream_t st) {
+    if (n == 0) return 0;
+    const u32 nscan = (u32)((n + RS_TILE - 1) / RS_TILE);
+    cudaMemsetAsync(status, 0, (size_t)nscan * 8 + 8, st);
+    cudaMemsetAsync(tile_counter, 0, sizeof(u32), st);
+    rs_scan_kernel<<<nscan, SV_THREADS, 0, st>>>(data, n, status, tile_counter);
+    return 1;
+}
+
 size_t svk_sort_scratch_bytes(u64 n) {
     const u64 ntiles = (n + RS_TILE - 1) / RS_TILE + 1;
     const u64 ncounts = 256 * ntiles;
