@@ -65,6 +65,8 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     __shared__ double2 sU[64];      // [cx][xr][xc], ma = 1: up to 8 control patterns x 4
     __shared__ int s_cpos[SV_MAX_M], s_mc;
     __shared__ int s_sw[8], s_unit; // PERM: block cx swaps the bit; every nonzero entry is exactly 1
+    __shared__ int s_ctrl_only;     // PERM: only the all-ones control pattern swaps (CNOT, Toffoli, C3X)
+    __shared__ u64 s_cmask;         // PERM: the control bits (new layout)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     if (PAIR || PERM) {
@@ -81,6 +83,12 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                 if (cx < (1 << gtab->mc) && !(x.x == 1.0 && x.y == 0.0 && y.x == 1.0 && y.y == 0.0)) unit = 0;
             }
             s_unit = unit;
+            const int full = (1 << gtab->mc) - 1;
+            int co = 1;
+            u64 cm = 0;
+            for (int cx = 0; cx <= full; ++cx) if (s_sw[cx] != (cx == full ? 1 : 0)) co = 0;
+            for (int q = 0; q < gtab->mc; ++q) cm |= 1ull << gtab->ctrl_pos[q];
+            s_ctrl_only = co; s_cmask = cm;
         }
     }
     const u64 bit = 1ull << p;
@@ -187,6 +195,9 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
             // ---- keys only: output key, source slot and output position of VT merged terms ----
             u64 okey[BP_VT]; int osrc[BP_VT], opos[BP_VT];
             u64 lastA = (PERM && i > 0) ? Wk[i - 1] : ~0ull;   // PERM: a B term's partner is the A term merged just before it
+            const bool ctrl_only = PERM && s_ctrl_only;
+            const u64 cmask = PERM ? s_cmask : 0ull;
+            const int mc_m = PERM ? s_mc : 0;
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v) {
                 okey[v] = 0; osrc[v] = 0; opos[v] = -1;
@@ -198,10 +209,14 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                     int row = takeA ? 0 : 1, shift = 0;
                     if (PERM) {
                         const bool partner = takeA ? (kb == k) : (lastA == k);
-                        int cx = 0;
-                        const int mc = s_mc;
-                        for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
-                        const int sw = s_sw[cx];
+                        int sw;
+                        if (ctrl_only) sw = ((nk & cmask) == cmask) ? 1 : 0;
+                        else {
+                            int cx = 0;
+                            for (int q = 0; q < mc_m; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
+                            sw = s_sw[cx];
+                        }
+                        osrc[v] |= (row << 15);                            // the term's ORIGINAL bit travels with its slot
                         if (partner && sw) shift = row ? -1 : 1;           // partners that swap rows trade places
                         row ^= sw;
                     }
@@ -222,19 +237,18 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
             const bool phase = PERM && !s_unit;
             for (int idx = tid; idx < cnt; idx += SV_THREADS) {
                 const u64 key = Wk[BP_SWK(idx)];
-                double2 a = La[Wi[BP_SWK(idx)]];
+                const u32 code = Wi[BP_SWK(idx)];
+                double2 a = La[code & 0x7fffu];
                 const int row = (int)(key & 1ull);
-                int cx = 0, c = row;
-                if (PERM) {
-                    for (int q = 0; q < mc; ++q) cx |= (int)((key >> s_cpos[q]) & 1ull) << q;
-                    c = row ^ s_sw[cx];
-                }
+                const int c = PERM ? (int)(code >> 15) : row;              // the bit the term had before the gate
                 if (pd.active) {
                     const u64 old = (key & himask) | ((key >> 1) & lowmask) | (c ? bit : 0ull);   // the stored key it came from
                     if (pend_keep(pd, old, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
                     else { a.x = 0.0; a.y = 0.0; }
                 }
                 if (phase) {
+                    int cx = 0;
+                    for (int q = 0; q < mc; ++q) cx |= (int)((key >> s_cpos[q]) & 1ull) << q;
                     const double2 u = sU[(cx << 2) | (row << 1) | c];
                     const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
                     const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
