@@ -64,13 +64,22 @@ __global__ void find_splits_kernel(const u64* __restrict__ keys, u64 n, int p, i
     const u64 lowmask = (1ull << p) - 1;
     const u64 kt = keys[t];
     const u64 blk = (p == 63) ? 0 : ((kt >> (p + 1)) << (p + 1));
-    const u64 s = (p == 63) ? 0 : lower_bound_g(keys, 0, t + 1, blk);
-    const u64 mid = lower_bound_g(keys, s, n, blk | (1ull << p));
-    u64 e = n;
-    if (p < 63) {
-        const u64 nxt = blk + (2ull << p);
-        if (nxt != 0) e = lower_bound_g(keys, mid, n, nxt);   // nxt == 0: wrapped, last block
+    // block start s, start of its B run mid, block end e: three lower bounds over the globally sorted keys,
+    // bracketed by t and advanced TOGETHER so that their dependent loads overlap
+    const u64 vmid = blk | (1ull << p);
+    const u64 nxt = (p == 63) ? 0 : blk + (2ull << p);
+    const bool has_e = (p < 63) && nxt != 0;                    // nxt == 0: wrapped, last block
+    u64 slo = 0, shi = (p == 63) ? 0 : t;                       // keys[t] >= blk: s in [0, t]
+    u64 mlo = (kt & (1ull << p)) ? 0 : t + 1, mhi = (kt & (1ull << p)) ? t : n;
+    u64 elo = has_e ? t + 1 : n, ehi = n;                       // keys[t] < nxt: e in [t + 1, n]
+    while (slo < shi || mlo < mhi || elo < ehi) {
+        const u64 sm = slo + ((shi - slo) >> 1), mm = mlo + ((mhi - mlo) >> 1), em = elo + ((ehi - elo) >> 1);
+        const u64 ks = (slo < shi) ? keys[sm] : 0, km = (mlo < mhi) ? keys[mm] : 0, ke = (elo < ehi) ? keys[em] : 0;
+        if (slo < shi) { if (ks < blk) slo = sm + 1; else shi = sm; }
+        if (mlo < mhi) { if (km < vmid) mlo = mm + 1; else mhi = mm; }
+        if (elo < ehi) { if (ke < nxt) elo = em + 1; else ehi = em; }
     }
+    const u64 s = slo, mid = mlo, e = elo;
     TileDesc d;
     d.mid = mid; d.e = e;
     if (last) { d.ia = mid; d.ib = e; desc[j] = d; return; }
