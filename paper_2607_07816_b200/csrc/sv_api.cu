@@ -133,6 +133,8 @@ static int cuda_fail(sv_state* s, cudaError_t e, const char* where) {
         cudaError_t e__ = (call);                                          \
         if (e__ != cudaSuccess) return cuda_fail(s, e__, #call);           \
     } while (0)
+// SV_DEBUG_SYNC=1 in the environment: synchronise after every kernel of the truncation path and name the
+// first one that failed (compute-sanitizer is not available on every box).
 static bool dbg_sync_on() { static int v = -1; if (v < 0) v = getenv("SV_DEBUG_SYNC") ? 1 : 0; return v == 1; }
 #define DBG_SYNC(tag)                                                                            \
     do {                                                                                         \
@@ -633,13 +635,6 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     SelState ss;
     rc = run_select(s, max_terms, min_mass, &ss);
     if (rc != SV_OK) return rc;
-    if (getenv("SV_DEBUG")) {
-        SampleCtl c; cudaMemcpy(&c, s->sctl, sizeof(c), cudaMemcpyDeviceToHost);
-        fprintf(stderr, "[trunc] n=%llu K=%llu seeded=%d PT=%016llx KT=%016llx final=%llu kept=%.17g tot=%.17g | P_hi=%016llx P_lo=%016llx above=%llu below=%llu cand=%llu ovf=%llu Eref=%d\n",
-                (unsigned long long)s->count, (unsigned long long)max_terms, ss.seeded, (unsigned long long)ss.PT, (unsigned long long)ss.KT,
-                (unsigned long long)ss.final_count, ss.kept_mass, ss.total_mass, (unsigned long long)c.P_hi, (unsigned long long)c.P_lo,
-                (unsigned long long)c.above_cnt, (unsigned long long)c.below_cnt, (unsigned long long)c.cand_cnt, (unsigned long long)c.overflow, c.Eref);
-    }
     s->mass_est = ss.total_mass;
     if (ss.final_count >= s->count) return SV_OK;   // nothing dropped: bitwise no-op (reading R7)
     s->mass_est = 1.0;                              // renormalised

@@ -55,36 +55,6 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, u32 tile, u64 tot
     return excl;
 }
 
-// Warp-parallel look-back: all 32 lanes of ONE warp call it; 32 predecessors are inspected
-// per round, so a tile never walks a long chain of not-yet-inclusive predecessors one by one.
-__device__ __forceinline__ u64 lookback_exclusive_warp(u64* status, u32 tile, u64 total) {
-    const int lane = threadIdx.x & 31;
-    if (tile == 0) {
-        if (lane == 0) st_relaxed_u64(&status[0], SV_FLAG_INCL | total);
-        return 0;
-    }
-    if (lane == 0) st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
-    u64 excl = 0;
-    long long j = (long long)tile - 1;
-    for (;;) {
-        const long long idx = j - lane;
-        u64 v = (idx >= 0) ? ld_relaxed_u64(&status[idx]) : SV_FLAG_INCL;   // virtual tile -1: inclusive 0
-        const u32 flagged = __ballot_sync(0xffffffffu, (v >> 62) != 0);
-        const u32 incl = __ballot_sync(0xffffffffu, (v >> 62) == 2);
-        const int first = incl ? (__ffs(incl) - 1) : 32;
-        const u32 need = (first >= 31) ? 0xffffffffu : ((2u << first) - 1u);
-        if ((flagged & need) != need) continue;   // a needed predecessor has not published yet
-        u64 c = (lane <= first) ? (v & SV_VAL_MASK) : 0;
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
-        excl += c;
-        if (first < 32) break;
-        j -= 32;
-    }
-    if (lane == 0) st_relaxed_u64(&status[tile], SV_FLAG_INCL | (excl + total));
-    return excl;
-}
-
 // Two-level look-back.  A chain of one-warp windows resolves at most 32 tiles per L2 round
 // trip; a pass over 2^28 terms has 2.6e5 tiles of ~9000 cycles on ~600 resident blocks, i.e.
 // one tile every ~15 cycles -- more than such a chain can carry.  Here tiles are grouped by

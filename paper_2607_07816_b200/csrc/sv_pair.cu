@@ -350,11 +350,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                 }
             }
             if (h0 == 0 && tid < 32) {
-#ifdef BP_X_NOLOOKBACK
-                const u64 ex = (u64)tile * BP_TNOM * 2;
-#else
                 const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
-#endif
                 if (tid == 0) {
                     s_base = ex;
                     if (tile == ntiles - 1) *d_count = ex + (u64)total;
