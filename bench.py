@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--jsonl", default="", help="optional per-gate JSONL log")
+    ap.add_argument("--no-circuits", action="store_true", help="skip the circuit wall times of configs 1-4")
     return ap.parse_args()
 
 
@@ -150,6 +151,43 @@ def run_reference(args):
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def run_circuits(engine, W, dev, torch):
+    """Wall time (CUDA events around the whole gate loop, after one untimed run) of configs 1-4 at the sizes
+    BASELINE.json names; truncation after every gate where the config says so."""
+    out = {}
+    specs = [("cfg1", W.config1(), 1 << 13), ("cfg2", W.config2(), 1 << 22), ("cfg3", W.config3(), (1 << 26) + 1024),
+             ("cfg4", W.config4(), 1 << 30)]
+    for name, c, cap in specs:
+        free_b, _ = torch.cuda.mem_get_info(dev)
+        if engine.lib.sv_arena_bytes(cap) > 0.9 * free_b:
+            out[name] = {"skipped": "arena does not fit"}
+            continue
+        res = None
+        for rep in range(2):
+            sv = engine.SparseSV(c.n, cap, device=dev)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); a.record()
+            log_kept, peak_terms = 0.0, 1
+            try:
+                for g in c.gates:
+                    sv.apply_gate(g.qubits, g.U)
+                    if c.truncate_every_gate:
+                        peak_terms = max(peak_terms, sv.stats()["n_out"])
+                        kept = sv.truncate(c.max_terms, c.min_mass)
+                        log_kept += float(np.log(kept))
+                b.record(); torch.cuda.synchronize()
+                k, _, p = sv.top(1)
+                res = {"n_qubits": c.n, "gates": len(c.gates), "wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(),
+                       "peak_terms_before_cut": int(peak_terms), "log_retained_mass": log_kept, "top_p": float(p[0]),
+                       "top_is_secret": (int(k[0]) == c.secret) if c.secret is not None else None,
+                       "variant": c.notes.get("variant")}
+            except engine.SvError as ex:
+                res = {"error": str(ex)}
+            sv.close()
+        out[name] = res
+    return out
 
 
 # ------------------------------------------------------------------------------------------
@@ -294,6 +332,12 @@ def run_ours(args):
                "d2h_bytes_per_step": d2h, "steps": e_steps,
                "note": "sv_load(host pinned state) + %d x (sv_apply_gate + sv_truncate) + sv_top(16); same gates every step" % G}
 
+    # ---- circuit wall times of BASELINE.json configs[0..3] at their full sizes (reported, not the headline) ----
+    circuits = None
+    if rank == 0 and world == 1 and not args.no_circuits:
+        sv.close()
+        circuits = run_circuits(engine, W, dev, torch)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = oracle_sample(16, G, 2, 0, budget_s=args.cpu_seconds)
@@ -309,7 +353,7 @@ def run_ours(args):
                            "l2": "inputs larger than L2 (state %.2f GB)" % (24.0 * K / 1e9),
                            "parallelism": "replicas x%d" % world},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
-                "per_class": per_class, "circuit_ms_per_gate": max_ms / (args.steps * G)}
+                "per_class": per_class, "circuit_ms_per_gate": max_ms / (args.steps * G), "circuits": circuits}
         print(json.dumps(line), flush=True)
     if log:
         log.close()
