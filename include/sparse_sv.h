@@ -108,7 +108,7 @@ int sv_load(sv_state *s, const uint64_t *keys, const sv_c128 *amps, uint64_t n);
 int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amps, uint64_t n);
 
 /* Tuning knobs.  SV_OPT_SAMPLE_MIN_TERMS: states with at least this many terms find the
- * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^18), smaller
+ * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^21), smaller
  * ones with the full-state radix select.  Both are exact; tests force either. */
 enum { SV_OPT_SAMPLE_MIN_TERMS = 0 };
 int sv_set_option(sv_state *s, int option, uint64_t value);

@@ -238,7 +238,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->smp_scr = (u32*)(s->arena + L.smp_scr);
     s->seg_cnt = s->arena + L.seg_cnt;
     s->chunk_cnt = (u32*)(s->arena + L.chunk_cnt);
-    s->sample_min_terms = 1ull << 18;
+    s->sample_min_terms = 1ull << 21;   // below ~2^21 terms the state sits in L2 and the full select has fewer launches
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
         sv_destroy(s);

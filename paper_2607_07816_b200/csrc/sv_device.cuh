@@ -139,6 +139,26 @@ __device__ __forceinline__ int block_excl_scan(int v, int* red, int* total) {
     return red[warp] + inc - v;
 }
 
+// The same with ONE barrier: every warp publishes its total, every thread sums the totals of the warps
+// before its own.  `red` (SV_THREADS/32 ints) must not be in use by a previous call that other threads
+// may still be reading: callers separate two calls by a barrier of their own (the tile loops do).
+__device__ __forceinline__ int block_excl_scan1(int v, int* red, int* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += t;
+    }
+    if (lane == 31) red[warp] = inc;
+    __syncthreads();
+    int before = 0, all = 0;
+#pragma unroll
+    for (int w = 0; w < SV_THREADS / 32; ++w) { const int c = red[w]; all += c; if (w < warp) before += c; }
+    *total = all;
+    return before + inc - v;
+}
+
 // Complex product and accumulation with every operation rounded separately (no FMA):
 // the arithmetic contract of DESIGN.md "Determinism" (D1).
 __device__ __forceinline__ void cmul_acc(double& sr, double& si, double ur, double ui, double ar, double ai) {

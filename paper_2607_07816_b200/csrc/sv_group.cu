@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
             }
         }
         int total;
-        const int excl = block_excl_scan(mycount, red, &total);
+        const int excl = block_excl_scan1(mycount, red, &total);
 #pragma unroll
         for (int v = 0; v < BP_VT; ++v)
             if (e0 + v < cnt) s_info[e0 + v] = t_info[v];

@@ -37,12 +37,13 @@
 // entries (amplitude 0+0i) instead of being squeezed out, so the position of every output is known
 // from the tile descriptor alone: no scan, no look-back.
 // Staged outputs are written by threads that each own a few CONSECUTIVE output positions: without a
-// skew all lanes of a warp would hit the same banks (stride 4..8 entries).  One pad entry per 16 keys
-// (8 B) / per 8 amplitudes (16 B) makes those writes conflict free; the copy-out reads stay almost linear.
-#define BP_SWK(x) ((x) + ((x) >> 4))
-#define BP_SWA(x) ((x) + ((x) >> 3))
-#define BP_WKN (BP_TILE + BP_TILE / 16)        // entries of the key / slot work arrays
-#define BP_ROUND (BP_TILE - BP_TILE / 8)       // outputs staged per round when amplitudes are staged too (896 + 112 pads)
+// skew all lanes of a warp would hit the same banks (stride 4..8 entries).  The column (entry index
+// within a 128-byte row: 16 keys / 8 amplitudes) is XORed with the row index, which spreads such
+// writes over the banks and keeps the copy-out reads of consecutive entries inside one row.
+#define BP_SWK(x) ((x) ^ (((x) >> 4) & 15))
+#define BP_SWA(x) ((x) ^ (((x) >> 3) & 7))
+#define BP_WKN BP_TILE                         // entries of the key / slot work arrays
+#define BP_ROUND BP_TILE                       // outputs staged per round when amplitudes are staged too
 template <int MODE, bool FIXED>
 __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
@@ -329,9 +330,9 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
             }
         }
         int total;
-        const int excl = block_excl_scan(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
+        const int excl = block_excl_scan1(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
-        // BP_ROUND outputs per round, a gate that doubles the tile is written in up to three rounds), store coalesced
+        // BP_ROUND outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
         for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {
             if (h0 > 0) __syncthreads();
             {
