@@ -58,8 +58,8 @@ __device__ __forceinline__ u64 lower_bound_g(const u64* __restrict__ keys, u64 l
 __global__ void find_splits_kernel(const u64* __restrict__ keys, u64 n, int p, int w, u32 tnom, u32 ntiles,
                                    TileDesc* __restrict__ desc) {
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j > ntiles) return;
-    const bool last = (j == ntiles);
+    const bool active = j <= ntiles;               // (no early return: the warp shares search results below)
+    const bool last = (j >= ntiles);
     const u64 t = last ? n - 1 : (u64)j * tnom;   // n >= 1 here
     const u64 lowmask = (1ull << p) - 1;
     const u64 kt = keys[t];
@@ -69,9 +69,16 @@ __global__ void find_splits_kernel(const u64* __restrict__ keys, u64 n, int p, i
     const u64 vmid = blk | (1ull << p);
     const u64 nxt = (p == 63) ? 0 : blk + (2ull << p);
     const bool has_e = (p < 63) && nxt != 0;                    // nxt == 0: wrapped, last block
+    // Boundaries of one warp that fall into the same block share s, mid and e: only the first lane of each
+    // block searches (its brackets hold for the whole block), the others take its result.
+    const int lane = threadIdx.x & 31;
+    const unsigned peers = __match_any_sync(0xffffffffu, active ? blk : (~0ull - (u64)lane));
+    const int leader = __ffs(peers) - 1;
+    const bool searching = active && lane == leader;
     u64 slo = 0, shi = (p == 63) ? 0 : t;                       // keys[t] >= blk: s in [0, t]
     u64 mlo = (kt & (1ull << p)) ? 0 : t + 1, mhi = (kt & (1ull << p)) ? t : n;
     u64 elo = has_e ? t + 1 : n, ehi = n;                       // keys[t] < nxt: e in [t + 1, n]
+    if (!searching) { shi = slo; mhi = mlo; ehi = elo; }
     while (slo < shi || mlo < mhi || elo < ehi) {
         const u64 sm = slo + ((shi - slo) >> 1), mm = mlo + ((mhi - mlo) >> 1), em = elo + ((ehi - elo) >> 1);
         const u64 ks = (slo < shi) ? keys[sm] : 0, km = (mlo < mhi) ? keys[mm] : 0, ke = (elo < ehi) ? keys[em] : 0;
@@ -79,7 +86,9 @@ __global__ void find_splits_kernel(const u64* __restrict__ keys, u64 n, int p, i
         if (mlo < mhi) { if (km < vmid) mlo = mm + 1; else mhi = mm; }
         if (elo < ehi) { if (ke < nxt) elo = em + 1; else ehi = em; }
     }
-    const u64 s = slo, mid = mlo, e = elo;
+    const u64 s = __shfl_sync(0xffffffffu, slo, leader), mid = __shfl_sync(0xffffffffu, mlo, leader),
+              e = __shfl_sync(0xffffffffu, elo, leader);
+    if (!active) return;
     TileDesc d;
     d.mid = mid; d.e = e;
     if (last) { d.ia = mid; d.ib = e; desc[j] = d; return; }
