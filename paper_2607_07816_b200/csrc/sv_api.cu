@@ -60,7 +60,7 @@ struct sv_state {
     u64 sample_min_terms;   // states with fewer terms use the full-state select
     double mass_est;        // total mass of the current state if known (NaN: unknown); gates are taken as unitary
 };
-#define SV_SAMPLE_MAX (1u << 17)
+#define SV_SAMPLE_MAX (1u << 16)
 
 static void prof_drain(sv_state* s) {
     if (!s->npend) return;
@@ -582,7 +582,7 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st);
     DBG_SYNC("ss_sample");
     int in_alt = 0;
-    s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 32, s->smp_scr, st, &in_alt);
+    s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, st, &in_alt);   // keys are 24-bit pattern prefixes + 1 (< 2^24: finite p)
     s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st);
     DBG_SYNC("ss_sort+pivot");
     cudaEvent_t e0, e1;

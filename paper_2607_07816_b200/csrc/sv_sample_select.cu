@@ -4,8 +4,8 @@
 // histogram passes over the whole state.  Here ONE streaming pass over the amplitudes is
 // enough in the common case:
 //
-//   1. sample     M evenly spaced terms -> the top 32 bits of their probability patterns,
-//                 sorted (a 1 MB LSD radix sort that lives in L2);
+//   1. sample     M evenly spaced terms -> the top 24 bits of their probability patterns,
+//                 sorted (a 0.5 MB LSD radix sort that lives in L2);
 //   2. pivots     from the sorted sample, two patterns P_lo <= P_hi that bracket the cut
 //                 with wide statistical margins, for the top-k criterion (a quantile) and
 //                 for the p-mass criterion (the tail of the sample whose scaled mass is
@@ -28,18 +28,22 @@
 
 typedef unsigned __int128 u128;
 
+// The sample keeps the top 24 bits of a probability pattern (sign, exponent, 12 mantissa bits: 2.4e-4
+// relative resolution, far finer than the statistical margins of the pivots): three 8-bit sort passes.
+#define SS_DROP 40
+
 __global__ void __launch_bounds__(SV_THREADS) ss_sample_kernel(const double2* __restrict__ amps, u64 n, u32 M,
                                                                u64* __restrict__ smp) {
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= M) return;
     const u64 i = (u64)(((u128)j * n) / M);
     const double2 a = ld_stream_d2(amps + i);
-    // dead entries (0+0i) sort to the front as key 0; live terms get their pattern's top bits + 1
-    smp[j] = (a.x == 0.0 && a.y == 0.0) ? 0ull : (((u64)__double_as_longlong(prob_of(a)) >> 32) + 1ull);
+    // dead entries (0+0i) sort to the front as key 0; live terms get their pattern's top 24 bits + 1
+    smp[j] = (a.x == 0.0 && a.y == 0.0) ? 0ull : (((u64)__double_as_longlong(prob_of(a)) >> SS_DROP) + 1ull);
 }
 
-__device__ __forceinline__ double smp_prob(u64 top32) {   // mid-point of the values sharing these top bits
-    return __longlong_as_double((long long)((top32 << 32) | 0x80000000ull));
+__device__ __forceinline__ double smp_prob(u64 top) {   // mid-point of the values sharing these top bits
+    return __longlong_as_double((long long)((top << SS_DROP) | (1ull << (SS_DROP - 1))));
 }
 
 // One block of 1024 threads.  smp[0..M) ascending; the first z entries are 0 (dead sample points),
@@ -137,9 +141,9 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
     }
     SampleCtl c;
     memset(&c, 0, sizeof(c));
-    c.P_lo = (lo_idx <= 0 || Ml == 0) ? 0ull : ((live[min((long long)Ml, lo_idx) - 1] - 1) << 32);
-    c.P_hi = (hi_idx >= (long long)Ml) ? ~0ull : (((live[hi_idx] - 1) << 32) | 0xffffffffull);
-    int er = (Ml ? (int)((live[Ml - 1] - 1) >> 20) : 1023) + 12;
+    c.P_lo = (lo_idx <= 0 || Ml == 0) ? 0ull : ((live[min((long long)Ml, lo_idx) - 1] - 1) << SS_DROP);
+    c.P_hi = (hi_idx >= (long long)Ml) ? ~0ull : (((live[hi_idx] - 1) << SS_DROP) | ((1ull << SS_DROP) - 1));
+    int er = (Ml ? (int)((live[Ml - 1] - 1) >> (52 - SS_DROP)) : 1023) + 12;
     c.Eref = er > 2046 ? 2046 : er;
     *ctl = c;
 }
