@@ -542,6 +542,30 @@ static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 
     if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n_live, max_terms, min_mass, s->stream);
     int phase = 0;
     u64 ties = 0;
+    {   // The usual course of a select -- exponent level, up to three pattern levels, the tie keys, two key
+        // levels -- is launched AHEAD without reading anything back: every pass and step checks on the
+        // device that it is the select's current phase and is a no-op otherwise.  One read-back follows.
+        cudaEvent_t e0, e1;
+        prof_slot(s, SV_K_SELHIST, 16.0 * (double)n, &e0, &e1);
+        if (e0) cudaEventRecord(e0, s->stream);
+        static const int chain[7] = {0, 1, 1, 1, 2, 3, 3};
+        for (int c = 0; c < 7; ++c) {
+            const int ph = chain[c];
+            if (ph <= 1) s->stats.launches += svk_sel_pass(ph, amps, nullptr, n, s->sel, s->hist, s->stream);
+            else if (ph == 2) s->stats.launches += svk_sel_extract(keys, amps, n, s->sel, km, lk, s->hist, s->stream);
+            else s->stats.launches += svk_sel_pass(2, nullptr, lk, n, s->sel, s->hist, s->stream);
+            s->stats.launches += svk_sel_step(s->sel, s->hist, s->stream, ph);
+        }
+        if (e1) cudaEventRecord(e1, s->stream);
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        int rc = read_back(s, out, s->sel, sizeof(SelState));
+        if (rc != SV_OK) return rc;
+        if (out->done == 1 || out->done == 3) return SV_OK;
+        if (out->done != 0) return fail(s, SV_ERR_CUDA, "internal: radix select inconsistency");
+        phase = out->phase;
+        ties = out->tie_total;
+    }
     for (int it = 0; it < 64; ++it) {
         cudaEvent_t e0, e1;
         const double bytes = phase <= 1 ? 16.0 * (double)n : (phase == 2 ? 16.0 * (double)n + 16.0 * (double)ties : 8.0 * (double)ties);

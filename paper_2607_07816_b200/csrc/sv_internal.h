@@ -114,7 +114,7 @@ int svk_sel_init(SelState* ss, u64* hist, u64 n_live, u64 max_terms, double min_
 int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const SelState* ss, u64* hist, cudaStream_t st);
 int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
                     cudaStream_t st);
-int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st);
+int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st, int expected_phase = -1);
 // sampled fast path: sample -> (sort) -> pivots -> classify -> seed the select state
 int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,

@@ -116,6 +116,10 @@ int svk_sel_init(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass,
 template <int MODE>
 __global__ void __launch_bounds__(SV_THREADS) sel_pass_kernel(const double2* __restrict__ amps, const u64* __restrict__ lkeys,
                                                               u64 n, const SelState* __restrict__ ssp, u64* __restrict__ hist) {
+    // Launched ahead of the decision steps (see select_levels): a pass whose level is not the select's
+    // current phase, or that comes after the cut is final, does nothing.
+    if (ssp->done != 0 || ssp->phase != (MODE == 0 ? 0 : (MODE == 1 ? 1 : 3))) return;
+    if (MODE == 2 && ssp->tie_total < n) n = ssp->tie_total;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u32* scnt = reinterpret_cast<u32*>(smem_raw);
     u32* sand_lo = scnt + RS_BINS;
@@ -222,6 +226,7 @@ int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const S
 __global__ void __launch_bounds__(SV_THREADS) sel_extract_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
                                                                  u64 n, const SelState* __restrict__ ssp, KeyMap km,
                                                                  u64* __restrict__ lk_out, u64* __restrict__ hist) {
+    if (ssp->done != 0 || ssp->phase != 2) return;
     const u64 PT = ssp->PT;
     const int lane = threadIdx.x & 31;
     u64 a_and = ~0ull, a_or = 0;
@@ -322,7 +327,9 @@ __device__ __forceinline__ dd prod_u64_double(u64 t, double pv) {   // t * pv, e
     return two_sum(hi, __fma_rn(td, pv, -hi));
 }
 
-__global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64* hist) {
+__global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64* hist, int expected_phase) {
+    // expected_phase >= 0: the step of a pass that was launched ahead; it only runs if that pass ran
+    if (expected_phase >= 0 && (ssp->done != 0 || ssp->phase != expected_phase)) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     u64* h = reinterpret_cast<u64*>(smem_raw);
     for (int i = threadIdx.x; i < H_TOTAL; i += SV_THREADS) {
@@ -497,10 +504,10 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
     }
     *ssp = s;
 }
-int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st) {
+int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st, int expected_phase) {
     const size_t smem = (size_t)H_TOTAL * 8 + (size_t)RS_BINS * 16 + (size_t)SV_THREADS * 24;
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(sel_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
-    sel_step_kernel<<<1, SV_THREADS, smem, st>>>(ss, hist);
+    sel_step_kernel<<<1, SV_THREADS, smem, st>>>(ss, hist, expected_phase);
     return 1;
 }
