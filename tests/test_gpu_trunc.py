@@ -215,3 +215,41 @@ def test_pending_cut_and_dead_entries_twin(eng):
     assert_truncation_parity(sv.export()[:2], twin.export()[:2])
     assert sv.check_invariants()
     assert abs(sv.norm() - 1.0) <= 1e-12
+
+
+def test_monomial_phase_gates_and_bit63_with_pending_cut(eng):
+    """Position-preserving passes under a pending cut: monomial blocks with phases (controlled-Y), a plain
+    CNOT on qubit 63, pure moves inside a 3-qubit gate, a diagonal gate -- each applied right after a
+    truncation (no export in between) and compared with the oracle through a twin engine."""
+    rng = np.random.default_rng(21)
+    n = 64
+    keys, amps = W.random_state(rng, n, 40000, spread=1.0)
+    # give many terms a stored partner on qubits 63 and 7
+    keys = np.unique(np.concatenate([keys, keys[:15000] ^ np.uint64(1 << 63), keys[5000:20000] ^ np.uint64(1 << 7)]))
+    amps = (rng.standard_normal(keys.size) + 1j * rng.standard_normal(keys.size)) * np.exp(rng.standard_normal(keys.size))
+    amps /= np.sqrt(np.sum(np.abs(amps) ** 2))
+    sv = eng.SparseSV(n, 1 << 20)
+    twin = eng.SparseSV(n, 1 << 20)
+    sv.load(keys, amps)
+    twin.load(keys, amps)
+    cy = np.zeros((4, 4), dtype=np.complex128)       # controlled-Y, qubits = (control, target)
+    cy[0, 0] = cy[2, 2] = 1
+    cy[3, 1] = 1j
+    cy[1, 3] = -1j
+    gates = [([5, 63], cy), ([63, 7], W.mat_mcx(2)), ([7, 63], W.mat_mcx(2)), ([63], W.mat_rz(0.7)),
+             ([63, 7, 30], W.haar_unitary(rng, 8)), ([11, 7], cy), ([7], W.mat_h()), ([40, 41, 63], W.mat_mcx(3)),
+             ([63, 2], np.diag(np.exp(1j * rng.uniform(0, 6, 4)))), ([2, 63], W.haar_unitary(rng, 4))]
+    for i, (qs, U) in enumerate(gates):
+        f = 0.999 if i % 2 == 0 else 0.97
+        kcap = 0 if i % 3 else 30000
+        kg, kt = sv.truncate(kcap, f), twin.truncate(kcap, f)
+        assert kg == kt
+        k0, a0, _ = twin.export()
+        o = _oracle(n)
+        o.load(k0, a0)
+        sv.apply_gate(qs, U)
+        twin.apply_gate(qs, U)
+        o.apply_gate(qs, U)
+        assert sv.num_terms() == o.num_terms(), "gate %d" % i
+        assert_same_state(sv.export()[:2], o.export()[:2])
+        assert sv.check_invariants()
