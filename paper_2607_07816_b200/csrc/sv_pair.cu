@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
 #pragma unroll
                 for (int r = 0; r < BP_VT; ++r) {
                     const int e = tid + r * SV_THREADS;
-                    if (e < cnt) { Wk[e] = lk[r] & ~bit; Wi[e] = (unsigned short)e; }
+                    if (e < cnt) Wk[e] = lk[r] & ~bit;   // (the landing slot of entry e is e itself: Wi is not needed)
                 }
             } else {             // stable partition by bit p (the load order is the stored order)
                 u32 balA[BP_VT];
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                     const bool takeA = ka <= kb;
                     const u64 k = takeA ? ka : kb;
                     const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
-                    osrc[v] = takeA ? Wi[i] : WiB[j];
+                    osrc[v] = pc.oneblock ? (takeA ? i : nA + j) : (takeA ? (int)Wi[i] : (int)WiB[j]);
                     int row = takeA ? 0 : 1, shift = 0;
                     if (PERM) {
                         const bool partner = takeA ? (kb == k) : (lastA == k);
@@ -290,12 +290,12 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                     double2 a, pa = make_double2(0.0, 0.0);
                     bool has_partner = false;
                     if (takeA) {
-                        a = amp_at(Wi[i], k); ++i; ++pos;
+                        a = amp_at(pc.oneblock ? i : (int)Wi[i], k); ++i; ++pos;
                         has_partner = (kb == k);
-                        if (has_partner) { pa = amp_at(WiB[j], k | bit); ++j; ++pos; kb = (j < nB) ? WkB[j] : ~0ull; }
+                        if (has_partner) { pa = amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit); ++j; ++pos; kb = (j < nB) ? WkB[j] : ~0ull; }
                         ka = (i < nA) ? Wk[i] : ~0ull;
                     } else {
-                        a = amp_at(WiB[j], k | bit); ++j; ++pos;
+                        a = amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit); ++j; ++pos;
                         kb = (j < nB) ? WkB[j] : ~0ull;
                     }
                     int cx = 0;
@@ -319,7 +319,7 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                     fl |= (f0 | (f1 << 1)) << (2 * v);
                     nout += (int)(f0 + f1);
                 } else {   // compacting move
-                    const double2 a = takeA ? amp_at(Wi[i], k) : amp_at(WiB[j], k | bit);
+                    const double2 a = takeA ? amp_at(pc.oneblock ? i : (int)Wi[i], k) : amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit);
                     if (takeA) { ++i; ka = (i < nA) ? Wk[i] : ~0ull; } else { ++j; kb = (j < nB) ? WkB[j] : ~0ull; }
                     ++pos;
                     const u32 f0 = !(a.x == 0.0 && a.y == 0.0);
@@ -390,7 +390,8 @@ int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u6
     (void)tile_counter;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
-    cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
+    if (!(pair == 2 || (!pair && fixed)))   // the position-preserving variants have no scan
+        cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
 #define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st)
