@@ -120,10 +120,10 @@ int sv_get_stats(sv_state *s, sv_stats *out);
  * launch of the main kernels be bracketed by CUDA events on the state's stream;
  * sv_profile_get synchronises and returns, for one kernel, the summed device time, the
  * number of launches and the ALGORITHMIC bytes they had to move (DESIGN.md "Kernels":
- * diagonal 40 B/term; bit move 48 B/term; final pass of a one-bit gate (bitpass) and of a
- * multi-bit gate (grouppass) 24 B x (N_in + N_out); select histogram 16 B/term; compaction
+ * diagonal 40 B/term; bit move 48 B/term; final pass of a one-bit gate (bitpass: monomial blocks,
+ * position preserving; bitpass_gen: general blocks) and of a multi-bit gate (grouppass) 24 B x (N_in + N_out); select histogram 16 B/term; compaction
  * 24 B x (N_in + N_kept); sampled classification 16 B/term). */
-enum { SV_K_DIAG = 0, SV_K_MOVE = 1, SV_K_BITPASS = 2, SV_K_SELHIST = 3, SV_K_COMPACT = 4, SV_K_CLASSIFY = 5, SV_K_GROUPPASS = 6, SV_K_COUNT = 7 };
+enum { SV_K_DIAG = 0, SV_K_MOVE = 1, SV_K_BITPASS = 2, SV_K_SELHIST = 3, SV_K_COMPACT = 4, SV_K_CLASSIFY = 5, SV_K_GROUPPASS = 6, SV_K_BITPASS_GEN = 7, SV_K_COUNT = 8 };
 typedef struct { double ms; uint64_t launches; double alg_bytes; } sv_kernel_prof;
 int sv_profile(sv_state *s, int enable);
 int sv_profile_get(sv_state *s, int kernel, sv_kernel_prof *out);

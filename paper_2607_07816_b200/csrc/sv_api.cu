@@ -502,7 +502,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.n_out = s->count;
         return SV_OK;
     }
-    prof_slot(s, ma == 1 ? SV_K_BITPASS : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
+    prof_slot(s, ma == 1 ? SV_K_BITPASS_GEN : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
     const int gslot = s->npend - 1;
     const u64 n_live_in = s->count;
     if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)

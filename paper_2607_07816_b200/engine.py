@@ -19,7 +19,7 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option"]
-KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass"]
+KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
 
 
