@@ -42,7 +42,7 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--jsonl", default="", help="optional per-gate JSONL log")
-    ap.add_argument("--no-circuits", action="store_true", help="skip the circuit wall times of configs 1-4")
+    ap.add_argument("--no-circuits", action="store_true", help="skip the circuit wall times of configs 1-5")
     return ap.parse_args()
 
 
@@ -154,18 +154,19 @@ def run_reference(args):
 
 
 def run_circuits(engine, W, dev, torch):
-    """Wall time (CUDA events around the whole gate loop, after one untimed run) of configs 1-4 at the sizes
-    BASELINE.json names; truncation after every gate where the config says so."""
+    """Wall time (CUDA events around the whole gate loop, after one untimed run for configs 1-4) of the five
+    configs at the sizes BASELINE.json names; truncation after every gate where the config says so."""
     out = {}
-    specs = [("cfg1", W.config1(), 1 << 13), ("cfg2", W.config2(), 1 << 22), ("cfg3", W.config3(), (1 << 26) + 1024),
-             ("cfg4", W.config4(), 1 << 30)]
-    for name, c, cap in specs:
+    specs = [("cfg1", W.config1(), 1 << 13, 2), ("cfg2", W.config2(), 1 << 22, 2), ("cfg3", W.config3(), (1 << 26) + 1024, 2),
+             ("cfg4", W.config4(), 1 << 30, 2), ("cfg5", W.config5(), 1 << 31, 1)]   # cfg5: all 4000 gates, once
+    for name, c, cap, reps in specs:
+        torch.cuda.empty_cache()      # the previous arena sits in torch's cache; hand it back before asking
         free_b, _ = torch.cuda.mem_get_info(dev)
         if engine.lib.sv_arena_bytes(cap) > 0.9 * free_b:
             out[name] = {"skipped": "arena does not fit"}
             continue
         res = None
-        for rep in range(2):
+        for rep in range(reps):
             sv = engine.SparseSV(c.n, cap, device=dev)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             torch.cuda.synchronize(); a.record()
@@ -181,6 +182,7 @@ def run_circuits(engine, W, dev, torch):
                 k, _, p = sv.top(1)
                 res = {"n_qubits": c.n, "gates": len(c.gates), "wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(),
                        "peak_terms_before_cut": int(peak_terms), "log_retained_mass": log_kept, "top_p": float(p[0]),
+                       "norm": sv.norm(), "select_fallbacks": sv.stats()["fallbacks"],
                        "top_is_secret": (int(k[0]) == c.secret) if c.secret is not None else None,
                        "variant": c.notes.get("variant")}
             except engine.SvError as ex:
@@ -332,7 +334,7 @@ def run_ours(args):
                "d2h_bytes_per_step": d2h, "steps": e_steps,
                "note": "sv_load(host pinned state) + %d x (sv_apply_gate + sv_truncate) + sv_top(16); same gates every step" % G}
 
-    # ---- circuit wall times of BASELINE.json configs[0..3] at their full sizes (reported, not the headline) ----
+    # ---- circuit wall times of BASELINE.json configs[0..4] at their full sizes (reported, not the headline) ----
     circuits = None
     if rank == 0 and world == 1 and not args.no_circuits:
         sv.close()
