@@ -52,7 +52,9 @@ typedef struct {
     uint64_t n_in;         /* terms before the last call                                    */
     uint64_t n_out;        /* terms after it (N_pre for a gate, N_kept for a truncate)      */
     uint64_t launches;     /* kernels launched by this handle since creation                */
-    uint64_t fallbacks;    /* truncations whose sampled fast path missed and re-ran the full select */
+    uint64_t fallbacks;    /* sampled estimates that missed: truncations that re-ran the full select, fused gates that re-ran without a floor */
+    uint64_t n_mid;        /* sv_apply_gate_truncate: terms of the gate's output before the cut (logical; not all were written) */
+    uint64_t pre_dropped;  /* outputs the last gate did not write because the cut that follows drops them (fused call)          */
 } sv_stats;
 
 /* Bytes of device memory a state of this capacity needs (for sv_create_in_arena). */
@@ -88,6 +90,18 @@ int sv_apply_gate(sv_state *s, const int *qubits, int m, const sv_c128 *U);
  * *kept_fraction (nullable) receives kept mass / total mass. */
 int sv_truncate(sv_state *s, uint64_t max_terms, double min_mass, double *kept_fraction);
 
+/* sv_apply_gate followed by sv_truncate with these arguments, as ONE call (every
+ * gate, or fused block of gates, is applied and the state truncated before the next).  The result
+ * -- kept set, amplitudes, *kept_fraction -- is that of the two calls; knowing the cut that
+ * follows, the engine may estimate a floor for it from a sample of the gate's outputs and never
+ * write the outputs below that floor: less memory traffic,
+ * and a peak term count near max_terms instead of 2^m x N_in.  Arguments, errors and ownership as
+ * for the two calls; on an error from the gate nothing changed, on an error from the truncation
+ * the gate has been applied.  sv_get_stats then reports the gate's class, n_in = terms before the
+ * gate, n_out = terms kept. */
+int sv_apply_gate_truncate(sv_state *s, const int *qubits, int m, const sv_c128 *U,
+                           uint64_t max_terms, double min_mass, double *kept_fraction);
+
 /* *mass = sum of |a|^2 over all terms (Eq. 4) -- the mass, not its root. */
 int sv_norm(sv_state *s, double *mass);
 
@@ -109,8 +123,11 @@ int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amp
 
 /* Tuning knobs.  SV_OPT_SAMPLE_MIN_TERMS: states with at least this many terms find the
  * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^21), smaller
- * ones with the full-state radix select.  Both are exact; tests force either. */
-enum { SV_OPT_SAMPLE_MIN_TERMS = 0 };
+ * ones with the full-state radix select.  Both are exact; tests force either.  The same threshold gates the
+ * output floor of sv_apply_gate_truncate.  SV_OPT_PRE_SLACK (an int64 passed as uint64, default 0): sample
+ * points added to that floor's safety margin; a negative value makes the margin fail so that tests reach the
+ * re-run path. */
+enum { SV_OPT_SAMPLE_MIN_TERMS = 0, SV_OPT_PRE_SLACK = 1 };
 int sv_set_option(sv_state *s, int option, uint64_t value);
 
 /* Statistics of the last call and the launch counter. */

@@ -59,6 +59,12 @@ struct sv_state {
     u64 band_above, band_cand;
     u64 sample_min_terms;   // states with fewer terms use the full-state select
     double mass_est;        // total mass of the current state if known (NaN: unknown); gates are taken as unitary
+    // fused apply + truncate (sv_presample.cu)
+    PreCut* pre;            // device: floor of the running gate, then count / mass of the outputs it left out
+    u64 fuse_K;             // != 0 while sv_apply_gate runs on behalf of sv_apply_gate_truncate: the cap that follows
+    bool pre_valid;         // the current arrays lack pre_cnt outputs of the last gate (all below every stored term)
+    u64 pre_cnt;
+    long long pre_slack;    // SV_OPT_PRE_SLACK: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
 
@@ -97,7 +103,7 @@ int sv_sm_count() {
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 static u64 desc_entries(u64 cap) { return cap / 112 + 8; }
 
-struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, sctl, smp_k[2], smp_v[2], smp_scr, seg_cnt, chunk_cnt, total; };
+struct ArenaLayout { size_t keys[2], amps[2], desc, status, hist, sel, tab, misc, partials, lut, sctl, pre, smp_k[2], smp_v[2], smp_scr, seg_cnt, chunk_cnt, total; };
 static ArenaLayout layout_for(u64 cap) {
     ArenaLayout L; size_t o = 0;
     for (int i = 0; i < 2; ++i) { L.keys[i] = o; o += align_up(cap * 8); }
@@ -111,6 +117,7 @@ static ArenaLayout layout_for(u64 cap) {
     L.partials = o; o += align_up(1024 * 8 + 8);
     L.lut = o; o += align_up(8 * 256 * 8);
     L.sctl = o; o += align_up(sizeof(SampleCtl));
+    L.pre = o; o += align_up(sizeof(PreCut));
     for (int i = 0; i < 2; ++i) { L.smp_k[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 8); }
     for (int i = 0; i < 2; ++i) { L.smp_v[i] = o; o += align_up((size_t)SV_SAMPLE_MAX * 4); }
     L.smp_scr = o; o += align_up(svk_sort_scratch_bytes(SV_SAMPLE_MAX));
@@ -234,6 +241,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->partials = (double*)(s->arena + L.partials);
     s->lut = (u64*)(s->arena + L.lut);
     s->sctl = (SampleCtl*)(s->arena + L.sctl);
+    s->pre = (PreCut*)(s->arena + L.pre);
     for (int i = 0; i < 2; ++i) { s->smp_k[i] = (u64*)(s->arena + L.smp_k[i]); s->smp_v[i] = (u32*)(s->arena + L.smp_v[i]); }
     s->smp_scr = (u32*)(s->arena + L.smp_scr);
     s->seg_cnt = s->arena + L.seg_cnt;
@@ -296,6 +304,7 @@ extern "C" int sv_profile_get(sv_state* s, int kernel, sv_kernel_prof* out) {
 extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
+    if (option == SV_OPT_PRE_SLACK) { s->pre_slack = (long long)value; return SV_OK; }
     return fail(s, SV_ERR_INVALID_ARG, "unknown option");
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
@@ -348,6 +357,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     }
     const int d = 1 << m;
     s->err[0] = 0;
+    s->pre_valid = false;
     s->stats.m = m; s->stats.n_in = s->count; s->stats.n_out = s->count; s->stats.passes = 0;
 
     // a-1: bit j is control-like iff U never connects patterns that differ in bit j
@@ -502,23 +512,53 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.n_out = s->count;
         return SV_OK;
     }
-    prof_slot(s, ma == 1 ? SV_K_BITPASS_GEN : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
-    const int gslot = s->npend - 1;
     const u64 n_live_in = s->count;
-    if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)
-        s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 0,
-                                         s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1);
-    } else {
-        s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
-                                           s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1);
+    // Fused apply + truncate (one active bit): when the cap that follows will cut deep into the gate's output,
+    // a floor for that cut is estimated from a sample of the outputs, and the pass leaves out what lies below it.
+    u64 preM = s->phys / 8;
+    if (preM > SV_SAMPLE_MAX) preM = SV_SAMPLE_MAX;
+    bool use_pre = ma == 1 && s->fuse_K != 0 && s->count >= s->sample_min_terms && s->phys < (1ull << 32) && preM >= 64 &&
+                   2 * s->count > s->fuse_K + s->fuse_K / 8;
+    s->stats.pre_dropped = 0;
+    u64 nout = 0, ndead = 0, npre = 0;
+    for (;;) {
+        u32 pre_parts = 0;
+        if (use_pre) {
+            const u32 M = (u32)preM;
+            s->stats.launches += svk_pre_sample1(s->keys[s->cur], s->amps[s->cur], s->phys, plast > 0 ? plast : 0, s->tab, s->defer, M,
+                                                 s->smp_k[0], s->stream);
+            int in_alt = 0;
+            s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, s->stream, &in_alt);
+            s->stats.launches += svk_pre_pivot(s->smp_k[in_alt ? 1 : 0], M, s->phys, s->fuse_K, s->pre_slack, s->pre, s->stream);
+            DBG_SYNC("pre_sample+pivot");
+        }
+        prof_slot(s, ma == 1 ? SV_K_BITPASS_GEN : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
+        const int gslot = s->npend - 1;
+        if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)
+            double* pmass = reinterpret_cast<double*>(s->hist);          // per-block partials (the select's histogram is idle)
+            u64* pcnt = s->hist + SV_SEL_BINS;
+            s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 0,
+                                             s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1,
+                                             use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts);
+            if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
+        } else {
+            s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
+                                               s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1);
+        }
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        u64 cnts[3] = {0, 0, 0};   // stored outputs, dead ones among them (exact cancellations of a multi-bit gate), left out
+        int rc = read_back(s, cnts, s->d_count, use_pre ? 3 * sizeof(u64) : (ma == 1 ? sizeof(u64) : 2 * sizeof(u64)));
+        if (rc != SV_OK) return rc;
+        nout = cnts[0]; ndead = (ma == 1) ? 0 : cnts[1]; npre = use_pre ? cnts[2] : 0;
+        if (ge0) s->pend[gslot].bytes = 24.0 * ((double)n_live_in + (double)(nout > s->cap ? s->cap : nout));
+        if (use_pre && npre > 0 && nout <= s->fuse_K) {   // the floor was too high (its margin failed): once more without it
+            s->stats.fallbacks += 1;
+            use_pre = false;
+            continue;
+        }
+        break;
     }
-    CHECK_LAUNCH();
-    s->stats.passes += 1;
-    u64 cnts[2] = {0, 0};   // stored outputs, dead ones among them (exact cancellations of a multi-bit gate)
-    int rc = read_back(s, cnts, s->d_count, ma == 1 ? sizeof(u64) : 2 * sizeof(u64));
-    if (rc != SV_OK) return rc;
-    const u64 nout = cnts[0], ndead = (ma == 1) ? 0 : cnts[1];
-    if (ge0) s->pend[gslot].bytes = 24.0 * ((double)n_live_in + (double)(nout > s->cap ? s->cap : nout));
     if (nout > s->cap) {
         s->stats.n_out = nout;
         return fail(s, SV_ERR_CAPACITY, "gate output exceeds capacity (state unchanged)");
@@ -527,8 +567,33 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     s->cur ^= 1;
     s->count = nout - ndead; s->phys = nout;
     s->defer.active = 0;
-    s->stats.n_out = s->count;
+    s->pre_valid = npre > 0; s->pre_cnt = npre;
+    s->stats.n_out = s->count + npre; s->stats.pre_dropped = npre;
     return SV_OK;
+}
+
+// apply the (fused) gate, then truncate.  One call, so that the engine may let the gate's pass
+// leave out what the cut is certain to drop (sv_presample.cu); the result is that of the two calls.
+extern "C" int sv_apply_gate_truncate(sv_state* s, const int* qubits, int m, const sv_c128* U, uint64_t max_terms, double min_mass,
+                                      double* kept_fraction) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    if (!(min_mass > 0.0)) return fail(s, SV_ERR_INVALID_ARG, "min_mass must be > 0");
+    s->fuse_K = max_terms;
+    int rc = sv_apply_gate(s, qubits, m, U);
+    s->fuse_K = 0;
+    if (rc != SV_OK) { s->pre_valid = false; return rc; }
+    const sv_stats g = s->stats;
+    rc = sv_truncate(s, max_terms, min_mass, kept_fraction);
+    s->pre_valid = false;
+    // statistics of the pair: the gate's class and passes, terms before the gate and after the cut
+    const uint64_t n_kept = s->stats.n_out;
+    const int tp = s->stats.passes;
+    const uint64_t launches = s->stats.launches, fallbacks = s->stats.fallbacks;
+    s->stats = g;
+    s->stats.passes += tp; s->stats.launches = launches; s->stats.fallbacks = fallbacks;
+    s->stats.n_mid = g.n_out;
+    if (rc == SV_OK) s->stats.n_out = n_kept;
+    return rc;
 }
 
 // ---------------------------------------------------------------------------------------
@@ -539,7 +604,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
 static int select_levels(sv_state* s, const u64* keys, const double2* amps, u64 n, u64 n_live, u64* lk, bool seeded, u64 max_terms,
                          double min_mass, SelState* out) {
     const KeyMap km = keymap_of(s);
-    if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n_live, max_terms, min_mass, s->stream);
+    if (!seeded) s->stats.launches += svk_sel_init(s->sel, s->hist, n_live, max_terms, min_mass, s->stream, s->pre_valid ? s->pre : nullptr);
     int phase = 0;
     u64 ties = 0;
     {   // The usual course of a select -- exponent level, up to three pattern levels, the tie keys, two key
@@ -607,7 +672,8 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     DBG_SYNC("ss_sample");
     int in_alt = 0;
     s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, st, &in_alt);   // keys are 24-bit pattern prefixes + 1 (< 2^24: finite p)
-    s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st);
+    const PreCut* pre = s->pre_valid ? s->pre : nullptr;   // outputs the gate's pass left out (fused apply + truncate)
+    s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st, pre);
     DBG_SYNC("ss_sort+pivot");
     cudaEvent_t e0, e1;
     prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
@@ -615,7 +681,7 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], want_band ? s->seg_cnt : nullptr, st);
     if (e1) cudaEventRecord(e1, st);
     DBG_SYNC("ss_classify");
-    s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st);
+    s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st, pre);
     DBG_SYNC("sel_seed");
     CHECK_LAUNCH();
     s->stats.passes += 1;
@@ -648,7 +714,7 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     if (!(min_mass > 0.0)) return fail(s, SV_ERR_INVALID_ARG, "min_mass must be > 0");
     s->err[0] = 0;
     s->stats.gate_class = SV_CLASS_NONE; s->stats.m = 0; s->stats.active_bits = 0; s->stats.passes = 0;
-    s->stats.n_in = s->count; s->stats.n_out = s->count;
+    s->stats.n_in = s->count + (s->pre_valid ? s->pre_cnt : 0); s->stats.n_out = s->count;
     if (kept_fraction) *kept_fraction = 1.0;
     const bool needK = max_terms != 0 && max_terms < s->count, needM = min_mass < 1.0;
     if (s->count == 0 || (!needK && !needM)) return SV_OK;

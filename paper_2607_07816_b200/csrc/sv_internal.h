@@ -53,6 +53,7 @@ struct SelState {
     int seeded, pad2_;   // 1: the select runs on the candidates of the sampled fast path (sv_sample_select.cu)
     u64 P_lo;            // seeded: every term outside the candidates and not above them has a pattern < P_lo
     u64 below_cnt;       // seeded: terms certainly below the candidates; a cut that would need them is a band miss (done = 3)
+    double pre_hi, pre_lo;   // mass of the outputs a fused apply+truncate never wrote (PreCut); part of S
 };
 
 // Sampled fast path of the truncation cut (sv_sample_select.cu): pivots and the results of the
@@ -63,6 +64,14 @@ struct SampleCtl {
     int Eref, pad_;
     u64 above_cnt, below_cnt, cand_cnt, overflow;
     u64 tot[2], abv[2];
+};
+
+// Fused apply + truncate (sv_presample.cu): outputs of the gate whose probability pattern is below
+// P_floor are not written by the pass; cnt / mass (double-double) describe what was left out.
+struct PreCut {
+    u64 P_floor;
+    u64 cnt;
+    double mass_hi, mass_lo;
 };
 
 // stored (physical) key -> logical key.  The map is a bit permutation plus the lazy X mask,
@@ -97,9 +106,17 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
 // pair == 0: pure move.  A pending truncation is applied while loading.  Writes the output
 // count to *d_count.
+// pre != nullptr (pair == 1 only): outputs below pre->P_floor are left out; their per-block masses and counts go
+// to pre_mass / pre_cnt[0 .. *pre_parts).
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
-                u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
+                u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr,
+                const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr);
+// fused apply + truncate: pre-sample of a one-bit gate's outputs -> (sort) -> floor; per-block partials -> totals (d_count[2] = count)
+int svk_pre_sample1(const u64* keys, const double2* amps, u64 n, int p, const GateTab* tab, const PendPred& pend, u32 M, u64* smp,
+                    cudaStream_t st);
+int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st);
+int svk_pre_finish(const double* part_mass, const u64* part_cnt, u32 nparts, PreCut* pre, u64* d_count, cudaStream_t st);
 int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
 // Diagonal gate fused with a pending truncation (out of place, compacting).
 int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
@@ -110,7 +127,7 @@ int svk_diag_pend(const u64* keys, double2* amps, u64 n, const GateTab* tab, int
 
 int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaStream_t st);
 
-int svk_sel_init(SelState* ss, u64* hist, u64 n_live, u64 max_terms, double min_mass, cudaStream_t st);
+int svk_sel_init(SelState* ss, u64* hist, u64 n_live, u64 max_terms, double min_mass, cudaStream_t st, const PreCut* pre = nullptr);
 int svk_sel_pass(int mode, const double2* amps, const u64* lkeys, u64 n, const SelState* ss, u64* hist, cudaStream_t st);
 int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
                     cudaStream_t st);
@@ -118,14 +135,15 @@ int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st, int expected_phase = 
 // sampled fast path: sample -> (sort) -> pivots -> classify -> seed the select state
 int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
-                 cudaStream_t st);
+                 cudaStream_t st, const PreCut* pre = nullptr);
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
                     cudaStream_t st);
 // squeeze out the entries below the sampled band (uses the classify pass's per-segment counts)
 int svk_ss_band_compact(const u64* keys, const double2* amps, u64 n, const SampleCtl* ctl, const unsigned char* seg_cnt,
                         u32* chunk_cnt, u64* scan_status, u32* tile_counter, u64* kout, double2* aout, cudaStream_t st);
 int svk_scan_u32(u32* data, u64 n, u64* status, u32* tile_counter, cudaStream_t st);
-int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st);
+int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st,
+                 const PreCut* pre = nullptr);
 int svk_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n,
                 const PendPred& pd, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);
 

@@ -44,12 +44,16 @@
 #define BP_SWA(x) ((x) ^ (((x) >> 3) & 7))
 #define BP_WKN BP_TILE                         // entries of the key / slot work arrays
 #define BP_ROUND BP_TILE                       // outputs staged per round when amplitudes are staged too
-template <int MODE, bool FIXED>
+// PRE (MODE 1 only; fused apply + truncate, sv_presample.cu): outputs whose probability pattern is below
+// pre->P_floor are not written; every block leaves the mass and the number of what it left out in
+// pre_mass / pre_cnt[blockIdx.x] (tiles are taken in a fixed order, so these sums are the same every run).
+template <int MODE, bool FIXED, bool PRE>
 __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
-                                                                u64* d_count, u64 cap, u32 ntiles) {
+                                                                u64* d_count, u64 cap, u32 ntiles, const PreCut* __restrict__ pre,
+                                                                double* __restrict__ pre_mass, u64* __restrict__ pre_cnt) {
     constexpr bool PAIR = (MODE == 1);
     constexpr bool PERM = (MODE == 2);
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -94,6 +98,9 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
     }
     const u64 bit = 1ull << p;
     const u64 himask = (p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
+    const u64 Pf = PRE ? pre->P_floor : 0ull;
+    double dmass = 0.0;     // PRE: mass and number of the outputs this thread left out
+    u32 dcnt = 0;
     u64* gstat = status + ntiles;                       // group statuses follow the tile statuses
     // Persistent blocks (the grid is sized to be fully resident): tile t is taken by block t mod gridDim.x,
     // so a block only ever waits on tiles that resident blocks have taken already.  While a tile is
@@ -314,7 +321,12 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                         cmul_acc(r0, m0, u[1].x, u[1].y, a.x, a.y);
                         cmul_acc(r1, m1, u[3].x, u[3].y, a.x, a.y);
                     }
-                    const u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
+                    u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
+                    if (PRE) {   // below the floor of the cut that follows: never written
+                        const double p0 = prob_of(make_double2(r0, m0)), p1 = prob_of(make_double2(r1, m1));
+                        if (f0 && (u64)__double_as_longlong(p0) < Pf) { f0 = 0; dmass = __dadd_rn(dmass, p0); ++dcnt; }
+                        if (f1 && (u64)__double_as_longlong(p1) < Pf) { f1 = 0; dmass = __dadd_rn(dmass, p1); ++dcnt; }
+                    }
                     ok[v] = nk; o0r[v] = r0; o0i[v] = m0; o1r[v] = r1; o1i[v] = m1;
                     fl |= (f0 | (f1 << 1)) << (2 * v);
                     nout += (int)(f0 + f1);
@@ -367,35 +379,60 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
         }
         __syncthreads();   // A* | B* and this landing buffer are reused
     }
+    if (PRE) {   // block totals, summed in a fixed order (lanes by a fixed tree, warps ascending)
+        __shared__ double s_pm[BP_WARPS];
+        __shared__ u32 s_pc[BP_WARPS];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            dmass = __dadd_rn(dmass, __shfl_xor_sync(0xffffffffu, dmass, d));
+            dcnt += __shfl_xor_sync(0xffffffffu, dcnt, d);
+        }
+        if (lane == 0) { s_pm[warp] = dmass; s_pc[warp] = dcnt; }
+        __syncthreads();
+        if (tid == 0) {
+            double m = 0.0; u64 c = 0;
+            for (int w = 0; w < BP_WARPS; ++w) { m = __dadd_rn(m, s_pm[w]); c += s_pc[w]; }
+            pre_mass[blockIdx.x] = m; pre_cnt[blockIdx.x] = c;
+        }
+    }
 }
 
-template <int MODE, bool FIXED>
-static void launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
-                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
+template <int MODE, bool FIXED, bool PRE>
+static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
+                          const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
+                          const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
     const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2);   // amplitudes x 2, landing keys, A* | B* keys, slots
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
     if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<MODE, FIXED>, SV_THREADS, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<MODE, FIXED, PRE>, SV_THREADS, smem);
         if (per_sm < 1) per_sm = 1;
     }
     const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    bitpass_kernel<MODE, FIXED><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles);
+    bitpass_kernel<MODE, FIXED, PRE><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles,
+                                                                     pre, pre_mass, pre_cnt);
+    return grid;
 }
 
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
-                u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
+                u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1, const PreCut* pre, double* pre_mass,
+                u64* pre_cnt, u32* pre_parts) {
     (void)tile_counter;
+    if (pre_parts) *pre_parts = 0;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
     const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
     if (!(pair == 2 || (!pair && fixed)))   // the position-preserving variants have no scan
         cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
     int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
-#define SV_BP(P_, F_) launch_bitpass<P_, F_>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st)
+#define SV_BP(P_, F_) launch_bitpass<P_, F_, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st)
     if (pair == 2) SV_BP(2, true);                       // monomial blocks: always position preserving
+    else if (pair && pre) {
+        const u32 g = launch_bitpass<1, false, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt);
+        if (pre_parts) *pre_parts = g;
+    }
     else if (pair) SV_BP(1, false);
     else { if (fixed) SV_BP(0, true); else SV_BP(0, false); }
 #undef SV_BP

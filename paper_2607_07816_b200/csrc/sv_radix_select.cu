@@ -90,7 +90,7 @@ __device__ __forceinline__ u64 top_bits(u64 diff, int k) {   // the k most signi
     return m;
 }
 
-__global__ void sel_init_kernel(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass) {
+__global__ void sel_init_kernel(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass, const PreCut* pre) {
     for (int i = threadIdx.x; i < H_TOTAL; i += blockDim.x)
         hist[i] = ((i >= H_AND && i < H_OR) || i == H_EXT + 1) ? ~0ull : 0ull;
     if (threadIdx.x == 0) {
@@ -102,11 +102,12 @@ __global__ void sel_init_kernel(SelState* ss, u64* hist, u64 n, u64 max_terms, d
         s.mass_active = (min_mass < 1.0) ? 1 : 0;
         s.min_mass = min_mass;
         s.cand_count = n;
+        if (pre) { s.pre_hi = pre->mass_hi; s.pre_lo = pre->mass_lo; }   // left out by a fused apply + truncate: part of S
         *ss = s;
     }
 }
-int svk_sel_init(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass, cudaStream_t st) {
-    sel_init_kernel<<<1, SV_THREADS, 0, st>>>(ss, hist, n, max_terms, min_mass);
+int svk_sel_init(SelState* ss, u64* hist, u64 n, u64 max_terms, double min_mass, cudaStream_t st, const PreCut* pre) {
+    sel_init_kernel<<<1, SV_THREADS, 0, st>>>(ss, hist, n, max_terms, min_mass, pre);
     return 1;
 }
 
@@ -282,7 +283,8 @@ __device__ __forceinline__ dd dd_from_fx(const u64* lohi, int Eref) {
     const dd v = dd_add(dd_scale2(dd_from_u64(lohi[1]), 64), dd_from_u64(lohi[0]));
     return dd_scale2(v, Eref - 1075 - 41);
 }
-__global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass) {
+__global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass,
+                                const PreCut* pre) {
     for (int i = threadIdx.x; i < H_TOTAL; i += blockDim.x)
         hist[i] = ((i >= H_AND && i < H_OR) || i == H_EXT + 1) ? ~0ull : 0ull;
     if (threadIdx.x != 0) return;
@@ -295,7 +297,14 @@ __global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u
     s.below_cnt = c.below_cnt;
     s.P_lo = c.P_lo;
     s.min_mass = min_mass;
-    const dd tot = dd_from_fx(c.tot, c.Eref), abv = dd_from_fx(c.abv, c.Eref);
+    dd tot = dd_from_fx(c.tot, c.Eref);
+    const dd abv = dd_from_fx(c.abv, c.Eref);
+    if (pre) {   // outputs a fused apply + truncate never wrote: below every stored term, part of S
+        dd pm; pm.hi = pre->mass_hi; pm.lo = pre->mass_lo;
+        tot = dd_add(tot, pm);
+        s.pre_hi = pm.hi; s.pre_lo = pm.lo;
+        s.below_cnt += pre->cnt;
+    }
     s.total_hi = tot.hi; s.total_lo = tot.lo;
     s.kept_hi = abv.hi; s.kept_lo = abv.lo;
     s.kept_count = c.above_cnt;
@@ -313,8 +322,9 @@ __global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u
     if (miss) s.done = 3;
     *ss = s;
 }
-int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st) {
-    sel_seed_kernel<<<1, SV_THREADS, 0, st>>>(ss, hist, ctl, n_orig, max_terms, min_mass);
+int svk_sel_seed(SelState* ss, u64* hist, const SampleCtl* ctl, u64 n_orig, u64 max_terms, double min_mass, cudaStream_t st,
+                 const PreCut* pre) {
+    sel_seed_kernel<<<1, SV_THREADS, 0, st>>>(ss, hist, ctl, n_orig, max_terms, min_mass, pre);
     return 1;
 }
 
@@ -371,6 +381,7 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
             dd tot = dd_make(0.0);
             for (int t = 0; t < SV_THREADS; ++t)
                 if (sgc[t]) { dd x; x.hi = sgh[t]; x.lo = sgl[t]; tot = dd_add(tot, x); }
+            { dd pm; pm.hi = s.pre_hi; pm.lo = s.pre_lo; tot = dd_add(tot, pm); }
             s.total_hi = tot.hi; s.total_lo = tot.lo;
             rem = dd_make(__dmul_rn(s.min_mass, tot.hi));
         }

@@ -50,7 +50,8 @@ __device__ __forceinline__ double smp_prob(u64 top) {   // mid-point of the valu
 // the live ones hold (top 32 pattern bits) + 1.  Warp w owns a contiguous range of the live part
 // and walks it 32 elements at a time.
 __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ smp, u32 M, u64 n_live, u64 max_terms,
-                                                        double min_mass, double mass_est, SampleCtl* __restrict__ ctl) {
+                                                        double min_mass, double mass_est, SampleCtl* __restrict__ ctl,
+                                                        const PreCut* __restrict__ precut) {
     __shared__ double wsum[32];
     __shared__ u32 cnt[2][3];   // [sweep][threshold]
     __shared__ u32 s_z;
@@ -79,8 +80,10 @@ __global__ void __launch_bounds__(1024) ss_pivot_kernel(const u64* __restrict__ 
     // mass to drop, in sample units (the tail is made of small terms, so the scaled sample tail
     // estimates it well even when a few heavy terms carry most of S)
     const double per_sample = (double)n_live / (double)max(Ml, 1u);
-    const double S_est = (mass_est == mass_est && mass_est > 0.0) ? mass_est : T * per_sample;
-    const double X0 = (1.0 - min_mass) * S_est / per_sample;
+    // a fused apply + truncate has left D_pre of the mass out already (all of it below every stored term)
+    const double D_pre = precut ? precut->mass_hi : 0.0;
+    const double S_est = (mass_est == mass_est && mass_est > 0.0) ? mass_est : T * per_sample + D_pre;
+    const double X0 = fmax(0.0, (1.0 - min_mass) * S_est - D_pre) / per_sample;
     // sweep 1: a0 = sample elements in the nominal tail; sweep 2: the band X0 / (1 + eps) .. X0 * (1 + eps)
     // with eps ~ 10 / sqrt(a0) (the relative noise of a tail sum of a0 sampled terms)
     double X[3] = {X0, X0, X0};
@@ -263,8 +266,8 @@ int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st) 
     return 1;
 }
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
-                 cudaStream_t st) {
-    ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n_live, max_terms, min_mass, mass_est, ctl);
+                 cudaStream_t st, const PreCut* pre) {
+    ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n_live, max_terms, min_mass, mass_est, ctl, pre);
     return 1;
 }
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,

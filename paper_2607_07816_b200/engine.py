@@ -18,14 +18,17 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
-           "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option"]
+           "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
+           "sv_apply_gate_truncate"]
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
+OPT_PRE_SLACK = 1
 
 
 class SvStats(C.Structure):
     _fields_ = [("gate_class", C.c_int), ("m", C.c_int), ("active_bits", C.c_int), ("passes", C.c_int),
-                ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64), ("fallbacks", C.c_uint64)]
+                ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64), ("fallbacks", C.c_uint64),
+                ("n_mid", C.c_uint64), ("pre_dropped", C.c_uint64)]
 
 
 class SvKernelProf(C.Structure):
@@ -56,6 +59,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_apply_gate.argtypes = [vp, vp, i32, vp]
     lib.sv_truncate.restype = i32
     lib.sv_truncate.argtypes = [vp, u64, dbl, C.POINTER(dbl)]
+    lib.sv_apply_gate_truncate.restype = i32
+    lib.sv_apply_gate_truncate.argtypes = [vp, vp, i32, vp, u64, dbl, C.POINTER(dbl)]
     lib.sv_norm.restype = i32
     lib.sv_norm.argtypes = [vp, C.POINTER(dbl)]
     lib.sv_top.restype = i32
@@ -133,6 +138,17 @@ class SparseSV:
             raise ValueError("U must be 2^m x 2^m")
         self._chk(lib.sv_apply_gate(self._h, q.ctypes.data, int(q.size), U.ctypes.data))
 
+    def apply_gate_truncate(self, qubits, U, max_terms: int = 0, min_mass: float = 1.0) -> float:
+        """apply_gate followed by truncate in one call (same result; the engine may skip writing what the cut drops)."""
+        q = np.ascontiguousarray(qubits, dtype=np.int32)
+        U = np.ascontiguousarray(U, dtype=np.complex128)
+        if U.shape != (1 << q.size, 1 << q.size):
+            raise ValueError("U must be 2^m x 2^m")
+        kept = C.c_double(1.0)
+        self._chk(lib.sv_apply_gate_truncate(self._h, q.ctypes.data, int(q.size), U.ctypes.data, int(max_terms), float(min_mass),
+                                             C.byref(kept)))
+        return kept.value
+
     def truncate(self, max_terms: int = 0, min_mass: float = 1.0) -> float:
         kept = C.c_double(1.0)
         self._chk(lib.sv_truncate(self._h, int(max_terms), float(min_mass), C.byref(kept)))
@@ -181,7 +197,7 @@ class SparseSV:
         self._chk(lib.sv_get_stats(self._h, C.byref(st)))
         return {"class": CLASS_NAMES.get(st.gate_class, "?"), "m": st.m, "active_bits": st.active_bits,
                 "passes": st.passes, "n_in": int(st.n_in), "n_out": int(st.n_out), "launches": int(st.launches),
-                "fallbacks": int(st.fallbacks)}
+                "fallbacks": int(st.fallbacks), "n_mid": int(st.n_mid), "pre_dropped": int(st.pre_dropped)}
 
     def set_option(self, option: int, value: int):
         self._chk(lib.sv_set_option(self._h, int(option), int(value)))
