@@ -38,6 +38,8 @@ def parse_args():
     ap.add_argument("--k-log2", type=int, default=28, help="log2 of the hard cap K (28 = the config's own)")
     ap.add_argument("--gates-per-step", type=int, default=32)
     ap.add_argument("--cap-mult", type=int, default=8, help="capacity = cap-mult * K (8 = worst case of an 8x8 gate)")
+    ap.add_argument("--two-call", action="store_true",
+                    help="time sv_apply_gate + sv_truncate instead of the fused sv_apply_gate_truncate")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -173,11 +175,12 @@ def run_circuits(engine, W, dev, torch):
             log_kept, peak_terms = 0.0, 1
             try:
                 for g in c.gates:
-                    sv.apply_gate(g.qubits, g.U)
                     if c.truncate_every_gate:
-                        peak_terms = max(peak_terms, sv.stats()["n_out"])
-                        kept = sv.truncate(c.max_terms, c.min_mass)
+                        kept = sv.apply_gate_truncate(g.qubits, g.U, c.max_terms, c.min_mass)
+                        peak_terms = max(peak_terms, sv.stats()["n_mid"])
                         log_kept += float(np.log(kept))
+                    else:
+                        sv.apply_gate(g.qubits, g.U)
                 b.record(); torch.cuda.synchronize()
                 k, _, p = sv.top(1)
                 res = {"n_qubits": c.n, "gates": len(c.gates), "wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(),
@@ -221,10 +224,13 @@ def run_ours(args):
         sv.apply_gate(g.qubits, g.U); sv.truncate(c.max_terms, c.min_mass)
     ramp_gates = gi
 
-    per_gate = []   # (klass, name, n_in, n_pre, n_kept, passes, e_a0, e_a1, e_t1)
+    per_gate = []   # (klass, name, n_in, n_pre, n_kept, passes, e_a0, e_a1 (None: fused call), e_t1)
+    fused_default = not args.two_call
 
-    def one_step(record):
+    def one_step(record, fused=None, sink=None):
         nonlocal gi
+        fused = fused_default if fused is None else fused
+        sink = per_gate if sink is None else sink
         nt = 0
         for _ in range(G):
             g = c.gates[gi % len(c.gates)]; gi += 1
@@ -232,13 +238,20 @@ def run_ours(args):
             if record:
                 e0, e1, e2 = ev(), ev(), ev()
                 e0.record()
-            sv.apply_gate(g.qubits, g.U)
-            if record:
-                st = sv.stats(); e1.record()
-            sv.truncate(c.max_terms, c.min_mass)
-            if record:
-                e2.record()
-                per_gate.append((g.klass, g.name, n_in, st["n_out"], sv.stats()["n_out"], st["passes"], e0, e1, e2))
+            if fused:
+                sv.apply_gate_truncate(g.qubits, g.U, c.max_terms, c.min_mass)
+                if record:
+                    e2.record()
+                    st = sv.stats()
+                    sink.append((g.klass, g.name, n_in, st["n_mid"], st["n_out"], st["passes"], e0, None, e2))
+            else:
+                sv.apply_gate(g.qubits, g.U)
+                if record:
+                    st = sv.stats(); e1.record()
+                sv.truncate(c.max_terms, c.min_mass)
+                if record:
+                    e2.record()
+                    sink.append((g.klass, g.name, n_in, st["n_out"], sv.stats()["n_out"], st["passes"], e0, e1, e2))
             nt += n_in
         return nt
 
@@ -265,24 +278,48 @@ def run_ours(args):
 
     # ---- per gate class summary (rank 0) ----
     hbm, peak_kind = peaks()
-    classes = {}
-    for (kl, name, n_in, n_pre, n_kept, passes, e0, e1, e2) in per_gate:
-        ta, tt = e0.elapsed_time(e1), e1.elapsed_time(e2)
-        d = classes.setdefault(kl, {"gates": 0, "n_in": 0, "apply_ms": 0.0, "trunc_ms": 0.0, "apply_bytes": 0.0, "trunc_bytes": 0.0, "passes": 0})
-        d["gates"] += 1; d["n_in"] += n_in; d["apply_ms"] += ta; d["trunc_ms"] += tt; d["passes"] += passes
-        d["apply_bytes"] += 24.0 * (n_in + n_pre); d["trunc_bytes"] += 24.0 * (n_pre + n_kept)
-        if log:
-            log.write(json.dumps({"class": kl, "gate": name, "n_in": n_in, "n_pre": n_pre, "n_kept": n_kept, "passes": passes,
-                                  "apply_ms": ta, "trunc_ms": tt}) + "\n")
-    per_class = {}
-    for kl, d in classes.items():
-        per_class[kl] = {
-            "gates": d["gates"], "mean_passes": d["passes"] / d["gates"],
-            "apply_terms_per_s": d["n_in"] / (d["apply_ms"] * 1e-3) if d["apply_ms"] > 0 else None,
-            "apply_roofline_frac_of_8TBs": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / 8.0e12 if d["apply_ms"] > 0 else None,
-            "apply_roofline_frac_of_measured": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / (hbm * 1e9) if d["apply_ms"] > 0 else None,
-            "trunc_roofline_frac_of_measured": d["trunc_bytes"] / (d["trunc_ms"] * 1e-3) / (hbm * 1e9) if d["trunc_ms"] > 0 else None,
-            "apply_ms_mean": d["apply_ms"] / d["gates"], "trunc_ms_mean": d["trunc_ms"] / d["gates"]}
+
+    def summarise(records, logf):
+        classes = {}
+        for (kl, name, n_in, n_pre, n_kept, passes, e0, e1, e2) in records:
+            total = e0.elapsed_time(e2)
+            ta, tt = (e0.elapsed_time(e1), e1.elapsed_time(e2)) if e1 is not None else (None, None)
+            d = classes.setdefault(kl, {"gates": 0, "n_in": 0, "ms": 0.0, "apply_ms": 0.0, "trunc_ms": 0.0, "apply_bytes": 0.0,
+                                        "trunc_bytes": 0.0, "passes": 0, "split": True})
+            d["gates"] += 1; d["n_in"] += n_in; d["ms"] += total; d["passes"] += passes
+            d["apply_bytes"] += 24.0 * (n_in + n_pre); d["trunc_bytes"] += 24.0 * (n_pre + n_kept)
+            if ta is None:
+                d["split"] = False
+            else:
+                d["apply_ms"] += ta; d["trunc_ms"] += tt
+            if logf:
+                logf.write(json.dumps({"class": kl, "gate": name, "n_in": n_in, "n_pre": n_pre, "n_kept": n_kept, "passes": passes,
+                                       "ms": total, "apply_ms": ta, "trunc_ms": tt}) + "\n")
+        out = {}
+        for kl, d in classes.items():
+            o = {"gates": d["gates"], "mean_passes": d["passes"] / d["gates"], "ms_mean": d["ms"] / d["gates"],
+                 "terms_per_s": d["n_in"] / (d["ms"] * 1e-3) if d["ms"] > 0 else None}
+            if d["split"] and d["apply_ms"] > 0:
+                o.update({
+                    "apply_terms_per_s": d["n_in"] / (d["apply_ms"] * 1e-3),
+                    "apply_roofline_frac_of_8TBs": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / 8.0e12,
+                    "apply_roofline_frac_of_measured": d["apply_bytes"] / (d["apply_ms"] * 1e-3) / (hbm * 1e9),
+                    "trunc_roofline_frac_of_measured": d["trunc_bytes"] / (d["trunc_ms"] * 1e-3) / (hbm * 1e9) if d["trunc_ms"] > 0 else None,
+                    "apply_ms_mean": d["apply_ms"] / d["gates"], "trunc_ms_mean": d["trunc_ms"] / d["gates"]})
+            out[kl] = o
+        return out
+
+    per_class = summarise(per_gate, log)
+    # the same gates through the two separate calls, after the timed region: the apply / truncate split per class
+    per_class_two_call = None
+    if fused_default:
+        two = []
+        g_keep = gi
+        for _ in range(min(args.steps, 3)):
+            one_step(True, fused=False, sink=two)
+        torch.cuda.synchronize()
+        gi = g_keep
+        per_class_two_call = summarise(two, None)
 
     dom = max(prof, key=lambda k: prof[k]["ms"])
     dk = prof[dom]
@@ -332,7 +369,7 @@ def run_ours(args):
         et, em = dist.aggregate(e_terms, e_ms, dev)
         e2e = {"value": et / (em * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(hk_p.nbytes + ha_p.nbytes + G * 16 * 64),
                "d2h_bytes_per_step": d2h, "steps": e_steps,
-               "note": "sv_load(host pinned state) + %d x (sv_apply_gate + sv_truncate) + sv_top(16); same gates every step" % G}
+               "note": "sv_load(host pinned state) + %d x (the same call as the timed region) + sv_top(16); same gates every step" % G}
 
     # ---- circuit wall times of BASELINE.json configs[0..4] at their full sizes (reported, not the headline) ----
     circuits = None
@@ -351,11 +388,12 @@ def run_ours(args):
                 "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": "cfg5", "n_qubits": c.n, "K_log2": args.k_log2, "min_mass": c.min_mass,
-                           "gates_per_step": G, "capacity_terms": cap_mult * K, "ramp_gates": ramp_gates,
+                           "gates_per_step": G, "call": "sv_apply_gate + sv_truncate" if args.two_call else "sv_apply_gate_truncate",
+                           "capacity_terms": cap_mult * K, "ramp_gates": ramp_gates,
                            "l2": "inputs larger than L2 (state %.2f GB)" % (24.0 * K / 1e9),
                            "parallelism": "replicas x%d" % world},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
-                "per_class": per_class, "circuit_ms_per_gate": max_ms / (args.steps * G), "circuits": circuits}
+                "per_class": per_class, "per_class_two_call": per_class_two_call, "circuit_ms_per_gate": max_ms / (args.steps * G), "circuits": circuits}
         print(json.dumps(line), flush=True)
     if log:
         log.close()

@@ -64,6 +64,9 @@ struct sv_state {
     u64 fuse_K;             // != 0 while sv_apply_gate runs on behalf of sv_apply_gate_truncate: the cap that follows
     bool pre_valid;         // the current arrays lack pre_cnt outputs of the last gate (all below every stored term)
     u64 pre_cnt;
+    bool fuse_on;           // sv_apply_gate runs on behalf of sv_apply_gate_truncate
+    bool diag_deferred;     // the diagonal gate in s->tab (and the pending cut) has not been applied yet: the truncation's
+                            // classification pass applies it in place (sv_sample_select.cu, XF)
     long long pre_slack;    // SV_OPT_PRE_SLACK: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
@@ -341,6 +344,27 @@ static int materialize(sv_state* s) {
 // Dead entries (terms dropped in place) are tolerated up to 1/8 of the live terms.
 static inline bool few_dead(const sv_state* s) { return s->phys - s->count <= s->count / 8; }
 
+// In-place diagonal gate from s->tab, fused with a pending truncation if there is one (few dead entries).
+static int launch_diag_in_place(sv_state* s) {
+    cudaEvent_t e0, e1;
+    prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &e0, &e1);
+    if (e0) cudaEventRecord(e0, s->stream);
+    if (s->defer.active) {   // dropped terms become dead entries
+        s->stats.launches += svk_diag_pend(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, 1, s->defer, s->stream);
+        s->defer.active = 0;
+    } else {
+        s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, s->stream);
+    }
+    if (e1) cudaEventRecord(e1, s->stream);
+    CHECK_LAUNCH();
+    return SV_OK;
+}
+static int flush_diag(sv_state* s) {
+    if (!s->diag_deferred) return SV_OK;
+    s->diag_deferred = false;
+    return launch_diag_in_place(s);
+}
+
 // ---------------------------------------------------------------------------------------
 // sv_apply_gate: classify (row a-1), plan the bit moves, launch
 // ---------------------------------------------------------------------------------------
@@ -415,17 +439,12 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
                                                       s->tab, s->defer, s->status, s->tile_counter, s->d_count, s->stream);
                 if (e1) cudaEventRecord(e1, s->stream);
                 s->cur = alt; s->phys = s->count; s->defer.active = 0;
-            } else if (s->defer.active) {            // in place: dropped terms become dead entries
-                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &e0, &e1);
-                if (e0) cudaEventRecord(e0, s->stream);
-                s->stats.launches += svk_diag_pend(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, 1, s->defer, s->stream);
-                if (e1) cudaEventRecord(e1, s->stream);
-                s->defer.active = 0;
+            } else if (s->fuse_on && s->count >= s->sample_min_terms && s->phys / 8 >= 64) {
+                // fused call: the sampled truncation that follows applies the gate in its own pass over the state
+                s->diag_deferred = true;
             } else {
-                prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &e0, &e1);
-                if (e0) cudaEventRecord(e0, s->stream);
-                s->stats.launches += svk_diag(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, s->stream);
-                if (e1) cudaEventRecord(e1, s->stream);
+                int rcd = launch_diag_in_place(s);
+                if (rcd != SV_OK) return rcd;
             }
             CHECK_LAUNCH();
             s->stats.passes = 1;
@@ -578,13 +597,18 @@ extern "C" int sv_apply_gate_truncate(sv_state* s, const int* qubits, int m, con
                                       double* kept_fraction) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (!(min_mass > 0.0)) return fail(s, SV_ERR_INVALID_ARG, "min_mass must be > 0");
-    s->fuse_K = max_terms;
+    s->fuse_K = max_terms; s->fuse_on = true;
     int rc = sv_apply_gate(s, qubits, m, U);
-    s->fuse_K = 0;
-    if (rc != SV_OK) { s->pre_valid = false; return rc; }
+    s->fuse_K = 0; s->fuse_on = false;
+    if (rc != SV_OK) { s->pre_valid = false; s->diag_deferred = false; return rc; }
     const sv_stats g = s->stats;
+    if (s->diag_deferred && !((max_terms != 0 && max_terms < s->count) || min_mass < 1.0)) {   // the truncation will not look at the state
+        rc = flush_diag(s);
+        if (rc != SV_OK) return rc;
+    }
     rc = sv_truncate(s, max_terms, min_mass, kept_fraction);
     s->pre_valid = false;
+    if (s->diag_deferred) { const int rcf = flush_diag(s); if (rc == SV_OK) rc = rcf; }
     // statistics of the pair: the gate's class and passes, terms before the gate and after the cut
     const uint64_t n_kept = s->stats.n_out;
     const int tp = s->stats.passes;
@@ -668,7 +692,10 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     if (m64 < 64) return SV_OK;
     const u32 M = (u32)m64;
     cudaStream_t st = s->stream;
-    s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st);
+    // fused diagonal gate + truncate: the gate (and the pending cut) is applied by the classification pass
+    const bool xf = s->diag_deferred;
+    const PendPred xpd = s->defer;
+    s->stats.launches += svk_ss_sample(s->amps[s->cur], n, M, s->smp_k[0], st, s->keys[s->cur], &xpd, xf ? s->tab : nullptr);
     DBG_SYNC("ss_sample");
     int in_alt = 0;
     s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, st, &in_alt);   // keys are 24-bit pattern prefixes + 1 (< 2^24: finite p)
@@ -676,10 +703,12 @@ static int run_select_sampled(sv_state* s, u64 max_terms, double min_mass, SelSt
     s->stats.launches += svk_ss_pivot(s->smp_k[in_alt ? 1 : 0], M, n_live, max_terms, min_mass, s->mass_est, s->sctl, st, pre);
     DBG_SYNC("ss_sort+pivot");
     cudaEvent_t e0, e1;
-    prof_slot(s, SV_K_CLASSIFY, 16.0 * (double)n, &e0, &e1);
+    prof_slot(s, SV_K_CLASSIFY, (xf ? 40.0 : 16.0) * (double)n, &e0, &e1);
     if (e0) cudaEventRecord(e0, st);
-    s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], want_band ? s->seg_cnt : nullptr, st);
+    s->stats.launches += svk_ss_classify(s->keys[s->cur], s->amps[s->cur], n, s->sctl, s->keys[alt], s->amps[alt], want_band ? s->seg_cnt : nullptr, st,
+                                         s->amps[s->cur], &xpd, xf ? s->tab : nullptr);
     if (e1) cudaEventRecord(e1, st);
+    if (xf) { s->diag_deferred = false; s->defer.active = 0; }   // applied in place: dropped terms are dead entries now
     DBG_SYNC("ss_classify");
     s->stats.launches += svk_sel_seed(s->sel, s->hist, s->sctl, n_live, max_terms, min_mass, st, pre);
     DBG_SYNC("sel_seed");
@@ -705,6 +734,7 @@ static int run_select(sv_state* s, u64 max_terms, double min_mass, SelState* out
         if (rc != SV_OK || used) return rc;
         s->stats.fallbacks += 1;
     }
+    { int rcd = flush_diag(s); if (rcd != SV_OK) return rcd; }   // (a deferred diagonal gate the sampled path did not get to)
     // full-state select; the idle buffer holds the extracted tie keys
     return select_levels(s, s->keys[s->cur], s->amps[s->cur], n, s->count, s->keys[s->cur ^ 1], false, max_terms, min_mass, out);
 }
@@ -719,7 +749,7 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     const bool needK = max_terms != 0 && max_terms < s->count, needM = min_mass < 1.0;
     if (s->count == 0 || (!needK && !needM)) return SV_OK;
     int rc = SV_OK;
-    if (s->defer.active) rc = materialize(s);   // a second truncation in a row: apply the first one now
+    if (s->defer.active && !s->diag_deferred) rc = materialize(s);   // a second truncation in a row: apply the first one now
     if (rc != SV_OK) return rc;
     if (dbg_sync_on()) { DBG_SYNC("before select"); fprintf(stderr, "[sv debug] truncate: count=%llu phys=%llu cap=%llu cur=%d defer=%d\n", (unsigned long long)s->count, (unsigned long long)s->phys, (unsigned long long)s->cap, s->cur, s->defer.active); }
     SelState ss;

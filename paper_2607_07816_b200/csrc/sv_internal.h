@@ -133,11 +133,14 @@ int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState*
                     cudaStream_t st);
 int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st, int expected_phase = -1);
 // sampled fast path: sample -> (sort) -> pivots -> classify -> seed the select state
-int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st);
+// xf_tab != nullptr (fused diagonal gate + truncate): the diagonal gate in xf_tab and the pending cut *pd are applied on the fly
+// (sample) / in place through amps_rw (classify) before the amplitude is looked at.
+int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st, const u64* keys = nullptr, const PendPred* pd = nullptr,
+                  const GateTab* xf_tab = nullptr);
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
                  cudaStream_t st, const PreCut* pre = nullptr);
 int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
-                    cudaStream_t st);
+                    cudaStream_t st, double2* amps_rw = nullptr, const PendPred* pd = nullptr, const GateTab* xf_tab = nullptr);
 // squeeze out the entries below the sampled band (uses the classify pass's per-segment counts)
 int svk_ss_band_compact(const u64* keys, const double2* amps, u64 n, const SampleCtl* ctl, const unsigned char* seg_cnt,
                         u32* chunk_cnt, u64* scan_status, u32* tile_counter, u64* kout, double2* aout, cudaStream_t st);

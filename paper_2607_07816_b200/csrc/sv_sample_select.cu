@@ -24,7 +24,7 @@
 // Exact masses (D3): p is converted to a 128-bit fixed-point integer relative to
 // a reference exponent, and integers are added -- the sums do not depend on the order in
 // which threads or blocks add them.
-#include "sv_device.cuh"
+#include "sv_tile.cuh"
 
 typedef unsigned __int128 u128;
 
@@ -32,12 +32,34 @@ typedef unsigned __int128 u128;
 // relative resolution, far finer than the statistical margins of the pivots): three 8-bit sort passes.
 #define SS_DROP 40
 
-__global__ void __launch_bounds__(SV_THREADS) ss_sample_kernel(const double2* __restrict__ amps, u64 n, u32 M,
-                                                               u64* __restrict__ smp) {
+// XF (fused diagonal gate + truncate, sv_apply_gate_truncate): the diagonal gate that precedes the truncation
+// has NOT been applied yet.  The sample and the classification pass see every amplitude as that gate leaves
+// it -- pending cut (dropped -> dead entry 0+0i), renormalisation, phase, exactly the arithmetic of
+// diag_kernel / diag_pend_kernel -- and the classification pass writes it back in place: the gate and the
+// truncation's pass over the state are ONE pass (key read, amplitude read + write: 40 B per term).
+__device__ __forceinline__ double2 xf_amp(double2 a, u64 k, const PendPred& pd, const double2* sd, const int* cpos, int mc) {
+    if (pd.active) {
+        if (a.x == 0.0 && a.y == 0.0) return a;                       // dead stays dead
+        if (!pend_keep(pd, k, a)) return make_double2(0.0, 0.0);
+        a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale);
+    }
+    int cx = 0;
+    for (int j = 0; j < mc; ++j) cx |= (int)((k >> cpos[j]) & 1ull) << j;
+    const double2 u = sd[cx];
+    double2 o;
+    o.x = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
+    o.y = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
+    return o;
+}
+
+template <bool XF>
+__global__ void __launch_bounds__(SV_THREADS) ss_sample_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps, u64 n, u32 M,
+                                                               u64* __restrict__ smp, PendPred pd, const GateTab* __restrict__ gtab) {
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= M) return;
     const u64 i = (u64)(((u128)j * n) / M);
-    const double2 a = ld_stream_d2(amps + i);
+    double2 a = ld_stream_d2(amps + i);
+    if (XF) a = xf_amp(a, keys[i], pd, gtab->U, gtab->ctrl_pos, gtab->mc);
     // dead entries (0+0i) sort to the front as key 0; live terms get their pattern's top 24 bits + 1
     smp[j] = (a.x == 0.0 && a.y == 0.0) ? 0ull : (((u64)__double_as_longlong(prob_of(a)) >> SS_DROP) + 1ull);
 }
@@ -183,11 +205,22 @@ __device__ __forceinline__ void atomic_add_u128(u64* lohi, u128 v) {   // lohi[0
 // Candidates are rare (a few per cent) but almost every warp meets one every few iterations.  They
 // are parked in a warp-private shared-memory buffer (amplitude + index) and flushed 64+ at a
 // time: one global atomic and one batch of key loads per flush instead of one per iteration.
+template <bool XF>
 __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
                                                                  u64 n, SampleCtl* __restrict__ ctl, u64* __restrict__ ckeys,
-                                                                 double2* __restrict__ camps, unsigned char* __restrict__ seg_cnt) {
+                                                                 double2* __restrict__ camps, unsigned char* __restrict__ seg_cnt,
+                                                                 double2* amps_rw, PendPred pd, const GateTab* __restrict__ gtab) {
     __shared__ double2 s_ba[SV_THREADS / 32][SC_WBUF];
     __shared__ u64 s_bi[SV_THREADS / 32][SC_WBUF];
+    __shared__ double2 sd[16];
+    __shared__ int s_cpos[SV_MAX_M], s_mc;
+    if (XF) {
+        if (threadIdx.x < 16) sd[threadIdx.x] = gtab->U[threadIdx.x];
+        if (threadIdx.x < SV_MAX_M) s_cpos[threadIdx.x] = gtab->ctrl_pos[threadIdx.x];
+        if (threadIdx.x == 0) s_mc = gtab->mc;
+        __syncthreads();
+    }
+    const int mc = XF ? s_mc : 0;
     const u64 P_hi = ctl->P_hi, P_lo = ctl->P_lo;
     const int Eref = ctl->Eref;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -211,10 +244,26 @@ __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __re
     const u64 nchunks = (n + chunk - 1) / chunk;
     for (u64 c = blockIdx.x; c < nchunks; c += gridDim.x) {
         double2 a[SC_IT];
+        u64 kx[XF ? SC_IT : 1];
 #pragma unroll
         for (int r = 0; r < SC_IT; ++r) {
             const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
-            a[r] = (i < n) ? ld_stream_d2(amps + i) : make_double2(0.0, 0.0);
+            if (XF) {
+                a[r] = (i < n) ? amps_rw[i] : make_double2(0.0, 0.0);
+                kx[r] = (i < n) ? ld_stream_u64(keys + i) : 0ull;
+            } else {
+                a[r] = (i < n) ? ld_stream_d2(amps + i) : make_double2(0.0, 0.0);
+            }
+        }
+        if (XF) {
+#pragma unroll
+            for (int r = 0; r < SC_IT; ++r) {
+                const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+                if (i < n && !(pd.active && a[r].x == 0.0 && a[r].y == 0.0)) {   // (a dead entry is not rewritten)
+                    a[r] = xf_amp(a[r], kx[r], pd, sd, s_cpos, mc);
+                    amps_rw[i] = a[r];
+                }
+            }
         }
 #pragma unroll
         for (int r = 0; r < SC_IT; ++r) {
@@ -261,8 +310,9 @@ __global__ void __launch_bounds__(SV_THREADS) ss_classify_kernel(const u64* __re
     }
 }
 
-int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st) {
-    ss_sample_kernel<<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(amps, n, M, smp);
+int svk_ss_sample(const double2* amps, u64 n, u32 M, u64* smp, cudaStream_t st, const u64* keys, const PendPred* pd, const GateTab* xf_tab) {
+    if (xf_tab) ss_sample_kernel<true><<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(keys, amps, n, M, smp, *pd, xf_tab);
+    else ss_sample_kernel<false><<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(nullptr, amps, n, M, smp, PendPred{}, nullptr);
     return 1;
 }
 int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double min_mass, double mass_est, SampleCtl* ctl,
@@ -270,17 +320,23 @@ int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double
     ss_pivot_kernel<<<1, 1024, 0, st>>>(smp_sorted, M, n_live, max_terms, min_mass, mass_est, ctl, pre);
     return 1;
 }
-int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
-                    cudaStream_t st) {
+template <bool XF>
+static void launch_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
+                            cudaStream_t st, double2* amps_rw, const PendPred& pd, const GateTab* tab) {
     static int per_sm = 0;   // one wave of resident blocks: a grid-stride loop has no tail
     if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_classify_kernel, SV_THREADS, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_classify_kernel<XF>, SV_THREADS, 0);
         if (per_sm < 1) per_sm = 1;
     }
     u64 blocks = (n + SV_THREADS * SC_IT - 1) / (SV_THREADS * SC_IT);
     if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
     if (blocks < 1) blocks = 1;
-    ss_classify_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps, seg_cnt);
+    ss_classify_kernel<XF><<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, ckeys, camps, seg_cnt, amps_rw, pd, tab);
+}
+int svk_ss_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
+                    cudaStream_t st, double2* amps_rw, const PendPred* pd, const GateTab* xf_tab) {
+    if (xf_tab) launch_classify<true>(keys, amps, n, ctl, ckeys, camps, seg_cnt, st, amps_rw, *pd, xf_tab);
+    else launch_classify<false>(keys, amps, n, ctl, ckeys, camps, seg_cnt, st, nullptr, PendPred{}, nullptr);
     return 1;
 }
 

@@ -125,6 +125,51 @@ def test_fused_floor_margin_failure_reruns():
     _same(a, b)
 
 
+@pytest.mark.parametrize("pending", [False, True])
+def test_fused_diagonal_gate_rides_on_the_classification_pass(pending):
+    """Diagonal gates (RZ, T, CZ, CCZ, a non-unitary diagonal): the fused call applies them inside the sampled
+    truncation's pass over the state; with and without a truncation pending on the input (dead entries)."""
+    n, N = 44, 1 << 18
+    rng = np.random.default_rng(31 + pending)
+    keys, amps = W.random_state(rng, n, N, spread=1.5)
+    eng, a, b = _engines(n, N + 64)
+    a.load(keys, amps); b.load(keys, amps)
+    if pending:
+        for sv in (a, b):
+            sv.truncate(int(0.97 * N), 1.0)
+            sv.apply_gate([2, 30], W.mat_mcx(2))          # position preserving: the dropped 3 % are dead entries now
+            sv.truncate(int(0.95 * N), 1.0)               # and this one stays pending
+    gates = [([7], W.mat_rz(0.3)), ([40], W.mat_t()), ([3, 25], W.mat_diag_minus_last(2)), ([0, 43, 12], W.mat_diag_minus_last(3)),
+             ([9, 1], np.diag([1.0, 0.5j, -2.0, 0.25]).astype(np.complex128))]
+    K = int(0.9 * N)
+    for i, (q, U) in enumerate(gates):
+        f = 1.0 if i % 2 == 0 else 1 - 1e-5
+        l0 = a.stats()["launches"]
+        ka = a.apply_gate_truncate(q, U, K, f)
+        la = a.stats()["launches"] - l0
+        l0 = b.stats()["launches"]
+        b.apply_gate(q, U); kb = b.truncate(K, f)
+        lb = b.stats()["launches"] - l0
+        assert la == lb - 1, "the fused call must save exactly the diagonal pass (%d vs %d launches)" % (la, lb)
+        assert ka == kb
+        _same(a, b)
+        K = int(0.97 * K)
+    assert a.check_invariants()
+    assert a.stats()["fallbacks"] == 0
+
+
+def test_fused_diagonal_without_a_cut_still_applies_the_gate():
+    n, N = 40, 1 << 16
+    rng = np.random.default_rng(3)
+    keys, amps = W.random_state(rng, n, N, spread=1.0)
+    eng, a, b = _engines(n, N + 64)
+    a.load(keys, amps); b.load(keys, amps)
+    assert a.apply_gate_truncate([5], W.mat_rz(1.1), 0, 1.0) == 1.0          # nothing to cut
+    assert a.apply_gate_truncate([6], W.mat_t(), 2 * N, 2.0) == 1.0
+    b.apply_gate([5], W.mat_rz(1.1)); b.apply_gate([6], W.mat_t())
+    _same(a, b)
+
+
 def test_fused_uncovered_gates_and_small_states():
     """Diagonal, permutation and multi-bit gates, and states below the sampling threshold, take the
     two calls internally."""
