@@ -382,6 +382,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     const int d = 1 << m;
     s->err[0] = 0;
     s->pre_valid = false;
+    s->stats.pre_dropped = 0; s->stats.n_mid = 0;
     s->stats.m = m; s->stats.n_in = s->count; s->stats.n_out = s->count; s->stats.passes = 0;
 
     // a-1: bit j is control-like iff U never connects patterns that differ in bit j
@@ -532,38 +533,43 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         return SV_OK;
     }
     const u64 n_live_in = s->count;
-    // Fused apply + truncate (one active bit): when the cap that follows will cut deep into the gate's output,
-    // a floor for that cut is estimated from a sample of the outputs, and the pass leaves out what lies below it.
+    // Fused apply + truncate: when the cap that follows will cut deep into the gate's output, a floor for that
+    // cut is estimated from a sample of the outputs, and the pass leaves out what lies below it.
     u64 preM = s->phys / 8;
     if (preM > SV_SAMPLE_MAX) preM = SV_SAMPLE_MAX;
-    bool use_pre = ma == 1 && s->fuse_K != 0 && s->count >= s->sample_min_terms && s->phys < (1ull << 32) && preM >= 64 &&
-                   2 * s->count > s->fuse_K + s->fuse_K / 8;
+    bool use_pre = s->fuse_K != 0 && s->count >= s->sample_min_terms && s->phys < (1ull << 32) && preM >= 64 &&
+                   ((u64)1 << ma) * s->count > s->fuse_K + s->fuse_K / 8;
     s->stats.pre_dropped = 0;
     u64 nout = 0, ndead = 0, npre = 0;
     for (;;) {
         u32 pre_parts = 0;
         if (use_pre) {
             const u32 M = (u32)preM;
-            s->stats.launches += svk_pre_sample1(s->keys[s->cur], s->amps[s->cur], s->phys, plast > 0 ? plast : 0, s->tab, s->defer, M,
-                                                 s->smp_k[0], s->stream);
+            if (ma == 1)
+                s->stats.launches += svk_pre_sample1(s->keys[s->cur], s->amps[s->cur], s->phys, plast > 0 ? plast : 0, s->tab, s->defer, M,
+                                                     s->smp_k[0], s->stream);
+            else
+                s->stats.launches += svk_pre_sample_group(s->keys[s->cur], s->amps[s->cur], s->phys, plast, ma, s->tab, s->defer, M,
+                                                          s->smp_k[0], s->stream);
             int in_alt = 0;
             s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, s->stream, &in_alt);
-            s->stats.launches += svk_pre_pivot(s->smp_k[in_alt ? 1 : 0], M, s->phys, s->fuse_K, s->pre_slack, s->pre, s->stream);
+            s->stats.launches += svk_pre_pivot(s->smp_k[in_alt ? 1 : 0], M, s->phys, 1u << ma, s->fuse_K, s->pre_slack, s->pre, s->stream);
             DBG_SYNC("pre_sample+pivot");
         }
         prof_slot(s, ma == 1 ? SV_K_BITPASS_GEN : SV_K_GROUPPASS, 0.0, &ge0, &ge1);
         const int gslot = s->npend - 1;
+        double* pmass = reinterpret_cast<double*>(s->hist);          // per-block partials (the select's histogram is idle)
+        u64* pcnt = s->hist + SV_SEL_BINS;
         if (ma == 1) {   // one active bit: the single-bit pass (p = 0 when the bit already sits at the LSB)
-            double* pmass = reinterpret_cast<double*>(s->hist);          // per-block partials (the select's histogram is idle)
-            u64* pcnt = s->hist + SV_SEL_BINS;
             s->stats.launches += svk_bitpass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast > 0 ? plast : 0, 1, 0,
                                              s->tab, s->defer, s->desc, s->status, s->tile_counter, s->d_count, s->cap, s->stream, ge0, ge1,
                                              use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts);
-            if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         } else {
             s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
-                                               s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1);
+                                               s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1,
+                                               use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts);
         }
+        if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         CHECK_LAUNCH();
         s->stats.passes += 1;
         u64 cnts[3] = {0, 0, 0};   // stored outputs, dead ones among them (exact cancellations of a multi-bit gate), left out

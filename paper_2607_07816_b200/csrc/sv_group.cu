@@ -15,13 +15,20 @@
 //     (counted, so the term count stays exact) instead of forcing a second scan.
 #include "sv_tile.cuh"
 
+//
+// PRE (fused apply + truncate, sv_presample.cu): outputs whose probability pattern is below pre->P_floor are not
+// written.  Which outputs survive is only known once they are computed: the term that opens a tuple computes the
+// tuple's possible rows itself in phase 2a and keeps the SURVIVING rows as the tuple's row mask; the scan, the
+// look-back and phase 2b then run on survivors only (a quarter or an eighth of the possible outputs at the cap),
+// which phase 2b computes once more, one per thread, and stores densely.
 #define GP_ROUND 2048
-template <int MA>
+template <int MA, bool PRE>
 __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                   u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                   const GateTab* __restrict__ gtab, PendPred pd,
                                                                   const TileDesc* __restrict__ desc, u64* status,
-                                                                  u64* d_count, u64 cap, u32 ntiles) {
+                                                                  u64* d_count, u64 cap, u32 ntiles, const PreCut* __restrict__ pre,
+                                                                  double* __restrict__ pre_mass, u64* __restrict__ pre_cnt) {
     constexpr int NP = 1 << MA;
     constexpr u64 AM = (u64)NP - 1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -41,6 +48,9 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     __shared__ int s_cpos[SV_MAX_M], s_col[16], s_mc;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool mv = p >= 0;
+    const u64 Pf = PRE ? pre->P_floor : 0ull;
+    double dmass = 0.0;     // PRE: mass and number of the outputs this thread left out (below the floor)
+    u32 dcnt = 0;
 
     for (int i = tid; i < 256; i += SV_THREADS) sU[i] = gtab->U[i];
     if (tid < SV_MAX_M) s_cpos[tid] = gtab->ctrl_pos[tid];
@@ -180,6 +190,32 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
             __syncthreads();
         }
 
+        // output row r of the tuple that term e opens (pm: live members, pk: stored members, cx: control block):
+        // columns added in ascending LOGICAL index (D1)
+        auto tuple_row_x = [&](int e, int r, u32 pm, u32 pk, int cx, double& sr, double& si) {
+            const double2* urow = &sU[((cx << MA) | r) << MA];
+            sr = 0.0; si = 0.0;
+            if ((pm & (pm - 1)) == 0) {                    // a single live member: one product
+                const int x = __ffs(pm) - 1;
+                const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+                const double2 u = urow[x];
+                cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+            } else {
+#pragma unroll
+                for (int t = 0; t < NP; ++t) {
+                    const int x = s_col[t];
+                    if ((pm >> x) & 1u) {
+                        const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+                        const double2 u = urow[x];
+                        cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+                    }
+                }
+            }
+        };
+        auto tuple_row = [&](int e, int r, double& sr, double& si) {
+            const u64 info = s_info[e];
+            tuple_row_x(e, r, (u32)((info >> 16) & 0xffffu), (u32)((info >> 32) & 0xffffu), (int)(info >> 48), sr, si);
+        };
         // ---- phase 2a: tuples, presence masks, possible output rows -> output counts ----
         const int e0 = min(tid * BP_VT, cnt);
         const int mc = s_mc;
@@ -202,6 +238,21 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                         pk |= 1u << x;
                         const double2 a = sa[e + w];
                         if (!(a.x == 0.0 && a.y == 0.0)) { pm |= 1u << x; rows |= s_nzr[cx][x]; }
+                    }
+                    if (PRE) {   // the rows that survive the floor of the cut that follows: computed here, once more in 2b
+                        u32 cand = rows;
+                        rows = 0;
+                        while (cand) {
+                            const int r = __ffs(cand) - 1;
+                            cand &= cand - 1;
+                            double sr, si;
+                            tuple_row_x(e, r, pm, pk, cx, sr, si);
+                            if (!(sr == 0.0 && si == 0.0)) {       // (an exact cancellation is simply not written)
+                                const double pr = prob_of(make_double2(sr, si));
+                                if ((u64)__double_as_longlong(pr) >= Pf) rows |= 1u << r;
+                                else { dmass = __dadd_rn(dmass, pr); ++dcnt; }
+                            }
+                        }
                     }
                     t_info[v] = (u64)rows | ((u64)pm << 16) | ((u64)pk << 32) | ((u64)cx << 48);
                     mycount += __popc(rows);
@@ -244,28 +295,9 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
             for (int q = tid; q < m; q += SV_THREADS) {
                 const u32 code = s_owner[q];
                 const int e = (int)(code >> 4), r = (int)(code & 15u);
-                const u64 info = s_info[e];
-                const u32 pm = (u32)((info >> 16) & 0xffffu), pk = (u32)((info >> 32) & 0xffffu);
-                const int cx = (int)(info >> 48);
                 const u64 k = sk[e];
-                const double2* urow = &sU[((cx << MA) | r) << MA];
-                double sr = 0.0, si = 0.0;
-                if ((pm & (pm - 1)) == 0) {                    // a single live member: one product
-                    const int x = __ffs(pm) - 1;
-                    const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
-                    const double2 u = urow[x];
-                    cmul_acc(sr, si, u.x, u.y, a.x, a.y);
-                } else {
-#pragma unroll
-                    for (int t = 0; t < NP; ++t) {             // ascending LOGICAL column index (D1)
-                        const int x = s_col[t];
-                        if ((pm >> x) & 1u) {
-                            const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
-                            const double2 u = urow[x];
-                            cmul_acc(sr, si, u.x, u.y, a.x, a.y);
-                        }
-                    }
-                }
+                double sr, si;
+                tuple_row(e, r, sr, si);
                 if (sr == 0.0 && si == 0.0) ++n_dead;          // exact cancellation: a dead entry
                 const u64 g = base + (u64)(h0 + q);
                 if (g < cap) { st_stream_u64(kout + g, (k & ~AM) | (u64)r); st_stream_d2(aout + g, make_double2(sr, si)); }
@@ -277,6 +309,22 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) n_dead += __shfl_xor_sync(0xffffffffu, n_dead, d);
     if (lane == 0 && n_dead) atomicAdd(&d_count[1], (u64)n_dead);
+    if (PRE) {   // block totals of what was left out, summed in a fixed order (see sv_pair.cu)
+        __shared__ double s_pm[BP_WARPS];
+        __shared__ u32 s_pc[BP_WARPS];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            dmass = __dadd_rn(dmass, __shfl_xor_sync(0xffffffffu, dmass, d));
+            dcnt += __shfl_xor_sync(0xffffffffu, dcnt, d);
+        }
+        if (lane == 0) { s_pm[warp] = dmass; s_pc[warp] = dcnt; }
+        __syncthreads();
+        if (tid == 0) {
+            double m = 0.0; u64 c = 0;
+            for (int w = 0; w < BP_WARPS; ++w) { m = __dadd_rn(m, s_pm[w]); c += s_pc[w]; }
+            pre_mass[blockIdx.x] = m; pre_cnt[blockIdx.x] = c;
+        }
+    }
 }
 
 // Tile boundaries when no bit has to move (the active bits already sit at positions 0 .. ma-1): nominal
@@ -295,27 +343,32 @@ __global__ void find_starts_kernel(const u64* __restrict__ keys, u64 n, int ma, 
     desc[j] = d;
 }
 
-template <int MA>
-static void launch_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
-                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st) {
+template <int MA, bool PRE>
+static u32 launch_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
+                            const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
+                            const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
     const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 8 + (size_t)GP_ROUND * 2;   // landing + work + tuple table + owners
     static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(grouppass_kernel<MA>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    if (!attr) { cudaFuncSetAttribute(grouppass_kernel<MA, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
     if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grouppass_kernel<MA>, SV_THREADS, smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grouppass_kernel<MA, PRE>, SV_THREADS, smem);
         if (per_sm < 1) per_sm = 1;
     }
     const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    grouppass_kernel<MA><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles);
+    grouppass_kernel<MA, PRE><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles,
+                                                                    pre, pre_mass, pre_cnt);
+    return grid;
 }
 
 // Final pass of a gate with ma >= 2 active bits.  p < 0: no bit has to move.  Writes the number of
 // stored outputs to d_count[0] and the number of dead ones among them (exact cancellations) to d_count[1].
 int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
                   const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
-                  u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1) {
+                  u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1, const PreCut* pre, double* pre_mass, u64* pre_cnt,
+                  u32* pre_parts) {
     cudaMemsetAsync(d_count, 0, 2 * sizeof(u64), st);
+    if (pre_parts) *pre_parts = 0;
     if (n == 0) return 0;
     const u32 tnom = (u32)(BP_TILE - (1 << ma));
     const u32 ntiles = (u32)((n + tnom - 1) / tnom);
@@ -324,10 +377,20 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
     if (p >= 0) launches += svk_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
     else { find_starts_kernel<<<(ntiles + 1 + 127) / 128, 128, 0, st>>>(kin, n, ma, tnom, ntiles, desc); launches += 1; }
     if (e0) cudaEventRecord(e0, st);
-    switch (ma) {
-        case 2: launch_grouppass<2>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
-        case 3: launch_grouppass<3>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
-        default: launch_grouppass<4>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+    if (pre) {
+        u32 g = 0;
+        switch (ma) {
+            case 2: g = launch_grouppass<2, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt); break;
+            case 3: g = launch_grouppass<3, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt); break;
+            default: g = launch_grouppass<4, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt); break;
+        }
+        if (pre_parts) *pre_parts = g;
+    } else {
+        switch (ma) {
+            case 2: launch_grouppass<2, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+            case 3: launch_grouppass<3, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+            default: launch_grouppass<4, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st); break;
+        }
     }
     if (e1) cudaEventRecord(e1, st);
     return launches;

@@ -98,9 +98,11 @@ int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStre
 
 // Final pass of a gate with ma >= 2 active bits (sv_group.cu).  p < 0: the active bits already sit at the
 // LSBs.  A pending truncation is applied while loading.  d_count[0] = stored outputs, d_count[1] = dead ones.
+// pre != nullptr (fused apply + truncate): outputs below pre->P_floor (and exact zeros) are left out, see svk_bitpass.
 int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
                   const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
-                  u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr);
+                  u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr,
+                  const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr);
 
 // Lean single-bit pass (sv_pair.cu): moves physical bit p to the LSB in one streaming pass.
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
@@ -115,7 +117,9 @@ int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u6
 // fused apply + truncate: pre-sample of a one-bit gate's outputs -> (sort) -> floor; per-block partials -> totals (d_count[2] = count)
 int svk_pre_sample1(const u64* keys, const double2* amps, u64 n, int p, const GateTab* tab, const PendPred& pend, u32 M, u64* smp,
                     cudaStream_t st);
-int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st);
+int svk_pre_sample_group(const u64* keys, const double2* amps, u64 n, int p, int ma, const GateTab* tab, const PendPred& pend, u32 M,
+                         u64* smp, cudaStream_t st);
+int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u32 mult, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st);
 int svk_pre_finish(const double* part_mass, const u64* part_cnt, u32 nparts, PreCut* pre, u64* d_count, cudaStream_t st);
 int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
 // Diagonal gate fused with a pending truncation (out of place, compacting).

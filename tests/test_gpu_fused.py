@@ -78,6 +78,79 @@ def test_fused_equals_two_calls(qubit, frac, f):
     assert abs(a.norm() - 1.0) <= 1e-13
 
 
+def _ctrl_block(V, nctrl=1):
+    """V on the low local bits, applied when the nctrl high local bits are all ones."""
+    d = V.shape[0]
+    D = d << nctrl
+    M = np.eye(D, dtype=np.complex128)
+    M[D - d:, D - d:] = V
+    return M
+
+
+@pytest.mark.parametrize("qubits,frac", [((5, 30), 0.9), ((0, 1), 1.5), ((43, 2), 3.0), ((7, 19, 33), 1.2), ((1, 0, 2), 5.0),
+                                          ((12, 40, 3, 27), 2.0)])
+def test_fused_multi_bit_gate_equals_two_calls(qubits, frac):
+    """Haar gates on 2, 3 and 4 qubits on generic terms (4x, 8x, 16x outputs before the cut): the count pass +
+    write pass of sv_group.cu (PRE) against apply + truncate."""
+    m = len(qubits)
+    n, N = 44, (1 << 17) if m < 4 else (1 << 15)
+    rng = np.random.default_rng(sum(qubits) + m)
+    keys, amps = W.random_state(rng, n, N, spread=1.5)
+    eng, a, b = _engines(n, (1 << m) * N + 64)
+    a.load(keys, amps); b.load(keys, amps)
+    U = W.haar_unitary(rng, 1 << m)
+    K = int(frac * N)
+    ka = a.apply_gate_truncate(list(qubits), U, K, 1.0)
+    st = a.stats()
+    b.apply_gate(list(qubits), U)
+    n_mid = b.num_terms()
+    kb = b.truncate(K, 1.0)
+    assert st["n_mid"] == n_mid and st["n_out"] == b.num_terms() == K
+    assert st["pre_dropped"] > 0 and st["fallbacks"] == 0, st
+    assert abs(ka - kb) <= 1e-13
+    _same(a, b)
+    assert a.check_invariants()
+
+
+def test_fused_multi_bit_chain_with_controls_and_pending_cuts():
+    """A chain of fused calls: SU(4), controlled SU(4) (3 qubits, 2 active), 8x8, H, diagonal and CNOT gates in
+    between, mass + cap criteria, so that every pass meets a pending cut and dead entries."""
+    n, N = 40, 1 << 16
+    rng = np.random.default_rng(77)
+    keys, amps = W.random_state(rng, n, N, spread=1.0)
+    eng, a, b = _engines(n, 16 * N)
+    a.load(keys, amps); b.load(keys, amps)
+    K = N
+    used = 0
+    for step in range(14):
+        kind = step % 7
+        if kind == 0:
+            q, U = [int(x) for x in rng.choice(n, 2, replace=False)], W.haar_unitary(rng, 4)
+        elif kind == 1:
+            q, U = [int(x) for x in rng.choice(n, 3, replace=False)], _ctrl_block(W.haar_unitary(rng, 4))
+        elif kind == 2:
+            q, U = [int(x) for x in rng.choice(n, 1)], W.mat_rz(0.7)
+        elif kind == 3:
+            q, U = [int(x) for x in rng.choice(n, 3, replace=False)], W.haar_unitary(rng, 8)
+        elif kind == 4:
+            q, U = [int(x) for x in rng.choice(n, 2, replace=False)], W.mat_mcx(2)
+        elif kind == 5:
+            q, U = [int(x) for x in rng.choice(n, 1)], W.mat_h()
+        else:
+            q, U = [int(x) for x in rng.choice(n, 2, replace=False)], _ctrl_block(_rand_u2(rng))
+        fa, fb = a.stats()["fallbacks"], b.stats()["fallbacks"]
+        ka = a.apply_gate_truncate(q, U, K, 1 - 1e-6)
+        used += 1 if a.stats()["pre_dropped"] else 0
+        b.apply_gate(q, U); kb = b.truncate(K, 1 - 1e-6)
+        assert abs(ka - kb) <= 1e-13, (step, ka, kb)
+        _same(a, b, exact=False)
+        print("step", step, kind, a.stats()["n_in"], a.stats()["n_mid"], a.stats()["n_out"], "pre", a.stats()["pre_dropped"],
+              "fallbacks +%d / +%d" % (a.stats()["fallbacks"] - fa, b.stats()["fallbacks"] - fb))
+    assert used >= 6, used
+    assert a.stats()["fallbacks"] <= b.stats()["fallbacks"] + 1
+    assert a.check_invariants()
+
+
 def test_fused_with_pending_cut_and_controls():
     """The input carries a deferred truncation and dead entries; controlled gates (only the control = 1
     tuples mix), then a chain of fused calls."""
@@ -112,7 +185,7 @@ def test_fused_floor_margin_failure_reruns():
     n, N = 44, 1 << 17
     rng = np.random.default_rng(9)
     keys, amps = W.random_state(rng, n, N, spread=1.5)
-    eng, a, b = _engines(n, 2 * N + 64)
+    eng, a, b = _engines(n, 4 * N)
     a.load(keys, amps); b.load(keys, amps)
     a.set_option(eng.OPT_PRE_SLACK, (-3000) & ((1 << 64) - 1))
     U = _rand_u2(rng)
@@ -121,6 +194,13 @@ def test_fused_floor_margin_failure_reruns():
     st = a.stats()
     assert st["fallbacks"] == 1 and st["pre_dropped"] == 0, st
     b.apply_gate([5], U); kb = b.truncate(K, 1.0)
+    assert abs(ka - kb) <= 1e-13
+    _same(a, b)
+    U4 = W.haar_unitary(rng, 4)                           # the same for the multi-bit pass
+    ka = a.apply_gate_truncate([8, 21], U4, K, 1.0)
+    st = a.stats()
+    assert st["fallbacks"] == 2 and st["pre_dropped"] == 0, st
+    b.apply_gate([8, 21], U4); kb = b.truncate(K, 1.0)
     assert abs(ka - kb) <= 1e-13
     _same(a, b)
 
