@@ -42,13 +42,16 @@
 // writes over the banks and keeps the copy-out reads of consecutive entries inside one row.
 #define BP_SWK(x) ((x) ^ (((x) >> 4) & 15))
 #define BP_SWA(x) ((x) ^ (((x) >> 3) & 7))
+#ifndef BP_GEN_CTAS
+#define BP_GEN_CTAS 3                          // resident blocks per SM of the general one-bit pass (0: BP_CTAS)
+#endif
 #define BP_WKN BP_TILE                         // entries of the key / slot work arrays
 #define BP_ROUND BP_TILE                       // outputs staged per round when amplitudes are staged too
 // PRE (MODE 1 only; fused apply + truncate, sv_presample.cu): outputs whose probability pattern is below
 // pre->P_floor are not written; every block leaves the mass and the number of what it left out in
 // pre_mass / pre_cnt[blockIdx.x] (tiles are taken in a fixed order, so these sums are the same every run).
 template <int MODE, bool FIXED, bool PRE>
-__global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+__global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GEN_CTAS : BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
@@ -294,32 +297,27 @@ __global__ void __launch_bounds__(SV_THREADS, BP_CTAS) bitpass_kernel(const u64*
                 const u64 k = takeA ? ka : kb;
                 const u64 nk = (k & himask) | ((k & lowmask) << 1);     // new layout, LSB = 0
                 if (PAIR) {
-                    double2 a, pa = make_double2(0.0, 0.0);
-                    bool has_partner = false;
-                    if (takeA) {
-                        a = amp_at(pc.oneblock ? i : (int)Wi[i], k); ++i; ++pos;
-                        has_partner = (kb == k);
-                        if (has_partner) { pa = amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit); ++j; ++pos; kb = (j < nB) ? WkB[j] : ~0ull; }
-                        ka = (i < nA) ? Wk[i] : ~0ull;
-                    } else {
-                        a = amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit); ++j; ++pos;
-                        kb = (j < nB) ? WkB[j] : ~0ull;
-                    }
+                    // one code path for the common case (a term without its partner, from either run): the run only
+                    // selects the landing slot and the column of U; a partner (rare in sparse states) adds its column
+                    const int slot = pc.oneblock ? (takeA ? i : nA + j) : (takeA ? (int)Wi[i] : (int)WiB[j]);
+                    const double2 a = amp_at(slot, takeA ? k : (k | bit));
+                    const int c = takeA ? 0 : 1;
+                    const bool has_partner = takeA && (kb == k);
+                    if (takeA) { ++i; ka = (i < nA) ? Wk[i] : ~0ull; } else { ++j; kb = (j < nB) ? WkB[j] : ~0ull; }
+                    ++pos;
                     int cx = 0;
                     const int mc = s_mc;
                     for (int q = 0; q < mc; ++q) cx |= (int)((nk >> s_cpos[q]) & 1ull) << q;
                     const double2* u = &sU[cx << 2];                    // u[xr * 2 + xc]
                     double r0 = 0.0, m0 = 0.0, r1 = 0.0, m1 = 0.0;
-                    if (takeA) {
-                        cmul_acc(r0, m0, u[0].x, u[0].y, a.x, a.y);
-                        cmul_acc(r1, m1, u[2].x, u[2].y, a.x, a.y);
-                        if (has_partner) {
-                            cmul_acc(r0, m0, u[1].x, u[1].y, pa.x, pa.y);
-                            cmul_acc(r1, m1, u[3].x, u[3].y, pa.x, pa.y);
-                        }
-                    } else {
-                        cmul_acc(r0, m0, u[1].x, u[1].y, a.x, a.y);
-                        cmul_acc(r1, m1, u[3].x, u[3].y, a.x, a.y);
+                    cmul_acc(r0, m0, u[c].x, u[c].y, a.x, a.y);
+                    cmul_acc(r1, m1, u[2 + c].x, u[2 + c].y, a.x, a.y);
+                    if (has_partner) {
+                        const double2 pa = amp_at(pc.oneblock ? nA + j : (int)WiB[j], k | bit);
+                        ++j; ++pos;
+                        kb = (j < nB) ? WkB[j] : ~0ull;
+                        cmul_acc(r0, m0, u[1].x, u[1].y, pa.x, pa.y);
+                        cmul_acc(r1, m1, u[3].x, u[3].y, pa.x, pa.y);
                     }
                     u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
                     if (PRE) {   // below the floor of the cut that follows: never written
