@@ -127,3 +127,64 @@ def test_config5_at_2e24_properties():
             assert abs(sv.norm() - 1.0) <= 1e-11
     assert sv.check_invariants()
     assert sv.stats()["fallbacks"] <= 40
+
+
+def test_config5_fused_call_equals_two_calls_at_2e22():
+    """The launch configuration bench.py times (sv_apply_gate_truncate, default sampling threshold 2^21) against
+    the two separate calls on a twin engine, config 5 at K = 2^22: identical term counts after every gate,
+    identical kept fractions to 1e-13, and identical states (keys bitwise, amplitudes to 1e-13 relative)
+    at check points; the fused path must have used its output floor and must not have needed a re-run."""
+    from paper_2607_07816_b200 import engine
+    K = 1 << 22
+    c = W.config5(num_gates=150, max_terms=K)
+    a, b = engine.SparseSV(c.n, 8 * K), engine.SparseSV(c.n, 8 * K)
+    used, peak_a = 0, 0
+    for i, g in enumerate(c.gates):
+        ka = a.apply_gate_truncate(g.qubits, g.U, c.max_terms, c.min_mass)
+        st = a.stats()
+        b.apply_gate(g.qubits, g.U)
+        n_mid = b.num_terms()
+        kb = b.truncate(c.max_terms, c.min_mass)
+        assert st["n_mid"] == n_mid, (i, g.name)
+        assert a.num_terms() == b.num_terms(), (i, g.name)
+        assert abs(ka - kb) <= 1e-13, (i, g.name, ka, kb)
+        used += 1 if st["pre_dropped"] else 0
+        if st["n_in"] >= (1 << 21):                      # (smaller states do not sample: they take the two calls)
+            peak_a = max(peak_a, n_mid - st["pre_dropped"])
+        if i in (110, 149):
+            ea, eb = a.export(), b.export()
+            assert np.array_equal(ea[0], eb[0])
+            assert np.allclose(ea[1], eb[1], rtol=1e-13, atol=0)
+    assert used >= 10, used
+    assert a.stats()["fallbacks"] <= b.stats()["fallbacks"]
+    assert peak_a <= int(1.2 * K), "the fused path stored %d outputs at its peak (K = %d)" % (peak_a, K)
+    assert a.check_invariants()
+
+
+def test_fused_floor_on_dense_tuples():
+    """A state that is dense in the gate's qubits (every tuple has all its members): the pre-sample accepts one
+    member per tuple, so its estimate of the output distribution must stay unbiased -- the floor is used and
+    holds (no re-run), for one-bit and two-bit gates, with the moved bit far from and at the LSB."""
+    from paper_2607_07816_b200 import engine
+    n = 22
+    rng = np.random.default_rng(8)
+    N = 1 << 19
+    keys = np.arange(N, dtype=np.uint64)                       # dense in qubits 0..18
+    amps = (rng.normal(size=N) + 1j * rng.normal(size=N)) * np.exp(rng.normal(size=N))
+    amps /= np.sqrt(np.sum(np.abs(amps) ** 2))
+    for qubits in ([0], [18], [7], [0, 1], [18, 3], [9, 20]):
+        a, b = engine.SparseSV(n, 4 * N), engine.SparseSV(n, 4 * N)
+        for sv in (a, b):
+            sv.set_option(engine.OPT_SAMPLE_MIN_TERMS, 512)
+            sv.load(keys, amps)
+        U = W.haar_unitary(rng, 1 << len(qubits))
+        K = N // 2
+        ka = a.apply_gate_truncate(qubits, U, K, 1.0)
+        st = a.stats()
+        b.apply_gate(qubits, U); kb = b.truncate(K, 1.0)
+        assert st["pre_dropped"] > 0 and st["fallbacks"] == 0, (qubits, st)
+        assert st["n_mid"] - st["pre_dropped"] <= int(1.15 * K), (qubits, st)
+        assert abs(ka - kb) <= 1e-13
+        ea, eb = a.export(), b.export()
+        assert np.array_equal(ea[0], eb[0]) and np.array_equal(ea[1], eb[1])
+        a.close(); b.close()
