@@ -242,11 +242,19 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                     if (PRE) {   // the rows that survive the floor of the cut that follows: computed here, once more in 2b
                         u32 cand = rows;
                         rows = 0;
+                        const bool single = (pm & (pm - 1)) == 0;          // one live member: its amplitude is read once
+                        const int x1 = __ffs(pm) - 1;
+                        const double2 a1 = single ? sa[e + __popc(pk & ((1u << x1) - 1u))] : make_double2(0.0, 0.0);
                         while (cand) {
                             const int r = __ffs(cand) - 1;
                             cand &= cand - 1;
-                            double sr, si;
-                            tuple_row_x(e, r, pm, pk, cx, sr, si);
+                            double sr = 0.0, si = 0.0;
+                            if (single) {
+                                const double2 u = sU[(((cx << MA) | r) << MA) | x1];
+                                cmul_acc(sr, si, u.x, u.y, a1.x, a1.y);
+                            } else {
+                                tuple_row_x(e, r, pm, pk, cx, sr, si);
+                            }
                             if (!(sr == 0.0 && si == 0.0)) {       // (an exact cancellation is simply not written)
                                 const double pr = prob_of(make_double2(sr, si));
                                 if ((u64)__double_as_longlong(pr) >= Pf) rows |= 1u << r;
