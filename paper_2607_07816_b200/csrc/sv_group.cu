@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                         const double2 a = sa[e + w];
                         if (!(a.x == 0.0 && a.y == 0.0)) { pm |= 1u << x; rows |= s_nzr[cx][x]; }
                     }
-                    if (PRE) {   // the rows that survive the floor of the cut that follows: computed here, once more in 2b
+                    if constexpr (PRE) {   // the rows that survive the floor of the cut that follows: computed here, once more in 2b
                         u32 cand = rows;
                         rows = 0;
                         const bool single = (pm & (pm - 1)) == 0;          // one live member: its amplitude is read once

@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                         cmul_acc(r1, m1, u[3].x, u[3].y, pa.x, pa.y);
                     }
                     u32 f0 = !(r0 == 0.0 && m0 == 0.0), f1 = !(r1 == 0.0 && m1 == 0.0);
-                    if (PRE) {   // below the floor of the cut that follows: never written
+                    if constexpr (PRE) {   // below the floor of the cut that follows: never written
                         const double p0 = prob_of(make_double2(r0, m0)), p1 = prob_of(make_double2(r1, m1));
                         if (f0 && (u64)__double_as_longlong(p0) < Pf) { f0 = 0; dmass = __dadd_rn(dmass, p0); ++dcnt; }
                         if (f1 && (u64)__double_as_longlong(p1) < Pf) { f1 = 0; dmass = __dadd_rn(dmass, p1); ++dcnt; }
