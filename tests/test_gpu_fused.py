@@ -250,6 +250,26 @@ def test_fused_diagonal_without_a_cut_still_applies_the_gate():
     _same(a, b)
 
 
+def test_fused_mass_only_and_count_only_criteria():
+    """max_terms = 0 (p-mass threshold only: no output floor, but the diagonal gate still rides on the classify pass)
+    and min_mass >= 1 (cap only), general and diagonal gates, after a host load (total mass not yet known exactly)."""
+    n, N = 42, 1 << 17
+    rng = np.random.default_rng(12)
+    keys, amps = W.random_state(rng, n, N, spread=1.5)
+    amps *= 1.7                                            # not normalised: S != 1
+    eng, a, b = _engines(n, 16 * N)
+    a.load(keys, amps); b.load(keys, amps)
+    seq = [([4], _rand_u2(rng), 0, 1 - 1e-3), ([9], W.mat_rz(0.4), 0, 1 - 1e-4), ([30, 2], W.haar_unitary(rng, 4), 0, 0.99),
+           ([11], W.mat_t(), N // 2, 2.0), ([6], _rand_u2(rng), N // 3, 1.0), ([1, 40], W.mat_diag_minus_last(2), 0, 0.999)]
+    for q, U, K, f in seq:
+        ka = a.apply_gate_truncate(q, U, K, f)
+        b.apply_gate(q, U); kb = b.truncate(K, f)
+        assert abs(ka - kb) <= 1e-13, (q, K, f, ka, kb)
+        _same(a, b, exact=False)
+    assert a.check_invariants()
+    assert abs(a.norm() - 1.0) <= 1e-13
+
+
 def test_fused_uncovered_gates_and_small_states():
     """Diagonal, permutation and multi-bit gates, and states below the sampling threshold, take the
     two calls internally."""
