@@ -102,6 +102,21 @@ int sv_truncate(sv_state *s, uint64_t max_terms, double min_mass, double *kept_f
 int sv_apply_gate_truncate(sv_state *s, const int *qubits, int m, const sv_c128 *U,
                            uint64_t max_terms, double min_mass, double *kept_fraction);
 
+/* Gate fusion ("for each block of single- and two-qubit gates we fuse those gates into a
+ * multi-qubit unitary operation", one state update and one truncation per block).  HOST ONLY: no device work.
+ * The n_gates input gates -- gate_m[g] qubits each, their qubit lists concatenated in gate_qubits, their row-major
+ * 2^m x 2^m matrices concatenated in gate_U (conventions of sv_apply_gate) -- are merged, in order and greedily,
+ * into blocks: a gate joins the running block while the union of qubits has at most max_m (<= SV_FUSE_MAX_M)
+ * members, else the block is closed and the gate opens the next one.  A block's qubits are listed in order of first
+ * appearance (local bit j = j-th listed qubit); its matrix is the product of its gates, later gates on the left.
+ * Outputs (caller-owned): *n_blocks; block_m[n_gates]; block_qubits[sum of gate_m], concatenated; block_U,
+ * concatenated, block_U_capacity entries available (n_gates * 4^max_m always suffices).  Each block is a gate for
+ * sv_apply_gate / sv_apply_gate_truncate.  SV_ERR_INVALID_ARG: bad sizes, a repeated or out-of-range qubit, a gate
+ * wider than max_m, or not enough room in block_U. */
+#define SV_FUSE_MAX_M 4
+int sv_fuse_gates(int n_gates, const int *gate_m, const int *gate_qubits, const sv_c128 *gate_U, int max_m,
+                  int *n_blocks, int *block_m, int *block_qubits, sv_c128 *block_U, size_t block_U_capacity);
+
 /* *mass = sum of |a|^2 over all terms (Eq. 4) -- the mass, not its root. */
 int sv_norm(sv_state *s, double *mass);
 

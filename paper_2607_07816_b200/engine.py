@@ -19,7 +19,7 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
-           "sv_apply_gate_truncate"]
+           "sv_apply_gate_truncate", "sv_fuse_gates"]
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
 OPT_PRE_SLACK = 1
@@ -59,6 +59,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_apply_gate.argtypes = [vp, vp, i32, vp]
     lib.sv_truncate.restype = i32
     lib.sv_truncate.argtypes = [vp, u64, dbl, C.POINTER(dbl)]
+    lib.sv_fuse_gates.restype = i32
+    lib.sv_fuse_gates.argtypes = [i32, vp, vp, vp, i32, C.POINTER(i32), vp, vp, vp, C.c_size_t]
     lib.sv_apply_gate_truncate.restype = i32
     lib.sv_apply_gate_truncate.argtypes = [vp, vp, i32, vp, u64, dbl, C.POINTER(dbl)]
     lib.sv_norm.restype = i32
@@ -89,6 +91,35 @@ def load_library(path: str = _LIBPATH):
 
 
 lib = load_library()
+
+
+def fuse_gates(gates, max_m: int = 4):
+    """sv_fuse_gates: gates = sequence of (qubits, U); returns the fused blocks as a list of
+    (qubits, U).  Argument marshalling only; the fusion itself is the library's host code."""
+    gates = list(gates)
+    if not gates:
+        return []
+    ms = np.array([len(q) for q, _ in gates], dtype=np.int32)
+    qs = np.ascontiguousarray(np.concatenate([np.asarray(q, dtype=np.int32) for q, _ in gates]))
+    for (q, U), m in zip(gates, ms):
+        if np.shape(U) != (1 << m, 1 << m):
+            raise ValueError("U must be 2^m x 2^m")
+    us = np.ascontiguousarray(np.concatenate([np.asarray(U, dtype=np.complex128).reshape(-1) for _, U in gates]))
+    cap = len(gates) << (2 * max_m)
+    nb = C.c_int(0)
+    bm = np.zeros(len(gates), dtype=np.int32)
+    bq = np.zeros(int(ms.sum()), dtype=np.int32)
+    bu = np.zeros(cap, dtype=np.complex128)
+    rc = lib.sv_fuse_gates(len(gates), ms.ctypes.data, qs.ctypes.data, us.ctypes.data, int(max_m), C.byref(nb),
+                           bm.ctypes.data, bq.ctypes.data, bu.ctypes.data, cap)
+    if rc != SV_OK:
+        raise SvError(rc, "sv_fuse_gates: invalid gate list")
+    out, qo, uo = [], 0, 0
+    for i in range(nb.value):
+        m = int(bm[i])
+        out.append(([int(x) for x in bq[qo:qo + m]], bu[uo:uo + (1 << (2 * m))].reshape(1 << m, 1 << m).copy()))
+        qo += m; uo += 1 << (2 * m)
+    return out
 
 
 class SparseSV:
