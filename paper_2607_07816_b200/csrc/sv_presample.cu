@@ -171,19 +171,25 @@ __global__ void pre_pivot_kernel(const u64* __restrict__ smp, u32 M, u64 n, u32 
     *pre = c;
 }
 
-// Sums the per-block partials of the pass in block order (fixed order: the same bits every run).
-__global__ void pre_finish_kernel(const double* __restrict__ part_mass, const u64* __restrict__ part_cnt, u32 nparts,
-                                  PreCut* __restrict__ pre, u64* __restrict__ d_count) {
+// Sums the per-block partials of the pass in block order (fixed order: the same bits every run).  The partials are
+// first brought to shared memory by the whole block (one round trip instead of one per partial).
+#define PF_MAX 2048
+__global__ void __launch_bounds__(1024) pre_finish_kernel(const double* __restrict__ part_mass, const u64* __restrict__ part_cnt,
+                                                          u32 nparts, PreCut* __restrict__ pre, u64* __restrict__ d_count) {
+    __shared__ double sm[PF_MAX];
+    __shared__ u64 sc[PF_MAX];
+    for (u32 b = threadIdx.x; b < nparts && b < PF_MAX; b += blockDim.x) { sm[b] = part_mass[b]; sc[b] = part_cnt[b]; }
+    __syncthreads();
     if (threadIdx.x != 0) return;
     double hi = 0.0, lo = 0.0;   // double-double running sum
     u64 cnt = 0;
     for (u32 b = 0; b < nparts; ++b) {
-        const double x = part_mass[b];
+        const double x = b < PF_MAX ? sm[b] : part_mass[b];
         const double s = __dadd_rn(hi, x);
         const double bb = __dsub_rn(s, hi);
         const double err = __dadd_rn(__dsub_rn(hi, __dsub_rn(s, bb)), __dsub_rn(x, bb));
         hi = s; lo = __dadd_rn(lo, err);
-        cnt += part_cnt[b];
+        cnt += b < PF_MAX ? sc[b] : part_cnt[b];
     }
     const double s = __dadd_rn(hi, lo);
     lo = __dsub_rn(lo, __dsub_rn(s, hi)); hi = s;
@@ -206,6 +212,6 @@ int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u32 mult, u64 max_terms, 
     return 1;
 }
 int svk_pre_finish(const double* part_mass, const u64* part_cnt, u32 nparts, PreCut* pre, u64* d_count, cudaStream_t st) {
-    pre_finish_kernel<<<1, 32, 0, st>>>(part_mass, part_cnt, nparts, pre, d_count);
+    pre_finish_kernel<<<1, 1024, 0, st>>>(part_mass, part_cnt, nparts, pre, d_count);
     return 1;
 }
