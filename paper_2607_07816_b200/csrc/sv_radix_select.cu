@@ -319,6 +319,17 @@ __global__ void sel_seed_kernel(SelState* ss, u64* hist, const SampleCtl* ctl, u
         if (!(rem.hi > 0.0)) miss = true;
         s.mass_rem_hi = rem.hi; s.mass_rem_lo = rem.lo;
     }
+    // The candidates lie in [P_lo, P_hi].  When both share the exponent field the exponent level would find one bin:
+    // start at the first pattern level instead, with the common leading bits of the band already resolved.
+    if (!miss && c.P_hi != ~0ull && (c.P_lo >> 52) == (c.P_hi >> 52) && c.P_lo != c.P_hi) {
+        const int e = (int)(c.P_lo >> 52) & 0x7ff;
+        const int hb = 63 - __clzll((long long)(c.P_lo ^ c.P_hi));          // highest bit in which the band's ends differ
+        const u64 low = (hb >= 63) ? ~0ull : ((2ull << hb) - 1);
+        s.E = e ? e : 1;
+        s.rmask = ~low; s.rval = c.P_lo & ~low;
+        s.dmask = top_bits(low, 11);
+        s.phase = 1;
+    }
     if (miss) s.done = 3;
     *ss = s;
 }
