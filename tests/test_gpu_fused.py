@@ -270,6 +270,30 @@ def test_fused_mass_only_and_count_only_criteria():
     assert abs(a.norm() - 1.0) <= 1e-13
 
 
+@pytest.mark.parametrize("f", [1.0, 1 - 1e-3])
+def test_fused_floor_then_full_state_select(f):
+    """The input is large enough for the output floor, but the cap is so small that what the pass stores falls below
+    the sampling threshold: the truncation then runs the FULL-state select, which must still count the left-out
+    outputs' mass in S (kept fraction) and treat them as dropped."""
+    n, N = 44, 1 << 17
+    rng = np.random.default_rng(21)
+    keys, amps = W.random_state(rng, n, N, spread=1.5)
+    eng, a, b = _engines(n, 4 * N, sample_min=N)
+    a.load(keys, amps); b.load(keys, amps)
+    K = 1 << 12
+    for q, U in (([7], _rand_u2(rng)),):
+        ka = a.apply_gate_truncate(q, U, K, f)
+        st = a.stats()
+        assert st["pre_dropped"] > 0 and st["n_mid"] - st["pre_dropped"] < N, st
+        b.apply_gate(q, U); kb = b.truncate(K, f)
+        assert abs(ka - kb) <= 1e-13, (ka, kb)
+        _same(a, b, exact=(f >= 1.0))
+    o = _oracle(n)
+    o.load(keys, amps); o.apply_gate([7], U); ko = o.truncate(K, f)
+    assert abs(ka - ko) <= MASS_TOL
+    assert_truncation_parity(a.export()[:2], o.export()[:2])
+
+
 def test_fused_uncovered_gates_and_small_states():
     """Diagonal, permutation and multi-bit gates, and states below the sampling threshold, take the
     two calls internally."""
