@@ -167,28 +167,21 @@ __global__ void __launch_bounds__(SV_THREADS) sel_pass_kernel(const double2* __r
             const u64 mant = x & ((1ull << 52) - 1);
             const u64 M = ((x >> 52) & 0x7ff) ? (mant | (1ull << 52)) : mant;
             const u32 h = (u32)(M >> 26), l = (u32)(M & ((1ull << 26) - 1));
-            u32 todo = __ballot_sync(0xffffffffu, valid);
-            while (todo) {   // one round per distinct bin in the warp
-                const int ldr = __ffs(todo) - 1;
-                const u32 b0 = __shfl_sync(0xffffffffu, bin, ldr);
-                const bool mine = valid && bin == b0;
-                const u32 grp = __ballot_sync(0xffffffffu, mine);
+            // lanes of the warp that hit the same bin form a group (one match instruction); the group's sums, AND and
+            // OR are reduced inside the group and its lowest lane updates the shared histogram once
+            const u32 act = __ballot_sync(0xffffffffu, valid);
+            if (valid) {
+                const u32 grp = __match_any_sync(act, bin);
                 u32 sh = 0, sl = 0;
-                if (MODE < 2) {
-                    sh = __reduce_add_sync(0xffffffffu, mine ? h : 0u);
-                    sl = __reduce_add_sync(0xffffffffu, mine ? l : 0u);
+                if (MODE < 2) { sh = __reduce_add_sync(grp, h); sl = __reduce_add_sync(grp, l); }
+                const u32 alo = __reduce_and_sync(grp, (u32)x), ahi = __reduce_and_sync(grp, (u32)(x >> 32));
+                const u32 olo = __reduce_or_sync(grp, (u32)x), ohi = __reduce_or_sync(grp, (u32)(x >> 32));
+                if (lane == __ffs(grp) - 1) {
+                    atomicAdd(&scnt[bin], (u32)__popc(grp));
+                    if (MODE < 2) { atomicAdd(&shi[bin], (u64)sh); atomicAdd(&slo[bin], (u64)sl); }
+                    atomicAnd(&sand_lo[bin], alo); atomicAnd(&sand_hi[bin], ahi);
+                    atomicOr(&sor_lo[bin], olo); atomicOr(&sor_hi[bin], ohi);
                 }
-                const u32 alo = __reduce_and_sync(0xffffffffu, mine ? (u32)x : ~0u);
-                const u32 ahi = __reduce_and_sync(0xffffffffu, mine ? (u32)(x >> 32) : ~0u);
-                const u32 olo = __reduce_or_sync(0xffffffffu, mine ? (u32)x : 0u);
-                const u32 ohi = __reduce_or_sync(0xffffffffu, mine ? (u32)(x >> 32) : 0u);
-                if (lane == ldr) {
-                    atomicAdd(&scnt[b0], (u32)__popc(grp));
-                    if (MODE < 2) { atomicAdd(&shi[b0], (u64)sh); atomicAdd(&slo[b0], (u64)sl); }
-                    atomicAnd(&sand_lo[b0], alo); atomicAnd(&sand_hi[b0], ahi);
-                    atomicOr(&sor_lo[b0], olo); atomicOr(&sor_hi[b0], ohi);
-                }
-                todo &= ~grp;
             }
         }
     }
