@@ -377,40 +377,63 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
         sgh[threadIdx.x] = sm.hi; sgl[threadIdx.x] = sm.lo; sgc[threadIdx.x] = sc;
     }
     __syncthreads();
-    if (threadIdx.x != 0) return;
+    if (threadIdx.x >= 32) return;
+    const int lane = threadIdx.x;
+    if (s.phase > 1 && lane != 0) return;
     dd kept; kept.hi = s.kept_hi; kept.lo = s.kept_lo;
     dd rem; rem.hi = s.mass_rem_hi; rem.lo = s.mass_rem_lo;
     if (s.phase <= 1) {
+        // The cut is found by warp 0: lane L owns segments 8L .. 8L+7 (64 bins).  A suffix scan over the lanes gives
+        // every lane the count and the mass ABOVE its bins; each lane then walks its own bins, highest first, and the
+        // highest lane that meets a criterion holds its cut bin (counts and masses only grow downwards).
+        constexpr int LSEG = SV_THREADS / 32;
+        dd lsum = dd_make(0.0); u64 lcnt = 0;
+        for (int t = lane * LSEG + LSEG - 1; t >= lane * LSEG; --t)
+            if (sgc[t]) { dd x; x.hi = sgh[t]; x.lo = sgl[t]; lsum = dd_add(lsum, x); lcnt += sgc[t]; }
+        dd inc = lsum; u64 cinc = lcnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            dd o; o.hi = __shfl_down_sync(0xffffffffu, inc.hi, d); o.lo = __shfl_down_sync(0xffffffffu, inc.lo, d);
+            const u64 oc = __shfl_down_sync(0xffffffffu, cinc, d);
+            if (lane + d < 32) { inc = dd_add(inc, o); cinc += oc; }
+        }
+        dd cum; cum.hi = __shfl_down_sync(0xffffffffu, inc.hi, 1); cum.lo = __shfl_down_sync(0xffffffffu, inc.lo, 1);
+        u64 cumc = __shfl_down_sync(0xffffffffu, cinc, 1);
+        if (lane == 31) { cum = dd_make(0.0); cumc = 0; }
+        dd all; all.hi = __shfl_sync(0xffffffffu, inc.hi, 0); all.lo = __shfl_sync(0xffffffffu, inc.lo, 0);   // all candidates
+        const u64 allc = __shfl_sync(0xffffffffu, cinc, 0);
         if (l0 && !s.seeded) {   // total mass S and the p-mass threshold min_mass * S (reading R5)
-            dd tot = dd_make(0.0);
-            for (int t = 0; t < SV_THREADS; ++t)
-                if (sgc[t]) { dd x; x.hi = sgh[t]; x.lo = sgl[t]; tot = dd_add(tot, x); }
+            dd tot = all;
             { dd pm; pm.hi = s.pre_hi; pm.lo = s.pre_lo; tot = dd_add(tot, pm); }
             s.total_hi = tot.hi; s.total_lo = tot.lo;
             rem = dd_make(__dmul_rn(s.min_mass, tot.hi));
         }
-        u64 cumc = 0; dd cum = dd_make(0.0);
         int dK = -1, dM = -1, dlow = -1;
         u64 aboveC_K = 0, aboveC_M = 0; dd aboveM_K = dd_make(0.0), aboveM_M = dd_make(0.0);
-        int lowest_seg = -1;
-        for (int t = 0; t < SV_THREADS && lowest_seg < 0; ++t) if (sgc[t]) lowest_seg = t;
-        for (int t = SV_THREADS - 1; t >= 0; --t) {
-            if (!sgc[t]) continue;
-            dd sgm; sgm.hi = sgh[t]; sgm.lo = sgl[t];
-            bool walk = (t == lowest_seg);                         // the lowest non-empty segment holds dlow
-            if (s.count_active && dK < 0 && cumc + sgc[t] >= s.k_rem) walk = true;
-            if (s.mass_active && dM < 0 && dd_add(cum, sgm).hi >= rem.hi - fabs(rem.hi) * 1e-12) walk = true;
-            if (!walk) { cumc += sgc[t]; cum = dd_add(cum, sgm); continue; }
-            for (int d = t * SEG + SEG - 1; d >= t * SEG; --d) {
-                const u64 c = cnt[d];
-                if (!c) continue;
-                dlow = d;
-                dd m; m.hi = mh[d]; m.lo = ml[d];
-                if (s.count_active && dK < 0 && cumc + c >= s.k_rem) { dK = d; aboveC_K = cumc; aboveM_K = cum; }
-                if (s.mass_active && dM < 0 && dd_ge(dd_add(cum, m), rem)) { dM = d; aboveC_M = cumc; aboveM_M = cum; }
-                cumc += c; cum = dd_add(cum, m);
-            }
+        for (int d = (lane * LSEG + LSEG) * SEG - 1; d >= lane * LSEG * SEG; --d) {
+            const u64 c = cnt[d];
+            if (!c) continue;
+            dlow = d;
+            dd m; m.hi = mh[d]; m.lo = ml[d];
+            if (s.count_active && dK < 0 && cumc + c >= s.k_rem) { dK = d; aboveC_K = cumc; aboveM_K = cum; }
+            if (s.mass_active && dM < 0 && dd_ge(dd_add(cum, m), rem)) { dM = d; aboveC_M = cumc; aboveM_M = cum; }
+            cumc += c; cum = dd_add(cum, m);
         }
+        {   // the highest lane that found a cut bin holds the first crossing; the lowest lane with a bin holds dlow
+            const u32 bK = __ballot_sync(0xffffffffu, dK >= 0), bM = __ballot_sync(0xffffffffu, dM >= 0);
+            const u32 bL = __ballot_sync(0xffffffffu, dlow >= 0);
+            const int lK = bK ? 31 - __clz(bK) : 0, lM = bM ? 31 - __clz(bM) : 0, lL = bL ? __ffs(bL) - 1 : 0;
+            dK = __shfl_sync(0xffffffffu, dK, lK); aboveC_K = __shfl_sync(0xffffffffu, aboveC_K, lK);
+            aboveM_K.hi = __shfl_sync(0xffffffffu, aboveM_K.hi, lK); aboveM_K.lo = __shfl_sync(0xffffffffu, aboveM_K.lo, lK);
+            dM = __shfl_sync(0xffffffffu, dM, lM); aboveC_M = __shfl_sync(0xffffffffu, aboveC_M, lM);
+            aboveM_M.hi = __shfl_sync(0xffffffffu, aboveM_M.hi, lM); aboveM_M.lo = __shfl_sync(0xffffffffu, aboveM_M.lo, lM);
+            dlow = __shfl_sync(0xffffffffu, dlow, lL);
+            if (!bK) dK = -1;
+            if (!bM) dM = -1;
+            if (!bL) dlow = -1;
+        }
+        if (lane != 0) return;
+        cumc = allc; cum = all;     // totals over the candidates, as the sequential walk would leave them
         if (dlow < 0) { s.done = s.seeded ? 3 : 1; s.PT = 0; s.KT = ~0ull; }   // no candidates at all
         else if (s.seeded && s.below_cnt > 0 && (!s.mass_active || dM < 0) && (!s.count_active || dK < 0)) {
             s.done = 3;             // the cut lies below the sampled band: the caller runs the full select
