@@ -117,6 +117,21 @@ int sv_apply_gate_truncate(sv_state *s, const int *qubits, int m, const sv_c128 
 int sv_fuse_gates(int n_gates, const int *gate_m, const int *gate_qubits, const sv_c128 *gate_U, int max_m,
                   int *n_blocks, int *block_m, int *block_qubits, sv_c128 *block_U, size_t block_U_capacity);
 
+/* Gate reordering ("we reorder the gates so that, during simulation, the set of currently active
+ * qubits is kept as small as possible, while the introduction of additional qubits is postponed for as long as the
+ * circuit dependencies allow ... we only reorder commuting gates or dependency-compatible gates").  HOST ONLY: no
+ * device work.  The paper states the goal, not an algorithm; the reading (R20) is a greedy list schedule.
+ * Two gates conflict when they share a qubit, unless both are flagged in gate_diag (nullable; gate_diag[g] != 0: U of
+ * gate g is diagonal, and diagonal gates commute).  A gate is ready once every EARLIER gate it conflicts with has been
+ * scheduled, so every conflicting pair keeps its order and the reordered list is the same operator.  A qubit is
+ * active once a scheduled gate has touched it.  Every step schedules the ready gate that activates the fewest new
+ * qubits, ties to the lowest original index.  gate_m / gate_qubits as for sv_fuse_gates (qubits < 64, distinct within
+ * a gate, any m <= 64: matrices are not needed).  Outputs (caller-owned, n_gates entries each): order[t] = index of
+ * the gate scheduled t-th; n_active_after[t] (nullable) = active qubits after it.  SV_ERR_INVALID_ARG: bad sizes, a
+ * repeated or out-of-range qubit. */
+int sv_reorder_gates(int n_gates, const int *gate_m, const int *gate_qubits, const unsigned char *gate_diag,
+                     int *order, int *n_active_after);
+
 /* *mass = sum of |a|^2 over all terms (Eq. 4) -- the mass, not its root. */
 int sv_norm(sv_state *s, double *mass);
 

@@ -19,7 +19,7 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
-           "sv_apply_gate_truncate", "sv_fuse_gates"]
+           "sv_apply_gate_truncate", "sv_fuse_gates", "sv_reorder_gates"]
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
 OPT_PRE_SLACK = 1
@@ -61,6 +61,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_truncate.argtypes = [vp, u64, dbl, C.POINTER(dbl)]
     lib.sv_fuse_gates.restype = i32
     lib.sv_fuse_gates.argtypes = [i32, vp, vp, vp, i32, C.POINTER(i32), vp, vp, vp, C.c_size_t]
+    lib.sv_reorder_gates.restype = i32
+    lib.sv_reorder_gates.argtypes = [i32, vp, vp, vp, vp, vp]
     lib.sv_apply_gate_truncate.restype = i32
     lib.sv_apply_gate_truncate.argtypes = [vp, vp, i32, vp, u64, dbl, C.POINTER(dbl)]
     lib.sv_norm.restype = i32
@@ -120,6 +122,27 @@ def fuse_gates(gates, max_m: int = 4):
         out.append(([int(x) for x in bq[qo:qo + m]], bu[uo:uo + (1 << (2 * m))].reshape(1 << m, 1 << m).copy()))
         qo += m; uo += 1 << (2 * m)
     return out
+
+
+def reorder_gates(gates, diag=None, return_active: bool = False):
+    """sv_reorder_gates: gates = sequence of (qubits, U) (U is not looked at); diag = optional sequence
+    of flags, True where a gate's matrix is diagonal.  Returns the order (list of indices into `gates`), and with
+    return_active also the number of active qubits after each scheduled gate.  Argument marshalling only."""
+    gates = list(gates)
+    if not gates:
+        return ([], []) if return_active else []
+    ms = np.array([len(q) for q, _ in gates], dtype=np.int32)
+    qs = np.ascontiguousarray(np.concatenate([np.asarray(q, dtype=np.int32) for q, _ in gates]))
+    dg = None if diag is None else np.ascontiguousarray(np.asarray(list(diag), dtype=np.uint8))
+    if dg is not None and dg.shape != (len(gates),):
+        raise ValueError("diag must have one flag per gate")
+    order = np.zeros(len(gates), dtype=np.int32)
+    act = np.zeros(len(gates), dtype=np.int32)
+    rc = lib.sv_reorder_gates(len(gates), ms.ctypes.data, qs.ctypes.data, None if dg is None else dg.ctypes.data,
+                              order.ctypes.data, act.ctypes.data)
+    if rc != SV_OK:
+        raise SvError(rc, "sv_reorder_gates: invalid gate list")
+    return (order.tolist(), act.tolist()) if return_active else order.tolist()
 
 
 class SparseSV:

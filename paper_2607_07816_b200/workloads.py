@@ -82,6 +82,19 @@ def mat_rx(theta: float) -> np.ndarray:
     return np.array([[c, complex(0, -s)], [complex(0, -s), c]], dtype=C128)
 
 
+def mat_u3(theta: float, phi: float, lam: float) -> np.ndarray:
+    """qelib1 u3(theta, phi, lambda) (PAPER.md:150-171 uses u3 and cz only)."""
+    c, sn = math.cos(0.5 * theta), math.sin(0.5 * theta)
+    if theta == math.pi:
+        c = 0.0              # cos(fl(pi)/2) rounds to 6e-17; with the exact 0, u3(pi, 0, pi) is the monomial X
+    return np.array([[c, -cmath_exp(lam) * sn],
+                     [cmath_exp(phi) * sn, cmath_exp(phi + lam) * c]], dtype=C128)
+
+
+def cmath_exp(a: float) -> complex:
+    return complex(math.cos(a), math.sin(a))
+
+
 def mat_diag_minus_last(m: int) -> np.ndarray:
     """CZ (m=2) / CCZ (m=3): identity with -1 on |1..1>."""
     d = np.ones(1 << m, dtype=C128)
@@ -267,6 +280,45 @@ def config5(n: int = 56, num_gates: int = 4000, seed: int = 4, max_terms: int = 
             gates.append(G("u8", _pick(rng, n, 3), haar_unitary(rng, 8), "gen3"))
     return Circuit("cfg5", n, gates, max_terms=max_terms, min_mass=min_mass,
                    truncate_every_gate=True, notes={"h_pool": [int(q) for q in pool]})
+
+
+def is_diagonal(U: np.ndarray) -> bool:
+    U = np.asarray(U)
+    return not np.any(U[~np.eye(U.shape[0], dtype=bool)] != 0)
+
+
+def ring_layers(rng, n: int, layers: int) -> List[Gate]:
+    """u3 + cz blocks on a ring, the SHAPE of the paper's workload ("layers of arbitrary
+    single-qubit rotations (u3), interleaved with controlled-Z (cz) entangling gates between neighboring qubits",
+    with a wrap-around coupling that closes the ring).  A block on (a, b) is u3(t, 0, -pi/2) on a, u3(t', 0, pi/2)
+    on b, cz a,b with t, t' ~ U[0, pi) drawn from the seed (the hackathon file's own angles are not available and
+    not reconstructed).  Even layers pair (0,1),(2,3),...; odd layers pair (1,2),...,(n-1,0)  [R21]."""
+    out: List[Gate] = []
+    for layer in range(layers):
+        a0 = layer % 2
+        for a in range(a0, n - 1 + a0, 2):
+            b = (a + 1) % n
+            out.append(G("u3", (a,), mat_u3(float(rng.uniform(0.0, math.pi)), 0.0, -0.5 * math.pi), "gen1"))
+            out.append(G("u3", (b,), mat_u3(float(rng.uniform(0.0, math.pi)), 0.0, 0.5 * math.pi), "gen1"))
+            out.append(G("cz", (a, b), mat_diag_minus_last(2), "diag"))
+    return out
+
+
+def ring_peaked(n: int = 44, layers: int = 4, seed: int = 5, sigma: float = 0.3, max_terms: int = 1 << 20,
+                min_mass: float = 1.0) -> Circuit:
+    """Row f-3: a peaked u3 + cz ring circuit of the paper's size (n = 44, 4 layers: 594 instructions; the paper's
+    has 580).  R = ring_layers, D = u3(theta_q ~ N(0, sigma^2), 0, 0) on every qubit, then R^dagger (cz, then the
+    inverse rotations u3(-t, -lambda, -phi)), then u3(pi, 0, pi) = X where the secret s has a 1: the state starts in
+    |0..0> and R^dagger D R is close to the identity, so the output is peaked at s."""
+    if n % 2:
+        raise ValueError("the ring pairing needs an even n")
+    rng = np.random.default_rng(seed)
+    R = ring_layers(rng, n, layers)
+    D = [G("u3", (q,), mat_u3(float(rng.normal(0.0, sigma)), 0.0, 0.0), "gen1") for q in range(n)]
+    s = int(rng.integers(0, 1 << n, dtype=np.uint64))
+    X = [G("u3", (q,), mat_u3(math.pi, 0.0, math.pi), "perm") for q in range(n) if (s >> q) & 1]
+    return Circuit("ring_peaked", n, R + D + adjoint(R) + X, max_terms=max_terms, min_mass=min_mass,
+                   truncate_every_gate=True, secret=s, notes={"layers": layers, "sigma": sigma})
 
 
 def random_state(rng: np.random.Generator, n: int, count: int, spread: float = 2.0):
