@@ -192,7 +192,43 @@ def run_circuits(engine, W, dev, torch):
                 res = {"error": str(ex)}
             sv.close()
         out[name] = res
+    out["ring44"] = run_ring_scaling(engine, W, dev, torch)
     return out
+
+
+def run_ring_scaling(engine, W, dev, torch):
+    """The paper's own experiment shape: the u3 + cz ring at n = 44 (synthetic
+    angles), reordered (sv_reorder_gates) and fused into <= 4-qubit blocks (sv_fuse_gates), one fused call per block
+    with top-k truncation, wall time against k (the paper's Fig. 2: time proportional to k).  Second of two runs."""
+    c = W.ring_peaked()
+    gates = [(list(g.qubits), g.U) for g in c.gates]
+    order = engine.reorder_gates(gates, [W.is_diagonal(U) for _, U in gates])
+    blocks = engine.fuse_gates([gates[i] for i in order], 4)
+    res = {"n_qubits": c.n, "instructions": len(gates), "blocks": len(blocks), "by_K_log2": {}}
+    for klog in (6, 12, 16, 20, 24, 26):
+        K = 1 << klog
+        torch.cuda.empty_cache()
+        free_b, _ = torch.cuda.mem_get_info(dev)
+        if engine.lib.sv_arena_bytes(16 * K) > 0.9 * free_b:
+            res["by_K_log2"][str(klog)] = {"skipped": "arena does not fit"}
+            continue
+        try:
+            for rep in range(2):
+                sv = engine.SparseSV(c.n, 16 * K, device=dev)
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(); a.record()
+                log_kept = 0.0
+                for q, U in blocks:
+                    log_kept += float(np.log(sv.apply_gate_truncate(q, U, K, 1.0)))
+                b.record(); torch.cuda.synchronize()
+                k, _, p = sv.top(1)
+                r = {"wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(), "log_retained_mass": log_kept,
+                     "top_p": float(p[0]), "top_is_secret": int(k[0]) == c.secret, "select_fallbacks": sv.stats()["fallbacks"]}
+                sv.close()
+            res["by_K_log2"][str(klog)] = r
+        except engine.SvError as ex:
+            res["by_K_log2"][str(klog)] = {"error": str(ex)}
+    return res
 
 
 # ------------------------------------------------------------------------------------------
