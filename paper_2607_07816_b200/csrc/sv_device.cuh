@@ -66,12 +66,19 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, u32 tile, u64 tot
 //   status[t]   AGG | total of tile t (never overwritten)
 //   gstat[g]    AGG | total of group g, later INCL | inclusive prefix through group g
 // Both arrays must be zero at launch.  Called by all 32 lanes of ONE warp.
+// PUBLISH = false: the tile's total has been published already (lookback_publish, by one thread, earlier), so that
+// other tiles could use it while this block went on with its next tile; this call only resolves the prefix.
+__device__ __forceinline__ void lookback_publish(u64* status, u64* gstat, u32 tile, u32 ntiles, u64 total) {
+    const u32 g = tile >> 5, r = tile & 31u;
+    st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
+    if (r == 0 && ((r == 31u) || (tile == ntiles - 1))) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | total);   // a group of one tile
+}
+template <bool PUBLISH = true>
 __device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat, u32 tile, u32 ntiles, u64 total) {
     const int lane = threadIdx.x & 31;
     const u32 g = tile >> 5, r = tile & 31u;
-    if (lane == 0) st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
+    if (PUBLISH && lane == 0) lookback_publish(status, gstat, tile, ntiles, total);
     const bool closes_group = (r == 31u) || (tile == ntiles - 1);
-    if (r == 0 && closes_group && lane == 0) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | total);   // a group of one tile
     u64 excl = 0;
     bool own_done = (r == 0);
     long long j = (long long)g - 1;          // newest group of the current window

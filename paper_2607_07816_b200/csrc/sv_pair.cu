@@ -63,8 +63,18 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     double2* La0 = reinterpret_cast<double2*>(smem_raw);       // landing amplitudes, double buffered
     double2* La1 = La0 + BP_TILE;
     u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);           // landing keys (consumed by prepare)
-    u64* Wk = Lk + BP_TILE;                                    // A* | B* keys with bit p cleared; later the staged output keys
-    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk + BP_WKN);   // their landing slots; later the staged source slots
+    u64* Wk0 = Lk + BP_TILE;                                   // A* | B* keys with bit p cleared; later the staged output keys
+    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk0 + BP_WKN);   // their landing slots; later the staged source slots
+    // PARK (general one-bit gate): a second key array, used in turns with the first, so that a tile whose outputs fit
+    // one round leaves them parked in shared memory (keys there, amplitudes in the tile's landing buffer), publishes
+    // its total at once and goes on with the block's next tile; its look-back is resolved after that tile's prepare
+    // step: the chain of L2 round trips (tile totals -> group total -> reader) has run
+    // behind that work instead of holding the whole block at a barrier.
+    constexpr bool PARK = !FIXED && MODE == 1;   // (the compacting move keeps 4 resident blocks: no room for the array)
+    u64* Wk1 = PARK ? reinterpret_cast<u64*>(Wi + BP_WKN) : Wk0;
+    bool pk_valid = false;      // uniform over the block
+    u32 pk_tile = 0; int pk_total = 0;
+    u64* pk_keys = Wk0; double2* pk_amps = La0;
     __shared__ int red[BP_WARPS + 2];
     __shared__ int wc[BP_VT][BP_WARPS];
     __shared__ int s_nA;
@@ -129,6 +139,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
         double2* La = par ? La1 : La0;          // this tile's amplitudes (by landing slot)
         double2* Lnext = par ? La0 : La1;
+        u64* Wk = par ? Wk1 : Wk0;
         const u32 next = tile + gridDim.x;
         u64 dnext = 0;
         if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
@@ -182,6 +193,23 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         }
         if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
         __syncthreads();       // A* | B* complete, every landed amplitude visible, landing keys consumed
+        if (PARK && pk_valid) {   // the previous tile's parked outputs: resolve its look-back, store coalesced
+            if (tid < 32) {
+                const u64 ex = lookback_exclusive_2level<false>(status, gstat, pk_tile, ntiles, (u64)pk_total);
+                if (tid == 0) {
+                    s_base = ex;
+                    if (pk_tile == ntiles - 1) *d_count = ex + (u64)pk_total;
+                }
+            }
+            __syncthreads();
+            const u64 base = s_base;
+            for (int idx = tid; idx < pk_total; idx += SV_THREADS) {
+                const u64 g = base + (u64)idx;
+                if (g < cap) { st_stream_u64(kout + g, pk_keys[BP_SWK(idx)]); st_stream_d2(aout + g, pk_amps[BP_SWA(idx)]); }
+            }
+            __syncthreads();   // the parked arrays are free again (the next loads land in pk_amps)
+            pk_valid = false;
+        }
         if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]), Lnext);
         const int nB = cnt - nA;
         const u64* WkB = Wk + nA;
@@ -343,6 +371,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         const int excl = block_excl_scan1(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
         // BP_ROUND outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
+        const bool park = PARK && total <= BP_ROUND;   // one round: its outputs wait in shared memory for the block's next tile
         for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {
             if (h0 > 0) __syncthreads();
             {
@@ -360,6 +389,11 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                     }
                 }
             }
+            if (park) {
+                if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);
+                pk_valid = true; pk_tile = tile; pk_total = total; pk_keys = Wk; pk_amps = La;
+                break;
+            }
             if (h0 == 0 && tid < 32) {
                 const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
                 if (tid == 0) {
@@ -375,7 +409,23 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                 if (g < cap) { st_stream_u64(kout + g, Wk[BP_SWK(idx)]); st_stream_d2(aout + g, La[BP_SWA(idx)]); }
             }
         }
-        __syncthreads();   // A* | B* and this landing buffer are reused
+        if (!park) __syncthreads();   // A* | B* and this landing buffer are reused (a parked tile's are not, until it is stored)
+    }
+    if (PARK && pk_valid) {   // the block's last tile
+        __syncthreads();
+        if (tid < 32) {
+            const u64 ex = lookback_exclusive_2level<false>(status, gstat, pk_tile, ntiles, (u64)pk_total);
+            if (tid == 0) {
+                s_base = ex;
+                if (pk_tile == ntiles - 1) *d_count = ex + (u64)pk_total;
+            }
+        }
+        __syncthreads();
+        const u64 base = s_base;
+        for (int idx = tid; idx < pk_total; idx += SV_THREADS) {
+            const u64 g = base + (u64)idx;
+            if (g < cap) { st_stream_u64(kout + g, pk_keys[BP_SWK(idx)]); st_stream_d2(aout + g, pk_amps[BP_SWA(idx)]); }
+        }
     }
     if (PRE) {   // block totals, summed in a fixed order (lanes by a fixed tree, warps ascending)
         __shared__ double s_pm[BP_WARPS];
@@ -399,7 +449,8 @@ template <int MODE, bool FIXED, bool PRE>
 static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                           const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
-    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2);   // amplitudes x 2, landing keys, A* | B* keys, slots
+    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2) +
+                        ((!FIXED && MODE == 1) ? (size_t)BP_WKN * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
     static bool attr = false;
     if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
     static int per_sm = 0;
