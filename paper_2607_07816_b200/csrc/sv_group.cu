@@ -272,19 +272,11 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
 #pragma unroll
         for (int v = 0; v < BP_VT; ++v)
             if (e0 + v < cnt) s_info[e0 + v] = t_info[v];
-        if (tid < 32) {
-            const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
-            if (tid == 0) {
-                s_base = ex;
-                if (tile == ntiles - 1) d_count[0] = ex + (u64)total;
-            }
-        }
-        __syncthreads();
         // ---- phase 2b: one thread per OUTPUT: consecutive threads write consecutive entries.  Outputs are
         // taken GP_ROUND at a time: the opening terms first post (term, row) for each of their outputs of
-        // the round in s_owner, then every thread computes the outputs t, t + 256, ... of the round ----
-        const u64 base = s_base;
-        for (int h0 = 0; h0 < total; h0 += GP_ROUND) {
+        // the round in s_owner, then every thread computes the outputs t, t + 256, ... of the round.  The
+        // first round is posted while warp 0 resolves the look-back (one barrier for both) ----
+        auto post_round = [&](int h0) {
             if (excl < h0 + GP_ROUND && excl + mycount > h0) {
                 int off = excl - h0;
 #pragma unroll
@@ -298,7 +290,20 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                     }
                 }
             }
-            __syncthreads();
+        };
+        if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);
+        post_round(0);
+        if (tid < 32) {
+            const u64 ex = lookback_exclusive_2level<false>(status, gstat, tile, ntiles, (u64)total);
+            if (tid == 0) {
+                s_base = ex;
+                if (tile == ntiles - 1) d_count[0] = ex + (u64)total;
+            }
+        }
+        __syncthreads();
+        const u64 base = s_base;
+        for (int h0 = 0; h0 < total; h0 += GP_ROUND) {
+            if (h0 > 0) { post_round(h0); __syncthreads(); }
             const int m = min(total - h0, GP_ROUND);
             for (int q = tid; q < m; q += SV_THREADS) {
                 const u32 code = s_owner[q];
