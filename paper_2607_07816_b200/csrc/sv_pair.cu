@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
         // BP_ROUND outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
         const bool park = PARK && total <= BP_ROUND;   // one round: its outputs wait in shared memory for the block's next tile
+        if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);   // at once: the later tiles read it while this one stages
         for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {
             if (h0 > 0) __syncthreads();
             {
@@ -390,12 +391,11 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                 }
             }
             if (park) {
-                if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);
                 pk_valid = true; pk_tile = tile; pk_total = total; pk_keys = Wk; pk_amps = La;
                 break;
             }
             if (h0 == 0 && tid < 32) {
-                const u64 ex = lookback_exclusive_2level(status, gstat, tile, ntiles, (u64)total);
+                const u64 ex = lookback_exclusive_2level<false>(status, gstat, tile, ntiles, (u64)total);
                 if (tid == 0) {
                     s_base = ex;
                     if (tile == ntiles - 1) *d_count = ex + (u64)total;
