@@ -5,6 +5,8 @@
 #define SV_FLAG_AGG  (1ull << 62)
 #define SV_FLAG_INCL (2ull << 62)
 #define SV_VAL_MASK  ((1ull << 62) - 1)
+#define SV_GRP_ONE   (1ull << 48)            // two-level look-back: one tile's contribution to its group's counter
+#define SV_GRP_VAL   ((1ull << 48) - 1)
 
 __device__ __forceinline__ u64 ld_relaxed_u64(const u64* p) {
     u64 v;
@@ -60,25 +62,29 @@ __device__ __forceinline__ u64 lookback_exclusive(u64* status, u32 tile, u64 tot
 // one tile every ~15 cycles -- more than such a chain can carry.  Here tiles are grouped by
 // 32.  A tile adds (a) the totals of the tiles before it in its own group and (b) a windowed
 // look-back over GROUP statuses, 32 groups (1024 tiles) per round trip; both polls are in
-// flight together.  The last tile of a group (by index) knows the group's total once (a) is
-// complete and publishes it; the first tile of the next group later upgrades it to the
-// inclusive prefix.  No atomics, one store to publish, one or two polls to resolve.
+// flight together.  A group's total is gathered by its tiles themselves (one atomic add each: value
+// and a count of contributions), so it is complete one round trip after the last of them published
+// -- no tile has to close the group; the first tile of the next group later upgrades it to the
+// inclusive prefix.  One store and one atomic add to publish, one or two polls to resolve.
 //   status[t]   AGG | total of tile t (never overwritten)
-//   gstat[g]    AGG | total of group g, later INCL | inclusive prefix through group g
+//   gstat[g]    sum of the totals published so far (bits 0..47) | how many (bits 48..55; complete at 32),
+//               later INCL | inclusive prefix through group g
 // Both arrays must be zero at launch.  Called by all 32 lanes of ONE warp.
 // PUBLISH = false: the tile's total has been published already (lookback_publish, by one thread, earlier), so that
 // other tiles could use it while this block went on with its next tile; this call only resolves the prefix.
 __device__ __forceinline__ void lookback_publish(u64* status, u64* gstat, u32 tile, u32 ntiles, u64 total) {
     const u32 g = tile >> 5, r = tile & 31u;
+    (void)r; (void)ntiles;
     st_relaxed_u64(&status[tile], SV_FLAG_AGG | total);
-    if (r == 0 && ((r == 31u) || (tile == ntiles - 1))) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | total);   // a group of one tile
+    // the group's total is gathered by its 32 tiles themselves: value in bits 0..47, number of tiles that have added
+    // theirs in bits 48..55 -- complete, for any reader, one L2 round trip after the last of them published
+    atomicAdd(reinterpret_cast<unsigned long long*>(&gstat[g]), (unsigned long long)(total + SV_GRP_ONE));
 }
 template <bool PUBLISH = true>
 __device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat, u32 tile, u32 ntiles, u64 total) {
     const int lane = threadIdx.x & 31;
     const u32 g = tile >> 5, r = tile & 31u;
     if (PUBLISH && lane == 0) lookback_publish(status, gstat, tile, ntiles, total);
-    const bool closes_group = (r == 31u) || (tile == ntiles - 1);
     u64 excl = 0;
     bool own_done = (r == 0);
     long long j = (long long)g - 1;          // newest group of the current window
@@ -95,16 +101,16 @@ __device__ __forceinline__ u64 lookback_exclusive_2level(u64* status, u64* gstat
                 for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
                 excl += c;
                 own_done = true;
-                if (closes_group && lane == 0) st_relaxed_u64(&gstat[g], SV_FLAG_AGG | (c + total));
             }
         }
         if (!groups_done) {
-            const u32 flagged = __ballot_sync(0xffffffffu, (v2 >> 62) != 0);
+            // a group before this tile's own always has 32 tiles: its total is complete when all 32 have added theirs
+            const u32 flagged = __ballot_sync(0xffffffffu, (v2 >> 62) == 2 || ((v2 >> 48) & 0xffull) == 32ull);
             const u32 incl = __ballot_sync(0xffffffffu, (v2 >> 62) == 2);
             const int first = incl ? (__ffs(incl) - 1) : 32;
             const u32 need = (first >= 31) ? 0xffffffffu : ((2u << first) - 1u);
             if ((flagged & need) == need) {
-                u64 c = (lane <= first) ? (v2 & SV_VAL_MASK) : 0;
+                u64 c = (lane <= first) ? (v2 & SV_GRP_VAL) : 0;
 #pragma unroll
                 for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
                 excl += c;
