@@ -151,13 +151,11 @@ int sv_load(sv_state *s, const uint64_t *keys, const sv_c128 *amps, uint64_t n);
 /* Same with DEVICE source arrays (no host copy; used to time device-resident input). */
 int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amps, uint64_t n);
 
-/* Tuning knobs.  SV_OPT_SAMPLE_MIN_TERMS: states with at least this many terms find the
+/* Tuning knob.  SV_OPT_SAMPLE_MIN_TERMS: states with at least this many terms find the
  * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^21), smaller
  * ones with the full-state radix select.  Both are exact; tests force either.  The same threshold gates the
- * output floor of sv_apply_gate_truncate.  SV_OPT_PRE_SLACK (an int64 passed as uint64, default 0): sample
- * points added to that floor's safety margin; a negative value makes the margin fail so that tests reach the
- * re-run path. */
-enum { SV_OPT_SAMPLE_MIN_TERMS = 0, SV_OPT_PRE_SLACK = 1 };
+ * output floor of sv_apply_gate_truncate. */
+enum { SV_OPT_SAMPLE_MIN_TERMS = 0 };
 int sv_set_option(sv_state *s, int option, uint64_t value);
 
 /* Statistics of the last call and the launch counter. */

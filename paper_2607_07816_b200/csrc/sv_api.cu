@@ -67,7 +67,7 @@ struct sv_state {
     bool fuse_on;           // sv_apply_gate runs on behalf of sv_apply_gate_truncate
     bool diag_deferred;     // the diagonal gate in s->tab (and the pending cut) has not been applied yet: the truncation's
                             // classification pass applies it in place (sv_sample_select.cu, XF)
-    long long pre_slack;    // SV_OPT_PRE_SLACK: sample points added to the floor's margin (tests force a failed margin with < 0)
+    long long pre_slack;    // sv_test_set_pre_slack: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
 
@@ -93,14 +93,20 @@ static void prof_slot(sv_state* s, int id, double bytes, cudaEvent_t* e0, cudaEv
     s->npend += 1;
 }
 
-int sv_sm_count() {
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+int sv_cur_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) dev = 0;
+    return dev < SV_MAX_DEV ? dev : SV_MAX_DEV - 1;
+}
+int sv_sm_count() {   // per device; concurrent first calls write the same value
+    static int n[SV_MAX_DEV];
+    const int dev = sv_cur_device();
+    if (!n[dev]) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v < 1) v = 148;
+        n[dev] = v;
     }
-    return n;
+    return n[dev];
 }
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -143,16 +149,17 @@ static int cuda_fail(sv_state* s, cudaError_t e, const char* where) {
         cudaError_t e__ = (call);                                          \
         if (e__ != cudaSuccess) return cuda_fail(s, e__, #call);           \
     } while (0)
-// SV_DEBUG_SYNC=1 in the environment: synchronise after every kernel of the truncation path and name the
-// first one that failed (compute-sanitizer is not available on every box).
-static bool dbg_sync_on() { static int v = -1; if (v < 0) v = getenv("SV_DEBUG_SYNC") ? 1 : 0; return v == 1; }
+// Debug builds only (-DSV_DEBUG_SYNC): synchronise after every kernel of the truncation path and name the first
+// one that failed.  The release library has no such code path.
+#ifdef SV_DEBUG_SYNC
 #define DBG_SYNC(tag)                                                                            \
     do {                                                                                         \
-        if (dbg_sync_on()) {                                                                     \
-            cudaError_t e__ = cudaStreamSynchronize(s->stream);                                  \
-            if (e__ != cudaSuccess) { fprintf(stderr, "[sv debug] %s: %s\n", tag, cudaGetErrorString(e__)); return cuda_fail(s, e__, tag); } \
-        }                                                                                        \
+        cudaError_t e__ = cudaStreamSynchronize(s->stream);                                      \
+        if (e__ != cudaSuccess) return cuda_fail(s, e__, tag);                                   \
     } while (0)
+#else
+#define DBG_SYNC(tag) do { } while (0)
+#endif
 #define CHECK_LAUNCH()                                                     \
     do {                                                                   \
         cudaError_t e__ = cudaGetLastError();                              \
@@ -307,8 +314,13 @@ extern "C" int sv_profile_get(sv_state* s, int kernel, sv_kernel_prof* out) {
 extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
-    if (option == SV_OPT_PRE_SLACK) { s->pre_slack = (long long)value; return SV_OK; }
     return fail(s, SV_ERR_INVALID_ARG, "unknown option");
+}
+// test hook (include/sparse_sv_test.h): sample points added to the margin of the fused call's output floor
+extern "C" int sv_test_set_pre_slack(sv_state* s, long long slack) {
+    if (!s) return SV_ERR_INVALID_ARG;
+    s->pre_slack = slack;
+    return SV_OK;
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
     if (!s || !out) return SV_ERR_INVALID_ARG;
@@ -416,7 +428,9 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     if (ma == 0)
         for (int c = 0; c < d; ++c) if (is_zero(U[c * d + c])) diag_nonzero = false;
 
-    if ((ma == 0 && diag_nonzero) || xor_class) {
+    // (ma == 0 with an exact zero on the diagonal -- a projector: U is not required to be unitary -- is still a diagonal
+    // gate; the terms it annihilates are dropped: they become dead entries and are counted below.)
+    if (ma == 0 || xor_class) {
         // phase table in stored patterns: every gate bit acts as a control of a diagonal
         tab.ma = 0; tab.mc = m;
         for (int j = 0; j < m; ++j) tab.ctrl_pos[j] = s->phys_of_log[qubits[j]];
@@ -440,7 +454,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
                                                       s->tab, s->defer, s->status, s->tile_counter, s->d_count, s->stream);
                 if (e1) cudaEventRecord(e1, s->stream);
                 s->cur = alt; s->phys = s->count; s->defer.active = 0;
-            } else if (s->fuse_on && s->count >= s->sample_min_terms && s->phys / 8 >= 64) {
+            } else if (diag_nonzero && s->fuse_on && s->count >= s->sample_min_terms && s->phys / 8 >= 64) {
                 // fused call: the sampled truncation that follows applies the gate in its own pass over the state
                 s->diag_deferred = true;
             } else {
@@ -449,9 +463,21 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
             }
             CHECK_LAUNCH();
             s->stats.passes = 1;
+            if (!diag_nonzero) {   // singular diagonal: count what is left
+                s->stats.launches += svk_count_live(s->amps[s->cur], s->phys, s->d_count, s->stream);
+                CHECK_LAUNCH();
+                u64 live = 0;
+                int rcl = read_back(s, &live, s->d_count, sizeof(u64));
+                if (rcl != SV_OK) return rcl;
+                s->count = live;
+                if (live == 0) s->phys = 0;
+                s->mass_est = nan("");
+                s->stats.n_out = live;
+            }
         }
         return SV_OK;
     }
+    if (ma < 1) return fail(s, SV_ERR_INVALID_ARG, "internal: gate without an active qubit in the group class");
 
     // GROUP class.  The active bits must occupy physical positions 0..ma-1.  Those already
     // forming a prefix {0..k-1} stay; the others are moved to the LSB one pass each, the
@@ -757,7 +783,7 @@ extern "C" int sv_truncate(sv_state* s, uint64_t max_terms, double min_mass, dou
     int rc = SV_OK;
     if (s->defer.active && !s->diag_deferred) rc = materialize(s);   // a second truncation in a row: apply the first one now
     if (rc != SV_OK) return rc;
-    if (dbg_sync_on()) { DBG_SYNC("before select"); fprintf(stderr, "[sv debug] truncate: count=%llu phys=%llu cap=%llu cur=%d defer=%d\n", (unsigned long long)s->count, (unsigned long long)s->phys, (unsigned long long)s->cap, s->cur, s->defer.active); }
+    DBG_SYNC("before select");
     SelState ss;
     rc = run_select(s, max_terms, min_mass, &ss);
     if (rc != SV_OK) return rc;
@@ -821,6 +847,13 @@ extern "C" int sv_check_invariants(sv_state* s, int* ok) {
 // ---------------------------------------------------------------------------------------
 // readout (row a-11): select k, gather, order by (p desc, key asc), copy to the host
 // ---------------------------------------------------------------------------------------
+// `bytes` of scratch inside the idle amplitude buffer, behind its first `keep` bytes; nullptr if they do not fit.
+static unsigned char* arena_scratch(sv_state* s, size_t keep, size_t bytes) {
+    const size_t room = (size_t)s->cap * 16;
+    keep = align_up(keep);
+    if (keep > room || bytes > room - keep) return nullptr;
+    return reinterpret_cast<unsigned char*>(s->amps[s->cur ^ 1]) + keep;
+}
 struct TmpBuf {
     void* p = nullptr;
     ~TmpBuf() { if (p) cudaFree(p); }
@@ -843,9 +876,15 @@ extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, do
     }
     const size_t a8 = align_up(kk * 8), a16 = align_up(kk * 16), a4 = align_up(kk * 4);
     const size_t sscr = align_up(svk_sort_scratch_bytes(kk));
+    // scratch: the idle amplitude buffer of the arena when the readout fits there (always for a small k), else a
+    // temporary allocation (full exports)
     TmpBuf tb;
-    if (tb.alloc(a8 * 6 + a16 * 2 + a4 * 2 + sscr) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_top: scratch allocation failed"); }
-    unsigned char* b = (unsigned char*)tb.p;
+    const size_t need = a8 * 6 + a16 * 2 + a4 * 2 + sscr;
+    unsigned char* b = arena_scratch(s, 0, need);
+    if (!b) {
+        if (tb.alloc(need) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_top: scratch allocation failed"); }
+        b = (unsigned char*)tb.p;
+    }
     u64* pat = (u64*)b; b += a8;
     u64* lkey = (u64*)b; b += a8;
     u64* ka = (u64*)b; b += a8;
@@ -895,8 +934,8 @@ extern "C" int sv_top(sv_state* s, uint64_t k, uint64_t* keys, sv_c128* amps, do
 // ---------------------------------------------------------------------------------------
 // load: establish the sorted storage order with the radix sort
 // ---------------------------------------------------------------------------------------
-extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c128* dev_amps, uint64_t n) {
-    if (!s || (n && (!dev_keys || !dev_amps))) return SV_ERR_INVALID_ARG;
+// staged: dev_keys / dev_amps live in the arena scratch behind `staged_bytes` of the idle amplitude buffer (sv_load)
+static int load_device_impl(sv_state* s, const uint64_t* dev_keys, const sv_c128* dev_amps, uint64_t n, size_t dest_and_staged_bytes) {
     s->err[0] = 0;
     if (n > s->cap) return fail(s, SV_ERR_INVALID_ARG, "sv_load: n exceeds capacity");
     if (n >= (1ull << 32)) return fail(s, SV_ERR_INVALID_ARG, "sv_load supports n < 2^32");
@@ -904,9 +943,13 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
     const int alt = s->cur ^ 1;
     if (n > 0) {
         const size_t a8 = align_up(n * 8), a4 = align_up(n * 4);
+        const size_t need = a8 * 2 + a4 * 2 + align_up(svk_sort_scratch_bytes(n));
         TmpBuf tb;
-        if (tb.alloc(a8 * 2 + a4 * 2 + align_up(svk_sort_scratch_bytes(n))) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: scratch allocation failed"); }
-        unsigned char* b = (unsigned char*)tb.p;
+        unsigned char* b = arena_scratch(s, dest_and_staged_bytes, need);   // behind the destination (and the staged input)
+        if (!b) {
+            if (tb.alloc(need) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: scratch allocation failed"); }
+            b = (unsigned char*)tb.p;
+        }
         u64* ka = (u64*)b; b += a8;
         u64* kb = (u64*)b; b += a8;
         u32* va = (u32*)b; b += a4;
@@ -921,7 +964,7 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
         s->stats.launches += svk_check(s->keys[alt], s->amps[alt], n, s->n, s->d_bad, st);
         CHECK_LAUNCH();
         int bad = 0;
-        int rc = read_back(s, &bad, s->d_bad, sizeof(int));
+        int rc = read_back(s, &bad, s->d_bad, sizeof(int));   // (synchronises: a temporary allocation may go now)
         if (rc != SV_OK) return rc;
         if (bad) return fail(s, SV_ERR_INVALID_ARG, "sv_load: duplicate key, key >= 2^n or zero amplitude (state unchanged)");
     }
@@ -941,16 +984,31 @@ extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c1
     return SV_OK;
 }
 
+extern "C" int sv_load_device(sv_state* s, const uint64_t* dev_keys, const sv_c128* dev_amps, uint64_t n) {
+    if (!s || (n && (!dev_keys || !dev_amps))) return SV_ERR_INVALID_ARG;
+    return load_device_impl(s, dev_keys, dev_amps, n, (size_t)n * 16);
+}
+
 extern "C" int sv_load(sv_state* s, const uint64_t* keys, const sv_c128* amps, uint64_t n) {
     if (!s || (n && (!keys || !amps))) return SV_ERR_INVALID_ARG;
     if (n > s->cap) return fail(s, SV_ERR_INVALID_ARG, "sv_load: n exceeds capacity");
-    TmpBuf tk, ta;
-    if (tk.alloc(n * 8) != 0 || ta.alloc(n * 16) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: staging allocation failed"); }
-    if (n) {
-        CU(cudaMemcpyAsync(tk.p, keys, n * 8, cudaMemcpyHostToDevice, s->stream));
-        CU(cudaMemcpyAsync(ta.p, amps, n * 16, cudaMemcpyHostToDevice, s->stream));
+    // staging of the host arrays: in the idle amplitude buffer behind the destination when it fits, else temporary
+    const size_t a8 = align_up(n * 8), a16 = align_up(n * 16);
+    TmpBuf tb;
+    size_t behind = a16;
+    unsigned char* stg = arena_scratch(s, a16, a8 + a16);
+    if (stg) behind = a16 + a8 + a16;
+    else {
+        if (tb.alloc(a8 + a16) != 0) { cudaGetLastError(); return fail(s, SV_ERR_NOMEM, "sv_load: staging allocation failed"); }
+        stg = (unsigned char*)tb.p;
     }
-    int rc = sv_load_device(s, (const uint64_t*)tk.p, (const sv_c128*)ta.p, n);
+    uint64_t* dk = (uint64_t*)stg;
+    sv_c128* da = (sv_c128*)(stg + a8);
+    if (n) {
+        CU(cudaMemcpyAsync(dk, keys, n * 8, cudaMemcpyHostToDevice, s->stream));
+        CU(cudaMemcpyAsync(da, amps, n * 16, cudaMemcpyHostToDevice, s->stream));
+    }
+    int rc = load_device_impl(s, dk, da, n, behind);
     cudaStreamSynchronize(s->stream);
     return rc;
 }

@@ -57,9 +57,8 @@ void absorb(Block& b, const Cx* G, int mg, const int* pos) {
     }
     b.U.swap(V);
 }
-}  // namespace
 
-extern "C" int sv_fuse_gates(int n_gates, const int* gate_m, const int* gate_qubits, const sv_c128* gate_U, int max_m,
+int fuse_impl(int n_gates, const int* gate_m, const int* gate_qubits, const sv_c128* gate_U, int max_m,
                              int* n_blocks, int* block_m, int* block_qubits, sv_c128* block_U, size_t block_U_capacity) {
     if (n_gates < 0 || max_m < 1 || max_m > SV_FUSE_MAX_M || !n_blocks || (n_gates && (!gate_m || !gate_qubits || !gate_U)) ||
         (n_gates && (!block_m || !block_qubits || !block_U)))
@@ -105,4 +104,15 @@ extern "C" int sv_fuse_gates(int n_gates, const int* gate_m, const int* gate_qub
         qoff += mg; uoff += (size_t)1 << (2 * mg);
     }
     return flush();
+}
+}  // namespace
+
+// (std::vector may throw: no C++ exception crosses the C ABI)
+extern "C" int sv_fuse_gates(int n_gates, const int* gate_m, const int* gate_qubits, const sv_c128* gate_U, int max_m,
+                             int* n_blocks, int* block_m, int* block_qubits, sv_c128* block_U, size_t block_U_capacity) {
+    try {
+        return fuse_impl(n_gates, gate_m, gate_qubits, gate_U, max_m, n_blocks, block_m, block_qubits, block_U, block_U_capacity);
+    } catch (...) {
+        return SV_ERR_NOMEM;
+    }
 }

@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(SV_THREADS) diag_kernel(const u64* __restrict_
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st) {
     if (n == 0) return 0;
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (blocks > 148ull * 16) blocks = 148ull * 16;
+    if (blocks > (u64)sv_sm_count() * 16) blocks = (u64)sv_sm_count() * 16;
     diag_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, tab);
     return 1;
 }

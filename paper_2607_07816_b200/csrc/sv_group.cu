@@ -14,6 +14,7 @@
 //     directly, consecutive threads writing consecutive entries.  A row that cancels to exactly 0+0i is written as a dead entry
 //     (counted, so the term count stays exact) instead of forcing a second scan.
 #include "sv_tile.cuh"
+#include "sv_launch.cuh"
 
 //
 // PRE (fused apply + truncate, sv_presample.cu): outputs whose probability pattern is below pre->P_floor are not
@@ -361,16 +362,9 @@ static u32 launch_grouppass(const u64* kin, const double2* ain, u64* kout, doubl
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
     const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 8 + (size_t)GP_ROUND * 2;   // landing + work + tuple table + owners
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(grouppass_kernel<MA, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
-    static int per_sm = 0;
-    if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, grouppass_kernel<MA, PRE>, SV_THREADS, smem);
-        if (per_sm < 1) per_sm = 1;
-    }
-    const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    grouppass_kernel<MA, PRE><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles,
-                                                                    pre, pre_mass, pre_cnt);
+    static int per_sm[SV_MAX_DEV];
+    const u32 grid = sv_launch_persistent(grouppass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
+                                          (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt);
     return grid;
 }
 

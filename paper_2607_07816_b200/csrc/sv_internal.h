@@ -91,7 +91,10 @@ struct PendPred {
     KeyMap km;
 };
 
-int sv_sm_count();   // SMs of the current device (cached)
+#define SV_MAX_DEV 64
+int sv_cur_device(); // ordinal of the current device, clamped to SV_MAX_DEV - 1 (index of the per-device caches)
+int sv_sm_count();   // SMs of the current device (cached per device)
+int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);

@@ -28,6 +28,7 @@
 //             exact zeros are dropped, block scan + two-level look-back give the
 //             offsets, outputs are staged and stored coalesced: sorted, unique keys by construction.
 #include "sv_tile.cuh"
+#include "sv_launch.cuh"
 
 // MODE 0: pure move.  MODE 1: gate with one active bit (2x2 mat-vec per tuple).  MODE 2 (FIXED only):
 // the same for MONOMIAL 2x2 blocks: every entry maps to one entry (its bit kept or flipped, times a
@@ -451,16 +452,9 @@ static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2
                           const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
     const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2) +
                         ((!FIXED && MODE == 1) ? (size_t)BP_WKN * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(bitpass_kernel<MODE, FIXED, PRE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
-    static int per_sm = 0;
-    if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, bitpass_kernel<MODE, FIXED, PRE>, SV_THREADS, smem);
-        if (per_sm < 1) per_sm = 1;
-    }
-    const u32 grid = min(ntiles, (u32)(sv_sm_count() * per_sm));
-    bitpass_kernel<MODE, FIXED, PRE><<<grid, SV_THREADS, smem, st>>>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles,
-                                                                     pre, pre_mass, pre_cnt);
+    static int per_sm[SV_MAX_DEV];
+    const u32 grid = sv_launch_persistent(bitpass_kernel<MODE, FIXED, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
+                                          (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt);
     return grid;
 }
 

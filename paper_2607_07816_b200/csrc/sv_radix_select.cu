@@ -19,6 +19,7 @@
 // cannot overflow.  Integer sums are order independent: every run takes bit-identical
 // decisions (D3).  The decisions are taken by one thread in double-double.
 #include "sv_device.cuh"
+#include "sv_launch.cuh"
 
 // ---------------------------------------------------------------------------------------
 // double-double helpers (cut decisions only; one thread)
@@ -200,10 +201,10 @@ __global__ void __launch_bounds__(SV_THREADS) sel_pass_kernel(const double2* __r
 template <int MODE>
 static int launch_pass(const double2* amps, const u64* lkeys, u64 n, const SelState* ss, u64* hist, cudaStream_t st) {
     const size_t smem = (size_t)RS_BINS * (5 * 4 + (MODE < 2 ? 16 : 0));
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(sel_pass_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    static bool attr[SV_MAX_DEV];
+    sv_set_smem_once(sel_pass_kernel<MODE>, smem, attr);
     u64 blocks = (n + SV_THREADS * SP_IT - 1) / (SV_THREADS * SP_IT);
-    const u64 maxb = 148ull * (MODE < 2 ? 3 : 4);
+    const u64 maxb = (u64)sv_sm_count() * (MODE < 2 ? 3 : 4);
     if (blocks > maxb) blocks = maxb;
     if (blocks < 1) blocks = 1;
     sel_pass_kernel<MODE><<<(unsigned)blocks, SV_THREADS, smem, st>>>(amps, lkeys, n, ss, hist);
@@ -264,7 +265,7 @@ __global__ void __launch_bounds__(SV_THREADS) sel_extract_kernel(const u64* __re
 int svk_sel_extract(const u64* keys, const double2* amps, u64 n, const SelState* ss, KeyMap km, u64* lk_out, u64* hist,
                     cudaStream_t st) {
     u64 blocks = (n + SV_THREADS * SP_IT - 1) / (SV_THREADS * SP_IT);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
     if (blocks < 1) blocks = 1;
     sel_extract_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ss, km, lk_out, hist);
     return 1;
@@ -544,8 +545,8 @@ __global__ void __launch_bounds__(SV_THREADS) sel_step_kernel(SelState* ssp, u64
 }
 int svk_sel_step(SelState* ss, u64* hist, cudaStream_t st, int expected_phase) {
     const size_t smem = (size_t)H_TOTAL * 8 + (size_t)RS_BINS * 16 + (size_t)SV_THREADS * 24;
-    static bool attr = false;
-    if (!attr) { cudaFuncSetAttribute(sel_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr = true; }
+    static bool attr[SV_MAX_DEV];
+    sv_set_smem_once(sel_step_kernel, smem, attr);
     sel_step_kernel<<<1, SV_THREADS, smem, st>>>(ss, hist, expected_phase);
     return 1;
 }

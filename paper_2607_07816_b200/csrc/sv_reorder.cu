@@ -15,8 +15,8 @@
 
 #include "../../include/sparse_sv.h"
 
-extern "C" int sv_reorder_gates(int n_gates, const int* gate_m, const int* gate_qubits, const unsigned char* gate_diag,
-                                int* order, int* n_active_after) {
+static int reorder_impl(int n_gates, const int* gate_m, const int* gate_qubits, const unsigned char* gate_diag,
+                        int* order, int* n_active_after) {
     if (n_gates < 0 || (n_gates && (!gate_m || !gate_qubits || !order))) return SV_ERR_INVALID_ARG;
     std::vector<uint64_t> qmask((size_t)n_gates, 0);
     {
@@ -69,4 +69,14 @@ extern "C" int sv_reorder_gates(int n_gates, const int* gate_m, const int* gate_
         if (n_active_after) n_active_after[step] = __builtin_popcountll(active);
     }
     return SV_OK;
+}
+
+// (std::vector may throw: no C++ exception crosses the C ABI)
+extern "C" int sv_reorder_gates(int n_gates, const int* gate_m, const int* gate_qubits, const unsigned char* gate_diag,
+                                int* order, int* n_active_after) {
+    try {
+        return reorder_impl(n_gates, gate_m, gate_qubits, gate_diag, order, n_active_after);
+    } catch (...) {
+        return SV_ERR_NOMEM;
+    }
 }

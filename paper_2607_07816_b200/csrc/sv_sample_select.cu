@@ -25,6 +25,7 @@
 // a reference exponent, and integers are added -- the sums do not depend on the order in
 // which threads or blocks add them.
 #include "sv_tile.cuh"
+#include "sv_launch.cuh"
 
 typedef unsigned __int128 u128;
 
@@ -323,11 +324,8 @@ int svk_ss_pivot(const u64* smp_sorted, u32 M, u64 n_live, u64 max_terms, double
 template <bool XF>
 static void launch_classify(const u64* keys, const double2* amps, u64 n, SampleCtl* ctl, u64* ckeys, double2* camps, unsigned char* seg_cnt,
                             cudaStream_t st, double2* amps_rw, const PendPred& pd, const GateTab* tab) {
-    static int per_sm = 0;   // one wave of resident blocks: a grid-stride loop has no tail
-    if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_classify_kernel<XF>, SV_THREADS, 0);
-        if (per_sm < 1) per_sm = 1;
-    }
+    static int per_sm_c[SV_MAX_DEV];   // one wave of resident blocks: a grid-stride loop has no tail
+    const int per_sm = sv_blocks_per_sm(ss_classify_kernel<XF>, 0, per_sm_c);
     u64 blocks = (n + SV_THREADS * SC_IT - 1) / (SV_THREADS * SC_IT);
     if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
     if (blocks < 1) blocks = 1;
@@ -399,11 +397,8 @@ int svk_ss_band_compact(const u64* keys, const double2* amps, u64 n, const Sampl
     const u32 nchunks = (u32)((n + chunk - 1) / chunk);
     ss_chunk_sum_kernel<<<(nchunks + 255) / 256, 256, 0, st>>>(seg_cnt, (n + 31) >> 5, nchunks, chunk_cnt);
     int launches = 1 + svk_scan_u32(chunk_cnt, nchunks, scan_status, tile_counter, st);
-    static int per_sm = 0;
-    if (!per_sm) {
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ss_band_compact_kernel, SV_THREADS, 0);
-        if (per_sm < 1) per_sm = 1;
-    }
+    static int per_sm_c[SV_MAX_DEV];
+    const int per_sm = sv_blocks_per_sm(ss_band_compact_kernel, 0, per_sm_c);
     u64 blocks = nchunks;
     if (blocks > (u64)sv_sm_count() * per_sm) blocks = (u64)sv_sm_count() * per_sm;
     ss_band_compact_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ctl, seg_cnt, chunk_cnt, kout, aout);

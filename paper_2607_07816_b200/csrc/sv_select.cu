@@ -43,6 +43,28 @@ int svk_norm(const double2* amps, u64 n, double* partials, double* d_out, cudaSt
     return 2;
 }
 
+// Number of live entries (amplitude != 0+0i) -> *d_count.  Used after a diagonal gate with exact zeros on its
+// diagonal (a projector): the terms it annihilates are dropped, i.e. become dead entries.
+__global__ void __launch_bounds__(SV_THREADS) count_live_kernel(const double2* __restrict__ amps, u64 n, u64* d_count) {
+    u64 c = 0;
+    const u64 stride = (u64)gridDim.x * blockDim.x;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const double2 a = ld_stream_d2(amps + i);
+        c += (a.x == 0.0 && a.y == 0.0) ? 0 : 1;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(reinterpret_cast<unsigned long long*>(d_count), (unsigned long long)c);
+}
+int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st) {
+    cudaMemsetAsync(d_count, 0, sizeof(u64), st);
+    if (n == 0) return 0;
+    u64 blocks = (n + SV_THREADS * 8 - 1) / (SV_THREADS * 8);
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
+    count_live_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(amps, n, d_count);
+    return 1;
+}
+
 // ---------------------------------------------------------------------------------------
 // a-9 cut + renormalise: stable compaction of the kept prefix, scale fused
 // ---------------------------------------------------------------------------------------
@@ -201,7 +223,7 @@ __global__ void __launch_bounds__(SV_THREADS) diag_pend_kernel(const u64* __rest
 int svk_diag_pend(const u64* keys, double2* amps, u64 n, const GateTab* tab, int has_phase, const PendPred& pend, cudaStream_t st) {
     if (n == 0) return 0;
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (blocks > 148ull * 8) blocks = 148ull * 8;
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
     diag_pend_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, pend, tab, has_phase);
     return 1;
 }
@@ -231,7 +253,7 @@ int svk_gather_top(const u64* keys, const double2* amps, u64 n, const SelState* 
     cudaMemsetAsync(d_count, 0, sizeof(u64), st);
     if (n == 0) return 0;
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
     gather_top_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, ss, use_sel, km, o_pat, o_lkey, o_amp,
                                                                d_count, kmax);
     return 1;
@@ -256,7 +278,7 @@ int svk_check(const u64* keys, const double2* amps, u64 n, int nq, int* d_bad, c
     cudaMemsetAsync(d_bad, 0, sizeof(int), st);
     if (n == 0) return 0;
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
     check_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, nq, d_bad);
     return 1;
 }

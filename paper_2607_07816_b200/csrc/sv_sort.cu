@@ -158,7 +158,7 @@ __global__ void pat_to_prob_kernel(const u64* __restrict__ pat, double* __restri
 }
 static unsigned grid_for(u64 n) {
     u64 b = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (b > 148 * 8) b = 148 * 8;
+    if (b > (u64)sv_sm_count() * 8) b = (u64)sv_sm_count() * 8;
     if (b < 1) b = 1;
     return (unsigned)b;
 }

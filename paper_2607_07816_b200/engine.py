@@ -20,9 +20,9 @@ EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "s
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
            "sv_apply_gate_truncate", "sv_fuse_gates", "sv_reorder_gates"]
+TEST_EXPORTS = ["sv_test_set_pre_slack"]      # include/sparse_sv_test.h
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
-OPT_PRE_SLACK = 1
 
 
 class SvStats(C.Structure):
@@ -89,6 +89,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_profile_get.argtypes = [vp, i32, C.POINTER(SvKernelProf)]
     lib.sv_set_option.restype = i32
     lib.sv_set_option.argtypes = [vp, i32, u64]
+    lib.sv_test_set_pre_slack.restype = i32
+    lib.sv_test_set_pre_slack.argtypes = [vp, C.c_longlong]
     return lib
 
 
@@ -255,6 +257,10 @@ class SparseSV:
 
     def set_option(self, option: int, value: int):
         self._chk(lib.sv_set_option(self._h, int(option), int(value)))
+
+    def test_set_pre_slack(self, slack: int):
+        """Test hook (include/sparse_sv_test.h)."""
+        self._chk(lib.sv_test_set_pre_slack(self._h, int(slack)))
 
     def check_invariants(self) -> bool:
         ok = C.c_int(0)

@@ -7,10 +7,10 @@ import re
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared():
-    src = open(os.path.join(ROOT, "include", "sparse_sv.h")).read()
+def _declared(header="sparse_sv.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sv_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sv_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_declares_the_mandated_calls():
@@ -22,7 +22,7 @@ def test_header_declares_the_mandated_calls():
 def test_library_exports_every_declared_symbol():
     from paper_2607_07816_b200 import build
     lib = ctypes.CDLL(build.build())
-    for name in _declared():
+    for name in _declared() + _declared("sparse_sv_test.h"):
         assert hasattr(lib, name), name
 
 
@@ -30,6 +30,7 @@ def test_binding_lists_every_declared_symbol():
     import importlib
     eng = importlib.import_module("paper_2607_07816_b200.engine")
     assert sorted(eng.EXPORTS) == _declared()
+    assert sorted(eng.TEST_EXPORTS) == _declared("sparse_sv_test.h")
     assert eng.lib.sv_arena_bytes(1 << 20) >= (1 << 20) * 48
 
 

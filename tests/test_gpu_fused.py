@@ -187,7 +187,7 @@ def test_fused_floor_margin_failure_reruns():
     keys, amps = W.random_state(rng, n, N, spread=1.5)
     eng, a, b = _engines(n, 4 * N)
     a.load(keys, amps); b.load(keys, amps)
-    a.set_option(eng.OPT_PRE_SLACK, (-3000) & ((1 << 64) - 1))
+    a.test_set_pre_slack(-3000)
     U = _rand_u2(rng)
     K = int(0.6 * N)
     ka = a.apply_gate_truncate([5], U, K, 1.0)

@@ -234,3 +234,76 @@ def test_top_order(eng):
         assert np.array_equal(gk, ok)
         assert np.array_equal(ga, oa)
         assert np.array_equal(gp, op)
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_singular_diagonal_gates_drop_terms(eng, fused):
+    """U need not be unitary (reading R10): a diagonal U with exact zeros on its diagonal -- a projector -- annihilates
+    terms, and an annihilated term is no longer stored ("only nonzero amplitudes").  diag(1,0),
+    diag(1,0,1,0), a three-qubit projector and the all-zero matrix, on a state whose storage order has been permuted
+    and with a truncation still pending on it, against the oracle."""
+    rng = np.random.default_rng(31)
+    n = 40
+    keys, amps = W.random_state(rng, n, 30000, spread=1.0)
+    sv = eng.SparseSV(n, 1 << 17)
+    sv.set_option(eng.OPT_SAMPLE_MIN_TERMS, 512)
+    o = _oracle(n)
+    sv.load(keys, amps); o.load(keys, amps)
+    for q in (7, 33):
+        sv.apply_gate([q], W.mat_h()); o.apply_gate([q], W.mat_h())
+    gates = [([7], np.diag([1.0, 0.0]).astype(np.complex128)),
+             ([33, 2], np.diag([1.0, 0.0, 1.0j, 0.0]).astype(np.complex128)),
+             ([5, 39, 11], np.diag([0, 1, 1, 0, 0.5, 0, 0, -1]).astype(np.complex128)),
+             ([20], np.diag([0.0, 2.0]).astype(np.complex128))]
+    for qs, U in gates:
+        sv.truncate(0, 0.999); o.truncate(0, 0.999)          # leaves a cut pending on the engine's side
+        if fused:
+            sv.apply_gate_truncate(qs, U, 0, 1.0)
+        else:
+            sv.apply_gate(qs, U)
+        o.apply_gate(qs, U)
+        assert sv.stats()["class"] == "diagonal"
+        assert sv.num_terms() == o.num_terms()
+        assert_same_state(sv.export()[:2], o.export()[:2])
+        assert sv.check_invariants()
+    assert sv.num_terms() < 30000
+    sv.apply_gate([3, 4], np.zeros((4, 4), dtype=np.complex128)); o.apply_gate([3, 4], np.zeros((4, 4), dtype=np.complex128))
+    assert sv.num_terms() == o.num_terms() == 0
+    sv.apply_gate([3], W.mat_h())                                  # an empty state stays empty
+    assert sv.num_terms() == 0
+
+
+def test_gates_while_another_stream_keeps_the_sms_busy(eng):
+    """The persistent passes wait on one another in their look-back; they are launched cooperatively, so that work
+    from another stream cannot leave part of their grid unscheduled while the rest spins (include/sparse_sv.h, "Streams").
+    A side stream runs long matmuls while the engine (own stream, own allocation) applies gates of every class and
+    truncates; the result must match the oracle and nothing may hang."""
+    import torch
+    rng = np.random.default_rng(5)
+    n = 44
+    keys, amps = W.random_state(rng, n, 300000, spread=1.0)
+    sv = eng.SparseSV(n, 1 << 22, torch_arena=False)             # its own non-blocking stream
+    sv.set_option(eng.OPT_SAMPLE_MIN_TERMS, 512)
+    o = _oracle(n)
+    sv.load(keys, amps); o.load(keys, amps)
+    side = torch.cuda.Stream()
+    a = torch.randn(8192, 8192, device="cuda", dtype=torch.float32)
+    gates = [([9], W.mat_h()), ([9, 30], W.mat_mcx(2)), ([30, 2], W.haar_unitary(rng, 4)), ([17], W.mat_rz(0.3)),
+             ([40, 3, 22], W.haar_unitary(rng, 8)), ([1, 40, 9], W.mat_mcx(3)), ([22], W.haar_unitary(rng, 2))]
+    with torch.cuda.stream(side):
+        for _ in range(60):
+            a = torch.tanh(a @ a) * 0.01
+    for qs, U in gates:
+        with torch.cuda.stream(side):
+            for _ in range(10):
+                a = torch.tanh(a @ a) * 0.01
+        kg = sv.apply_gate_truncate(qs, U, 400000, 0.9999)
+        o.apply_gate(qs, U)
+        ko = o.truncate(400000, 0.9999)
+        assert abs(kg - ko) <= 1e-10
+        assert sv.num_terms() == o.num_terms()
+    torch.cuda.synchronize()
+    from util_parity import assert_truncation_parity
+    assert_truncation_parity(sv.export()[:2], o.export()[:2])
+    assert sv.check_invariants()
+    sv.close()

@@ -126,6 +126,33 @@ def test_truncate_flat_ties_by_key(eng):
         assert_same_state(sv.export()[:2], o.export()[:2])
 
 
+@pytest.mark.parametrize("f,want", [(0.3, 300), (0.2999, 300), (0.3001, 301), (0.299, 299), (0.1, 100), (0.7, 700), (0.5, 500),
+                                    (0.999, 999), (0.9991, 1000), (1e-9, 1)])
+def test_truncate_knife_edge_closed_form(eng, f, want):
+    """1000 equal terms of amplitude 2^-5 (p = 2^-10, every sum exact in fp64): thresholds at and beside the knife
+    edge j * p == f * S.  min_mass = 0.3 keeps exactly 300 terms, the lowest logical keys ("minimum
+    fraction of probability mass to keep"; readings R5, R22) -- a closed form, checked against the engine AND the
+    oracle.  The storage order is scrambled first (H . H on two qubits moves bits, X sets the lazy mask)."""
+    rng = np.random.default_rng(12)
+    n = 30
+    keys = np.sort(rng.choice(1 << n, size=1000, replace=False).astype(np.uint64))
+    amps = np.full(1000, 2.0 ** -5 + 0.0j)
+    sv, o = _pair(eng, n, keys, amps, cap=1 << 12)
+    for q in (17, 3):                      # CNOT pairs: storage order changes, amplitudes stay bitwise
+        for _ in range(2):
+            sv.apply_gate([q, (q + 5) % n], W.mat_mcx(2))
+    sv.apply_gate([29], W.mat_x()); sv.apply_gate([29], W.mat_x())
+    kg = sv.truncate(0, f)
+    ko = o.truncate(0, f)
+    k, a, _ = sv.export()
+    assert k.size == want == o.num_terms()
+    assert np.array_equal(np.sort(k), keys[:want])
+    assert kg == ko == want / 1000.0
+    scale = 1.0 if want == 1000 else 1.0 / np.sqrt(want * 2.0 ** -10)
+    assert np.all(a == (2.0 ** -5) * scale)
+    assert_same_state(sv.export()[:2], o.export()[:2], tol=0.0)
+
+
 def test_truncate_many_ties_mixed(eng):
     rng = np.random.default_rng(5)
     keys, amps = W.random_state(rng, 36, 60000, spread=1.0)
@@ -161,9 +188,11 @@ def test_config2_scaled_step_locked(eng):
     assert sv.num_terms() <= 1 << 12
 
 
-def test_config4_scaled_step_locked(eng):
-    """configs[3] (peaked, 3 layers, 10% 8x8, cap + mass 0.9999 after every gate) at n=16, K=2^11."""
-    c = W.config4(n=16, max_terms=1 << 11, variant="noh")
+@pytest.mark.parametrize("variant", ["noh", "hboth"])
+def test_config4_scaled_step_locked(eng, variant):
+    """configs[3] (peaked, 3 layers, 10% 8x8, cap + mass 0.9999 after every gate) at n=16, K=2^11.  `hboth` is the
+    variant bench.py runs: its flat 2^n H layer is cut by the key tie-break alone (reading R4)."""
+    c = W.config4(n=16, max_terms=1 << 11, variant=variant)
     _run_step_locked(eng, c, cap=1 << 15)
 
 

@@ -148,3 +148,36 @@ def test_truncate_invalid():
         o.truncate(0, 0.0)
     with pytest.raises(ValueError):
         o.truncate(0, float("nan"))
+
+
+KNIFE_CASES = [(0.3, 300), (0.2999, 300), (0.3001, 301), (0.299, 299), (0.1, 100), (0.7, 700), (0.5, 500), (0.999, 999),
+               (0.9991, 1000), (1e-9, 1)]
+
+
+def knife_state():
+    """1000 terms of amplitude 2^-5 (p = 2^-10 exactly): every prefix sum and S = 1000 * 2^-10 are exact in fp64 in
+    any summation order, so the smallest prefix with j * 2^-10 >= fl(f * S) is a closed form ("minimum
+    fraction of probability mass to keep"; reading R5 / R22)."""
+    rng = np.random.default_rng(12)
+    keys = np.sort(rng.choice(1 << 30, size=1000, replace=False).astype(np.uint64))
+    amps = np.full(1000, 2.0 ** -5 + 0.0j)
+    return keys, amps
+
+
+@pytest.mark.parametrize("f,want", KNIFE_CASES)
+def test_knife_edge_closed_form(f, want):
+    """p-mass on a flat state, thresholds at and beside the knife edge j * p == f * S: f = 0.3 keeps exactly 300 of
+    1000 equal terms (fl(0.3 * 1000/1024) = 300/1024), the lowest keys first (R4)."""
+    keys, amps = knife_state()
+    S = 1000 * 2.0 ** -10
+    thr = f * S                                   # one rounding, as the procedure states it
+    j = next(j for j in range(1, 1001) if j * 2.0 ** -10 >= thr)
+    assert j == want, "the closed form itself"
+    o = _state(keys, amps)
+    kept = o.truncate(0, f)
+    k, a, _ = o.export()
+    assert k.size == want
+    assert np.array_equal(np.sort(k), keys[:want])
+    assert kept == want / 1000.0
+    scale = 1.0 if want == 1000 else 1.0 / math.sqrt(want * 2.0 ** -10)     # nothing dropped: bitwise no-op (R7)
+    assert np.all(a == (2.0 ** -5) * scale)

@@ -51,7 +51,7 @@ def assert_truncation_parity(g, o, p_before_by_key=None):
         pcut = min(pg.min(), po.min())
         for ks, kk, pp in ((only_g, gk, pg), (only_o, ok, po)):
             idx = np.searchsorted(kk, ks)
-            assert np.all(np.abs(pp[idx] - pcut) <= 10 * CUT_REL * pcut), "kept sets differ away from the cutoff"
+            assert np.all(np.abs(pp[idx] - pcut) <= CUT_REL * pcut), "kept sets differ away from the cutoff"
     return only_g.size + only_o.size
 
 
