@@ -559,6 +559,8 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         return SV_OK;
     }
     const u64 n_live_in = s->count;
+    bool dense = (ma >= 2 && mc == 0);   // every entry nonzero: each tuple yields exactly 2^ma outputs (sv_dense.cu)
+    for (int i = 0; i < (1 << (2 * ma)) && dense; ++i) dense = !(tab.U[i].x == 0.0 && tab.U[i].y == 0.0);
     // Fused apply + truncate: when the cap that follows will cut deep into the gate's output, a floor for that
     // cut is estimated from a sample of the outputs, and the pass leaves out what lies below it.
     u64 preM = s->phys / 8;
@@ -593,7 +595,8 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         } else {
             s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
                                                s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1,
-                                               use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts);
+                                               use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts, dense ? 1 : 0,
+                                               (s->defer.active || s->phys != s->count) ? 1 : 0);
         }
         if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         CHECK_LAUNCH();

@@ -1,0 +1,473 @@
+// Final pass of a DENSE gate with MA >= 2 active bits -- every entry of U nonzero, no control-like bit (Haar SU(4),
+// Haar 8x8, 16x16, fused blocks): SURVEY.md rows a-4 .. a-7.
+//
+// Front end as in sv_group.cu (persistent blocks, the next tile landing through cp.async, A* | B* partition, one
+// merge-path split per thread, the tile left in shared memory in its NEW order where the members of a tuple --
+// the terms that differ only in the gate's qubits -- are neighbours), except that dead entries and the
+// terms a pending truncation drops are squeezed out while the tile is partitioned: behind the front end every
+// element of the tile is a live term.
+//
+// Back end.  U has no zero entry, so every tuple yields exactly 2^MA candidate outputs: no owner table, no per-tuple row
+// masks.  ONE THREAD PER TUPLE computes all 2^MA rows in registers (columns added in ascending logical
+// index, every operation rounded separately: DESIGN.md D1): the tuple's members are read once, U comes from shared memory
+// with the lanes of a warp spread over its columns (conflict free), and a round of 256 * TPR tuples costs no per-candidate
+// bookkeeping.
+//   two calls (PRE = false): the tile's output count is known before any arithmetic; every warp transposes its round
+//     through 4 KB of swizzled shared memory so that consecutive lanes store consecutive entries (an exact cancellation
+//     is written as a counted dead entry); the look-back resolves behind the first round's arithmetic.
+//   fused apply + truncate (PRE = true): every candidate is computed ONCE, tested against the floor of the cut that
+//     follows (sv_presample.cu); survivors are ranked by warp scans + one block scan per round and staged in output
+//     order in shared memory; the tile's total is published when its last round is done and the staged outputs stay
+//     PARKED while the block prepares its next tile, then stored coalesced.  A tile with more survivors than the
+//     staging buffer holds (a heavy region of the state) resolves its look-back at once and computes its candidates a
+//     second time, storing them directly.
+#include "sv_tile.cuh"
+#include "sv_launch.cuh"
+#include <type_traits>
+
+#ifndef DP_STAGE
+#define DP_STAGE 2048                      // PRE: staged survivors per tile (about twice the mean at the cap)
+#endif
+
+template <int MA, bool PRE>
+__global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+                                                                            u64* __restrict__ kout, double2* __restrict__ aout, int p,
+                                                                            const GateTab* __restrict__ gtab, PendPred pd,
+                                                                            const TileDesc* __restrict__ desc, u64* status,
+                                                                            u64* d_count, u64 cap, u32 ntiles, const PreCut* __restrict__ pre,
+                                                                            double* __restrict__ pre_mass, u64* __restrict__ pre_cnt,
+                                                                            int maybe_dead) {
+    constexpr int NP = 1 << MA;
+    constexpr u64 AM = (u64)NP - 1;
+    constexpr int TPR = NP >= 8 ? 1 : 8 / NP;   // tuples per thread and round
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
+    double2* sa = La + BP_TILE;                                // the tile: partitioned, then in its new order
+    u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
+    u64* sk = Lk + BP_TILE;
+    unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
+    double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE: staged survivors, output order; else the warps' transposition buffers
+    u64* stg_k = reinterpret_cast<u64*>(stg_a + DP_STAGE);
+    __shared__ int wcA[BP_VT][BP_WARPS], wcB[BP_VT][BP_WARPS];
+    __shared__ int s_nA, s_nB, s_nt;
+    __shared__ int wtot[2][BP_WARPS];
+    __shared__ u64 s_desc[2][8];
+    __shared__ u64 s_base;
+    __shared__ double2 Us[NP * NP];          // Us[r * NP + x] = U[r][x] (physical patterns): lanes differ in x -> different banks
+    __shared__ int s_col[16];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const u32 lt = (1u << lane) - 1u;
+    const bool mv = p >= 0;
+    const u64 Pf = PRE ? pre->P_floor : 0ull;
+    double dmass = 0.0;     // PRE: mass and number of the outputs this thread left out (below the floor)
+    u32 dcnt = 0;
+    u32 n_dead = 0;         // !PRE: exact cancellations written as dead entries
+
+    if (tid < NP * NP) Us[tid] = gtab->U[tid];
+    if (tid < 16) s_col[tid] = gtab->colorder[tid];
+    __syncthreads();
+    u64 colpack = 0;        // logical column t -> physical pattern, 4 bits each
+#pragma unroll
+    for (int t = 0; t < NP; ++t) colpack |= (u64)(s_col[t] & 15) << (4 * t);
+    bool col_ident = true;
+#pragma unroll
+    for (int t = 0; t < NP; ++t) col_ident = col_ident && (s_col[t] == t);
+
+    const u64 bit = mv ? (1ull << p) : 0ull;
+    const u64 himask = (!mv || p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
+    u64* gstat = status + ntiles;
+    // parked tile (PRE): its staged outputs wait for the look-back while the next tile is prepared
+    bool pk_valid = false;  // uniform over the block
+    u32 pk_tile = 0; int pk_total = 0;
+
+    auto issue_loads = [&](const Pieces3& q) {
+#pragma unroll
+        for (int r = 0; r < BP_VT; ++r) {
+            const int e = tid + r * SV_THREADS;
+            if (e < q.cnt) {
+                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
+                cp_async8(Lk + e, kin + g);
+                cp_async16(La + e, ain + g);
+            }
+        }
+        cp_async_commit();
+    };
+    auto flush_parked = [&]() {   // resolve the parked tile's look-back, store its staged outputs coalesced
+        if (tid < 32) {
+            const u64 ex = lookback_exclusive_2level<false>(status, gstat, pk_tile, ntiles, (u64)pk_total);
+            if (tid == 0) {
+                s_base = ex;
+                if (pk_tile == ntiles - 1) d_count[0] = ex + (u64)pk_total;
+            }
+        }
+        __syncthreads();
+        const u64 base = s_base;
+        for (int idx = tid; idx < pk_total; idx += SV_THREADS) {
+            const u64 g = base + (u64)idx;
+            if (g < cap) { st_stream_u64(kout + g, stg_k[idx]); st_stream_d2(aout + g, stg_a[idx]); }
+        }
+        __syncthreads();          // staging (and s_base) are free again
+        pk_valid = false;
+    };
+
+    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+    __syncthreads();
+    issue_loads(pieces_of(s_desc[0]));
+    int par = 0;
+    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+        const u32 next = tile + gridDim.x;
+        u64 dnext = 0;
+        if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
+        const Pieces3 pc = pieces_of(s_desc[par]);
+        const int cnt = pc.cnt;
+        int nA, nL;
+        {   // pick up this thread's landed elements, apply a pending truncation, partition the LIVE ones into A* | B*
+            cp_async_wait_all();
+            u64 lk[BP_VT]; double2 la[BP_VT];
+#pragma unroll
+            for (int r = 0; r < BP_VT; ++r) {
+                const int e = tid + r * SV_THREADS;
+                lk[r] = 0; la[r] = make_double2(0.0, 0.0);
+                if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
+            }
+            if (pd.active) {
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    if (tid + r * SV_THREADS < cnt) {
+                        if (pend_keep(pd, lk[r], la[r])) { la[r].x = __dmul_rn(la[r].x, pd.scale); la[r].y = __dmul_rn(la[r].y, pd.scale); }
+                        else { la[r].x = 0.0; la[r].y = 0.0; }
+                    }
+                }
+            }
+            if (!maybe_dead && (!mv || pc.oneblock)) {   // load order = A* | B* already and nothing to squeeze out
+                nA = mv ? pc.l0 : cnt; nL = cnt;
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const int e = tid + r * SV_THREADS;
+                    if (e < cnt) { sk[e] = lk[r] & ~bit; sa[e] = la[r]; }
+                }
+            } else {
+                u32 balA[BP_VT], balB[BP_VT];
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const bool live = (tid + r * SV_THREADS < cnt) && !(la[r].x == 0.0 && la[r].y == 0.0);
+                    const bool isB = live && (lk[r] & bit);
+                    balA[r] = __ballot_sync(0xffffffffu, live && !isB);
+                    balB[r] = __ballot_sync(0xffffffffu, isB);
+                    if (lane == 0) { wcA[r][warp] = __popc(balA[r]); wcB[r][warp] = __popc(balB[r]); }
+                }
+                __syncthreads();
+                if (warp < 2) {   // lane = r * 8 + warp: exclusive scans of the 32 counts in load order (A: warp 0, B: warp 1)
+                    int* w = warp == 0 ? &wcA[0][0] : &wcB[0][0];
+                    const int c = w[lane];
+                    int inc = c;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                    w[lane] = inc - c;
+                    if (lane == 31) { if (warp == 0) s_nA = inc; else s_nB = inc; }
+                }
+                __syncthreads();
+                nA = s_nA; nL = nA + s_nB;
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    int slot = -1;
+                    if ((balA[r] >> lane) & 1u) slot = wcA[r][warp] + __popc(balA[r] & lt);
+                    else if ((balB[r] >> lane) & 1u) slot = nA + wcB[r][warp] + __popc(balB[r] & lt);
+                    if (slot >= 0) { sk[slot] = lk[r] & ~bit; sa[slot] = la[r]; }
+                }
+            }
+        }
+        if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+        __syncthreads();
+        if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]));
+
+        // ---- phase 1: bring the tile into its new order (moved bit at the LSB) ----
+        if (mv) {
+            const int nB = nL - nA;
+            const u64* skB = sk + nA;
+            const double2* saB = sa + nA;
+            const int diag = min(tid * BP_VT, nL);
+            int i, j;
+            {
+                int lo = max(0, diag - nB), hi = min(diag, nA);
+                while (lo < hi) {   // A first on ties
+                    const int mid = (lo + hi) >> 1;
+                    if (sk[mid] <= skB[diag - 1 - mid]) lo = mid + 1; else hi = mid;
+                }
+                i = lo; j = diag - lo;
+            }
+            const int endpos = min(diag + BP_VT, nL);
+            u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
+            u64 mk[BP_VT]; double2 ma_[BP_VT];
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v) {
+                mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
+                if (diag + v < endpos) {
+                    const bool takeA = ka <= kb;
+                    const u64 k = takeA ? ka : kb;
+                    ma_[v] = takeA ? sa[i] : saB[j];
+                    mk[v] = (k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull);
+                    if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
+                }
+            }
+            __syncthreads();   // every read of the partitioned tile is done
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (diag + v < endpos) { sk[diag + v] = mk[v]; sa[diag + v] = ma_[v]; }
+            __syncthreads();
+        }
+
+        // ---- phase 2: tuples (elements taken strided: conflict-free reads; counts scanned in element order) ----
+        {
+            u32 bs[BP_VT];
+#pragma unroll
+            for (int r = 0; r < BP_VT; ++r) {
+                const int e = tid + r * SV_THREADS;
+                const bool opens = (e < nL) && (e == 0 || (sk[e - 1] >> MA) != (sk[e] >> MA));
+                bs[r] = __ballot_sync(0xffffffffu, opens);
+                if (lane == 0) wcA[r][warp] = __popc(bs[r]);
+            }
+            __syncthreads();
+            if (warp == 0) {
+                int* w = &wcA[0][0];
+                const int c = w[lane];
+                int inc = c;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                w[lane] = inc - c;
+                if (lane == 31) s_nt = inc;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < BP_VT; ++r)
+                if ((bs[r] >> lane) & 1u) tst[wcA[r][warp] + __popc(bs[r] & lt)] = (unsigned short)(tid + r * SV_THREADS);
+            if (tid == 0) tst[s_nt] = (unsigned short)nL;
+        }
+        const int NT = s_nt;
+        const int NC = NT << MA;      // candidates of the tile
+        if (!PRE && tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)NC);   // known before any arithmetic
+        __syncthreads();              // tuple table complete
+        if (PRE && pk_valid) flush_parked();   // (the look-back of the previous tile has had the whole front end to resolve)
+
+        // ---- back end: ONE THREAD PER TUPLE, all 2^MA rows in registers ----
+        // A round takes 256 * TPR tuples; warp w the 32 * TPR consecutive ones from hw, lane l the tuples hw + u * 32 + l.
+        u64 base = 0;
+        bool have_base = false;     // !PRE: the look-back is resolved behind the first round's arithmetic
+        int run = 0;                // PRE: survivors of the earlier rounds (uniform over the block)
+        int wpar = 0;
+        auto round_compute = [&](int hw, double (&accr)[TPR][NP], double (&acci)[TPR][NP], u64 (&kb)[TPR], bool (&valid)[TPR]) {
+#pragma unroll
+            for (int u = 0; u < TPR; ++u) {
+                const int ti = hw + u * 32 + lane;
+                valid[u] = ti < NT;
+                kb[u] = 0;
+#pragma unroll
+                for (int r = 0; r < NP; ++r) { accr[u][r] = 0.0; acci[u][r] = 0.0; }
+                if (valid[u]) {
+                    const int e = tst[ti], nm = (int)tst[ti + 1] - e;
+                    kb[u] = sk[e] & ~AM;
+                    if (col_ident || nm <= 2) {          // members in stored order = ascending logical column (or the order cannot matter)
+                        for (int j = 0; j < nm; ++j) {
+                            const int x = (int)(sk[e + j] & AM);
+                            const double2 a = sa[e + j];
+#pragma unroll
+                            for (int r = 0; r < NP; ++r) {
+                                const double2 uu = Us[r * NP + x];
+                                cmul_acc(accr[u][r], acci[u][r], uu.x, uu.y, a.x, a.y);
+                            }
+                        }
+                    } else {                              // ascending LOGICAL column index (D1)
+                        u32 pk = 0;
+                        for (int j = 0; j < nm; ++j) pk |= 1u << (int)(sk[e + j] & AM);
+                        for (int t = 0; t < NP; ++t) {
+                            const int x = (int)((colpack >> (4 * t)) & 15ull);
+                            if ((pk >> x) & 1u) {
+                                const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+#pragma unroll
+                                for (int r = 0; r < NP; ++r) {
+                                    const double2 uu = Us[r * NP + x];
+                                    cmul_acc(accr[u][r], acci[u][r], uu.x, uu.y, a.x, a.y);
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+        };
+        if constexpr (!PRE) {
+            // ---- two calls: every candidate is an output.  The rows a thread holds are consecutive outputs; each warp
+            // transposes its round through its own 4 KB of shared memory (XOR-swizzled 16-byte entries: conflict free
+            // both ways) so that consecutive lanes store consecutive entries ----
+            double2* W = stg_a + warp * 256;
+            u64* KB = stg_k + warp * (32 * TPR);
+            constexpr int TP = 256 / NP;                 // tuples per transposition phase
+            constexpr int PH = (32 * TPR) / TP;          // phases per round (2 for 16 rows, else 1)
+            constexpr int SWS = MA > 3 ? MA : 3;
+            for (int h = 0; h < NT; h += SV_THREADS * TPR) {
+                const int hw = h + warp * (32 * TPR);
+                double accr[TPR][NP], acci[TPR][NP]; u64 kb[TPR]; bool valid[TPR];
+                round_compute(hw, accr, acci, kb, valid);
+#pragma unroll
+                for (int u = 0; u < TPR; ++u)
+#pragma unroll
+                    for (int r = 0; r < NP; ++r)
+                        if (valid[u] && accr[u][r] == 0.0 && acci[u][r] == 0.0) ++n_dead;   // exact cancellation: a dead entry
+                if (!have_base) {
+                    if (tid < 32) {
+                        const u64 ex = lookback_exclusive_2level<false>(status, gstat, tile, ntiles, (u64)NC);
+                        if (tid == 0) {
+                            s_base = ex;
+                            if (tile == ntiles - 1) d_count[0] = ex + (u64)NC;
+                        }
+                    }
+                    __syncthreads();
+                    base = s_base; have_base = true;
+                }
+#pragma unroll
+                for (int ph = 0; ph < PH; ++ph) {
+#pragma unroll
+                    for (int u = 0; u < TPR; ++u) {
+                        const int sl = u * 32 + lane;                  // this thread's tuple slot in the warp's round
+                        if (sl / TP == ph) {
+                            const int tl = sl % TP;
+                            KB[sl] = kb[u];
+#pragma unroll
+                            for (int r = 0; r < NP; ++r) {
+                                const int en = tl * NP + r;
+                                W[en ^ ((en >> SWS) & 7)] = make_double2(accr[u][r], acci[u][r]);
+                            }
+                        }
+                    }
+                    __syncwarp();
+#pragma unroll
+                    for (int s = 0; s < 8; ++s) {
+                        const int o = s * 32 + lane;
+                        const int sl = ph * TP + (o >> MA), row = o & (NP - 1);
+                        const int ti = hw + sl;
+                        const u64 g = base + ((u64)ti << MA) + (u64)row;
+                        if (ti < NT && g < cap) { st_stream_u64(kout + g, KB[sl] | (u64)row); st_stream_d2(aout + g, W[o ^ ((o >> SWS) & 7)]); }
+                    }
+                    __syncwarp();
+                }
+            }
+            if (!have_base) {   // (a tile without a live term still takes part in the chain)
+                if (tid < 32) {
+                    const u64 ex = lookback_exclusive_2level<false>(status, gstat, tile, ntiles, (u64)NC);
+                    if (tid == 0 && tile == ntiles - 1) d_count[0] = ex + (u64)NC;
+                }
+            }
+        } else {
+            // ---- fused apply + truncate: compute once, keep what reaches the floor, rank, stage in output order ----
+            auto rounds = [&](auto direct_tag) {
+                constexpr bool DIRECT = decltype(direct_tag)::value;
+                run = 0;
+                for (int h = 0; h < NT; h += SV_THREADS * TPR, wpar ^= 1) {
+                    const int hw = h + warp * (32 * TPR);
+                    double accr[TPR][NP], acci[TPR][NP]; u64 kb[TPR]; bool valid[TPR];
+                    round_compute(hw, accr, acci, kb, valid);
+                    u32 mask[TPR]; int ex[TPR];
+                    int wsum = 0;
+#pragma unroll
+                    for (int u = 0; u < TPR; ++u) {
+                        u32 m = 0;
+#pragma unroll
+                        for (int r = 0; r < NP; ++r) {
+                            if (valid[u] && !(accr[u][r] == 0.0 && acci[u][r] == 0.0)) {   // (an exact cancellation is simply not written)
+                                const double pr = prob_of(make_double2(accr[u][r], acci[u][r]));
+                                if ((u64)__double_as_longlong(pr) >= Pf) m |= 1u << r;
+                                else if (!DIRECT) { dmass = __dadd_rn(dmass, pr); ++dcnt; }
+                            }
+                        }
+                        mask[u] = m;
+                        const int c = __popc(m);
+                        int inc = c;
+#pragma unroll
+                        for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                        ex[u] = wsum + inc - c;
+                        wsum += __shfl_sync(0xffffffffu, inc, 31);
+                    }
+                    if (lane == 0) wtot[wpar][warp] = wsum;
+                    __syncthreads();
+                    int woff = 0, rtot = 0;
+#pragma unroll
+                    for (int w = 0; w < BP_WARPS; ++w) { const int c = wtot[wpar][w]; rtot += c; if (w < warp) woff += c; }
+#pragma unroll
+                    for (int u = 0; u < TPR; ++u) {
+                        int s = run + woff + ex[u];
+#pragma unroll
+                        for (int r = 0; r < NP; ++r) {
+                            if ((mask[u] >> r) & 1u) {
+                                if (DIRECT) {
+                                    const u64 g = base + (u64)s;
+                                    if (g < cap) { st_stream_u64(kout + g, kb[u] | (u64)r); st_stream_d2(aout + g, make_double2(accr[u][r], acci[u][r])); }
+                                } else if (s < DP_STAGE) { stg_k[s] = kb[u] | (u64)r; stg_a[s] = make_double2(accr[u][r], acci[u][r]); }
+                                ++s;
+                            }
+                        }
+                    }
+                    run += rtot;
+                }
+            };
+            rounds(std::false_type{});
+            const int total = run;
+            if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);
+            if (total <= DP_STAGE) {      // parked: stored after the next tile's front end
+                pk_valid = true; pk_tile = tile; pk_total = total;
+            } else {                      // more survivors than the staging buffer holds: second evaluation, direct stores
+                if (tid < 32) {
+                    const u64 ex = lookback_exclusive_2level<false>(status, gstat, tile, ntiles, (u64)total);
+                    if (tid == 0) {
+                        s_base = ex;
+                        if (tile == ntiles - 1) d_count[0] = ex + (u64)total;
+                    }
+                }
+                __syncthreads();
+                base = s_base;
+                rounds(std::true_type{});
+            }
+        }
+        __syncthreads();   // the tile and the tuple table are reused by the next tile
+    }
+    if (PRE && pk_valid) flush_parked();
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) n_dead += __shfl_xor_sync(0xffffffffu, n_dead, d);
+    if (lane == 0 && n_dead) atomicAdd(reinterpret_cast<unsigned long long*>(&d_count[1]), (unsigned long long)n_dead);
+    if (PRE) {   // block totals of what was left out, summed in a fixed order (see sv_pair.cu)
+        __shared__ double s_pm[BP_WARPS];
+        __shared__ u32 s_pc[BP_WARPS];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            dmass = __dadd_rn(dmass, __shfl_xor_sync(0xffffffffu, dmass, d));
+            dcnt += __shfl_xor_sync(0xffffffffu, dcnt, d);
+        }
+        if (lane == 0) { s_pm[warp] = dmass; s_pc[warp] = dcnt; }
+        __syncthreads();
+        if (tid == 0) {
+            double m = 0.0; u64 c = 0;
+            for (int w = 0; w < BP_WARPS; ++w) { m = __dadd_rn(m, s_pm[w]); c += s_pc[w]; }
+            pre_mass[blockIdx.x] = m; pre_cnt[blockIdx.x] = c;
+        }
+    }
+}
+
+template <int MA, bool PRE>
+static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
+                            const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
+                            const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
+    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)(BP_TILE + 8) * 2 + (size_t)DP_STAGE * 24;
+    static int per_sm[SV_MAX_DEV];
+    return sv_launch_persistent(densepass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
+                                (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead);
+}
+
+// Dispatch for svk_grouppass (sv_group.cu): the final pass of a dense gate.  Returns the grid size.
+u32 svk_densepass_launch(int ma, bool use_pre, const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
+                         const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
+                         const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
+#define SV_DP(MA_, PRE_) launch_densepass<MA_, PRE_>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt, maybe_dead)
+    if (use_pre) {
+        switch (ma) { case 2: return SV_DP(2, true); case 3: return SV_DP(3, true); case 4: return SV_DP(4, true); default: return 0; }
+    }
+    switch (ma) { case 2: return SV_DP(2, false); case 3: return SV_DP(3, false); case 4: return SV_DP(4, false); default: return 0; }
+#undef SV_DP
+}

@@ -105,7 +105,8 @@ int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStre
 int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
                   const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
                   u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr,
-                  const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr);
+                  const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr,
+                  int dense = 0, int maybe_dead = 1);   // dense: U has no zero entry and no control-like bit (sv_dense.cu)
 
 // Lean single-bit pass (sv_pair.cu): moves physical bit p to the LSB in one streaming pass.
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
