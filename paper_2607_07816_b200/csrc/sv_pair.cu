@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     double2* La0 = reinterpret_cast<double2*>(smem_raw);       // landing amplitudes, double buffered
     double2* La1 = La0 + BP_TILE;
     u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);           // landing keys (consumed by prepare)
-    u64* Wk0 = Lk + BP_TILE;                                   // A* | B* keys with bit p cleared; later the staged output keys
+    u64* Wk0 = Lk + BP_TILE + 8;                               // A* | B* keys with bit p cleared; later the staged output keys
     unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk0 + BP_WKN);   // their landing slots; later the staged source slots
     // PARK (general one-bit gate): a second key array, used in turns with the first, so that a tile whose outputs fit
     // one round leaves them parked in shared memory (keys there, amplitudes in the tile's landing buffer), publishes
@@ -81,6 +81,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     __shared__ int s_nA;
     __shared__ u64 s_desc[2][8];
     __shared__ u64 s_base;
+    __shared__ __align__(8) u64 s_bar;   // mbarrier of the landing bulk copies (one batch in flight at a time)
     __shared__ double2 sU[64];      // [cx][xr][xc], ma = 1: up to 8 control patterns x 4
     __shared__ int s_cpos[SV_MAX_M], s_mc;
     __shared__ int s_sw[8], s_unit; // PERM: block cx swaps the bit; every nonzero entry is exactly 1
@@ -121,18 +122,12 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     // merged and written, the block's NEXT tile is already on its way from HBM (cp.async, one thread per
     // element): every block keeps a full tile of loads in flight.  Each thread later files exactly the
     // keys it requested.  Tile descriptors travel one iteration ahead (s_desc).
+    // The tile lands by bulk copies (TMA): one thread arms the barrier and issues up to six copies (sv_tile.cuh).
     auto issue_loads = [&](const Pieces3& q, double2* La) {
-#pragma unroll
-        for (int r = 0; r < BP_VT; ++r) {
-            const int e = tid + r * SV_THREADS;
-            if (e < q.cnt) {
-                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
-                cp_async8(Lk + e, kin + g);
-                cp_async16(La + e, ain + g);
-            }
-        }
-        cp_async_commit();
+        if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
     };
+    if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
+    u32 bar_phase = 0;
     if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
     __syncthreads();
     issue_loads(pieces_of(s_desc[0]), La0);
@@ -148,12 +143,14 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         const int cnt = pc.cnt;
         int nA;
         {   // ---- prepare: keys only ----
-            cp_async_wait_all();      // this thread's own elements have landed
+            mbar_wait(&s_bar, bar_phase);      // the tile has landed
+            bar_phase ^= 1u;
+            const Landing3 ld = landing_of(pc);
             u64 lk[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
-                lk[r] = (e < cnt) ? Lk[e] : 0;
+                lk[r] = (e < cnt) ? Lk[landing_key_slot(pc, ld, e)] : 0;
             }
             if (pc.oneblock) {   // piece 0 is all A, piece 1 all B: the load order is already A* | B*
                 nA = pc.l0;
@@ -450,7 +447,7 @@ template <int MODE, bool FIXED, bool PRE>
 static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                           const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
-    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + (size_t)BP_WKN * (8 + 2) +
+    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + 64 + (size_t)BP_WKN * (8 + 2) +
                         ((!FIXED && MODE == 1) ? (size_t)BP_WKN * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
     static int per_sm[SV_MAX_DEV];
     const u32 grid = sv_launch_persistent(bitpass_kernel<MODE, FIXED, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,

@@ -31,6 +31,35 @@ __device__ __forceinline__ void cp_async16(void* sdst, const void* gsrc) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+// ---- bulk asynchronous copies (TMA, cp.async.bulk) + mbarrier: a tile is at most three CONTIGUOUS pieces of the key and
+// of the amplitude array, so one thread lands it with at most six bulk copies instead of one cp.async per element per
+// thread: no load instruction, no address arithmetic and no L1TEX traffic on the 256 threads' side.  Source and
+// destination must be 16-byte aligned and the size a multiple of 16: amplitudes (16 B) always are; a key piece that
+// starts at an odd index is fetched from the even index before it (one key over-fetched in front, possibly one behind),
+// see Landing3.
+__device__ __forceinline__ void mbar_init(u64* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, u32 parity) {
+    const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* sdst, const void* gsrc, u32 bytes, u64* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"((unsigned)__cvta_generic_to_shared(sdst)), "l"(gsrc), "r"(bytes), "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+// generic-proxy accesses to shared memory made before this point are ordered before later async-proxy (bulk copy) writes
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
 struct Pieces3 { u64 ps0, ps1, ps2; int l0, l1, l2, cnt; bool oneblock; };
 __device__ __forceinline__ Pieces3 pieces_of(const u64* w) {   // w: desc[tile] (4 words) followed by desc[tile + 1]
     Pieces3 q;
@@ -42,3 +71,30 @@ __device__ __forceinline__ Pieces3 pieces_of(const u64* w) {   // w: desc[tile] 
     return q;
 }
 
+// Landing slots of a tile that arrived by bulk copies: element e (load order) has its amplitude at La[e] and its key at
+// Lk[e + k0] (piece 0), Lk[e + k1] (piece 1) or Lk[e + k2] (piece 2): every key piece starts at an even slot and is
+// preceded by the one key that was over-fetched when its first index is odd.  Lk holds BP_TILE + 8 keys.
+struct Landing3 { int k0, k1, k2; };
+__device__ __forceinline__ Landing3 landing_of(const Pieces3& q) {
+    Landing3 L;
+    const int o0 = (int)(q.ps0 & 1ull), o1 = (int)(q.ps1 & 1ull), o2 = (int)(q.ps2 & 1ull);
+    const int b1 = (q.l0 + o0 + 1) & ~1;                 // slots taken by piece 0 (rounded to an even count)
+    const int b2 = b1 + ((q.l1 + o1 + 1) & ~1);
+    L.k0 = o0; L.k1 = b1 + o1 - q.l0; L.k2 = b2 + o2 - q.l0 - q.l1;
+    return L;
+}
+__device__ __forceinline__ int landing_key_slot(const Pieces3& q, const Landing3& L, int e) {
+    return e + (e < q.l0 ? L.k0 : (e < q.l0 + q.l1 ? L.k1 : L.k2));
+}
+// Issued by ONE thread: arm the barrier with the byte count, then the (up to six) copies.
+__device__ __forceinline__ void land_tile_bulk(const Pieces3& q, const u64* __restrict__ kin, const double2* __restrict__ ain,
+                                               u64* Lk, double2* La, u64* bar) {
+    const int o0 = (int)(q.ps0 & 1ull), o1 = (int)(q.ps1 & 1ull), o2 = (int)(q.ps2 & 1ull);
+    const int c0 = q.l0 ? ((q.l0 + o0 + 1) & ~1) : 0, c1 = q.l1 ? ((q.l1 + o1 + 1) & ~1) : 0, c2 = q.l2 ? ((q.l2 + o2 + 1) & ~1) : 0;
+    const int b1 = (q.l0 + o0 + 1) & ~1, b2 = b1 + ((q.l1 + o1 + 1) & ~1);
+    fence_proxy_async_smem();
+    mbar_expect_tx(bar, (u32)((c0 + c1 + c2) * 8 + (q.l0 + q.l1 + q.l2) * 16));
+    if (q.l0) { bulk_g2s(Lk, kin + (q.ps0 & ~1ull), (u32)c0 * 8u, bar); bulk_g2s(La, ain + q.ps0, (u32)q.l0 * 16u, bar); }
+    if (q.l1) { bulk_g2s(Lk + b1, kin + (q.ps1 & ~1ull), (u32)c1 * 8u, bar); bulk_g2s(La + q.l0, ain + q.ps1, (u32)q.l1 * 16u, bar); }
+    if (q.l2) { bulk_g2s(Lk + b2, kin + (q.ps2 & ~1ull), (u32)c2 * 8u, bar); bulk_g2s(La + q.l0 + q.l1, ain + q.ps2, (u32)q.l2 * 16u, bar); }
+}
