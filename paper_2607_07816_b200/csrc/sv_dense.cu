@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
     double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
     double2* sa = La + BP_TILE;                                // the tile: partitioned, then in its new order
     u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
-    u64* sk = Lk + BP_TILE;
+    u64* sk = Lk + BP_TILE + 8;
     unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
     double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE: staged survivors, output order; else the warps' transposition buffers
     u64* stg_k = reinterpret_cast<u64*>(stg_a + DP_STAGE);
@@ -53,6 +53,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
     __shared__ int wtot[2][BP_WARPS];
     __shared__ u64 s_desc[2][8];
     __shared__ u64 s_base;
+    __shared__ __align__(8) u64 s_bar;   // mbarrier of the landing bulk copies
     __shared__ double2 Us[NP * NP];          // Us[r * NP + x] = U[r][x] (physical patterns): lanes differ in x -> different banks
     __shared__ int s_col[16];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -80,18 +81,12 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
     bool pk_valid = false;  // uniform over the block
     u32 pk_tile = 0; int pk_total = 0;
 
+    // The tile lands by bulk copies (TMA): one thread arms the barrier and issues up to six copies (sv_tile.cuh).
     auto issue_loads = [&](const Pieces3& q) {
-#pragma unroll
-        for (int r = 0; r < BP_VT; ++r) {
-            const int e = tid + r * SV_THREADS;
-            if (e < q.cnt) {
-                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
-                cp_async8(Lk + e, kin + g);
-                cp_async16(La + e, ain + g);
-            }
-        }
-        cp_async_commit();
+        if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
     };
+    if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
+    u32 bar_phase = 0;
     auto flush_parked = [&]() {   // resolve the parked tile's look-back, store its staged outputs coalesced
         if (tid < 32) {
             const u64 ex = lookback_exclusive_2level<false>(status, gstat, pk_tile, ntiles, (u64)pk_total);
@@ -122,13 +117,15 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
         const int cnt = pc.cnt;
         int nA, nL;
         {   // pick up this thread's landed elements, apply a pending truncation, partition the LIVE ones into A* | B*
-            cp_async_wait_all();
+            mbar_wait(&s_bar, bar_phase);      // the tile has landed
+            bar_phase ^= 1u;
+            const Landing3 ld = landing_of(pc);
             u64 lk[BP_VT]; double2 la[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
                 lk[r] = 0; la[r] = make_double2(0.0, 0.0);
-                if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
+                if (e < cnt) { lk[r] = Lk[landing_key_slot(pc, ld, e)]; la[r] = La[e]; }
             }
             if (pd.active) {
 #pragma unroll
@@ -454,7 +451,7 @@ template <int MA, bool PRE>
 static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)(BP_TILE + 8) * 2 + (size_t)DP_STAGE * 24;
+    const size_t smem = (size_t)2 * BP_TILE * 24 + 64 + (size_t)(BP_TILE + 8) * 2 + (size_t)DP_STAGE * 24;
     static int per_sm[SV_MAX_DEV];
     return sv_launch_persistent(densepass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                 (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead);

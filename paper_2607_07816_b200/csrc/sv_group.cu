@@ -36,7 +36,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
     double2* sa = La + BP_TILE;                                // work buffer: partitioned tile, then the tile in its new order
     u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
-    u64* sk = Lk + BP_TILE;
+    u64* sk = Lk + BP_TILE + 8;
     u64* s_info = sk + BP_TILE;                                // per term: the tuple it opens (rows, masks, control block)
     unsigned short* s_owner = reinterpret_cast<unsigned short*>(s_info + BP_TILE);   // per output of a round: (term << 4) | row
     __shared__ int red[BP_WARPS + 2];
@@ -44,6 +44,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     __shared__ int s_nA;
     __shared__ u64 s_desc[2][8];
     __shared__ u64 s_base;
+    __shared__ __align__(8) u64 s_bar;   // mbarrier of the landing bulk copies
     __shared__ double2 sU[256];
     __shared__ unsigned short s_nzr[16][16];   // [cx][xc]: rows r with U[r][xc] != 0 in control block cx
     __shared__ int s_cpos[SV_MAX_M], s_col[16], s_mc;
@@ -73,18 +74,12 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     u64* gstat = status + ntiles;
     u32 n_dead = 0;
 
+    // The tile lands by bulk copies (TMA): one thread arms the barrier and issues up to six copies (sv_tile.cuh).
     auto issue_loads = [&](const Pieces3& q) {
-#pragma unroll
-        for (int r = 0; r < BP_VT; ++r) {
-            const int e = tid + r * SV_THREADS;
-            if (e < q.cnt) {
-                const u64 g = e < q.l0 ? q.ps0 + e : (e < q.l0 + q.l1 ? q.ps1 + (e - q.l0) : q.ps2 + (e - q.l0 - q.l1));
-                cp_async8(Lk + e, kin + g);
-                cp_async16(La + e, ain + g);
-            }
-        }
-        cp_async_commit();
+        if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
     };
+    if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
+    u32 bar_phase = 0;
     if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
     __syncthreads();
     issue_loads(pieces_of(s_desc[0]));
@@ -97,13 +92,15 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
         const int cnt = pc.cnt;
         int nA;
         {   // pick up this thread's landed elements, apply a pending truncation, partition into A* | B*
-            cp_async_wait_all();
+            mbar_wait(&s_bar, bar_phase);      // the tile has landed
+            bar_phase ^= 1u;
+            const Landing3 ld = landing_of(pc);
             u64 lk[BP_VT]; double2 la[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
                 lk[r] = 0; la[r] = make_double2(0.0, 0.0);
-                if (e < cnt) { lk[r] = Lk[e]; la[r] = La[e]; }
+                if (e < cnt) { lk[r] = Lk[landing_key_slot(pc, ld, e)]; la[r] = La[e]; }
             }
             if (pd.active) {
 #pragma unroll
@@ -361,7 +358,7 @@ template <int MA, bool PRE>
 static u32 launch_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + (size_t)BP_TILE * 8 + (size_t)GP_ROUND * 2;   // landing + work + tuple table + owners
+    const size_t smem = (size_t)2 * BP_TILE * 24 + 64 + (size_t)BP_TILE * 8 + (size_t)GP_ROUND * 2;   // landing + work + tuple table + owners
     static int per_sm[SV_MAX_DEV];
     const u32 grid = sv_launch_persistent(grouppass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                           (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt);
