@@ -38,12 +38,19 @@ def _compile(src, force, verbose, extra):
     return obj
 
 
-def build(force: bool = False, verbose: bool = False, extra=()) -> str:
+def build(force: bool = False, verbose: bool = False, extra=(), checked: bool = False) -> str:
+    """checked=True: the bounds-checked build (-DSV_CHECKED, see csrc/sv_device.cuh) INTO THE SAME libsparse_sv.so, for one
+    run of the GPU tests; build again without it afterwards."""
+    global OBJ
+    if checked:
+        OBJ = os.path.join(HERE, "build", "checked")
+        extra = list(extra) + ["-DSV_CHECKED"]
+        force = True
     os.makedirs(OBJ, exist_ok=True)
     srcs = sources()
     with ThreadPoolExecutor(max_workers=min(len(srcs), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(lambda s: _compile(s, force, verbose, list(extra)), srcs))
-    if (not force) and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(o) for o in objs):
+    if (not force) and (not checked) and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(o) for o in objs):
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
     subprocess.run([NVCC] + LFLAGS + ["-o", tmp] + objs, check=True)
@@ -53,4 +60,4 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
 
 if __name__ == "__main__":
     import sys
-    print(build(force="-f" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="-f" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv))

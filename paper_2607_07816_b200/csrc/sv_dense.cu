@@ -170,6 +170,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
                     int slot = -1;
                     if ((balA[r] >> lane) & 1u) slot = wcA[r][warp] + __popc(balA[r] & lt);
                     else if ((balB[r] >> lane) & 1u) slot = nA + wcB[r][warp] + __popc(balB[r] & lt);
+                    SV_CHK(slot < nL);
                     if (slot >= 0) { sk[slot] = lk[r] & ~bit; sa[slot] = la[r]; }
                 }
             }
@@ -193,6 +194,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
                 }
                 i = lo; j = diag - lo;
             }
+            SV_CHK(i >= 0 && i <= nA && j >= 0 && j <= nB);
             const int endpos = min(diag + BP_VT, nL);
             u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
             u64 mk[BP_VT]; double2 ma_[BP_VT];
@@ -241,6 +243,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
             if (tid == 0) tst[s_nt] = (unsigned short)nL;
         }
         const int NT = s_nt;
+        SV_CHK(NT >= 0 && NT <= nL && nL <= BP_TILE);
         const int NC = NT << MA;      // candidates of the tile
         if (!PRE && tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)NC);   // known before any arithmetic
         __syncthreads();              // tuple table complete
@@ -262,6 +265,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
                 for (int r = 0; r < NP; ++r) { accr[u][r] = 0.0; acci[u][r] = 0.0; }
                 if (valid[u]) {
                     const int e = tst[ti], nm = (int)tst[ti + 1] - e;
+                    SV_CHK(nm >= 1 && nm <= NP && e + nm <= nL);
                     kb[u] = sk[e] & ~AM;
                     if (col_ident || nm <= 2) {          // members in stored order = ascending logical column (or the order cannot matter)
                         for (int j = 0; j < nm; ++j) {
@@ -407,6 +411,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
             };
             rounds(std::false_type{});
             const int total = run;
+            SV_CHK(total >= 0 && total <= NC);
             if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);
             if (total <= DP_STAGE) {      // parked: stored after the next tile's front end
                 pk_valid = true; pk_tile = tile; pk_total = total;

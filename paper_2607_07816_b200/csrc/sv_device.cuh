@@ -2,6 +2,15 @@
 #pragma once
 #include "sv_internal.h"
 
+// Checked build (-DSV_CHECKED; python -m paper_2607_07816_b200.build --checked): every index that is computed from data
+// is tested against its bound where SV_CHK stands, and the kernel traps on a violation (the launch then fails with an
+// error code).  compute-sanitizer is closed on the pool this was developed on; this is what stands in for memcheck.
+#ifdef SV_CHECKED
+#define SV_CHK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define SV_CHK(cond) do { } while (0)
+#endif
+
 #define SV_FLAG_AGG  (1ull << 62)
 #define SV_FLAG_INCL (2ull << 62)
 #define SV_VAL_MASK  ((1ull << 62) - 1)

@@ -143,6 +143,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                     if (e < cnt) {
                         const int aBefore = wc[r][warp] + __popc(balA[r] & ((1u << lane) - 1u));
                         const int slot = (lk[r] & bit) ? nA + (e - aBefore) : aBefore;
+                        SV_CHK(slot >= 0 && slot < cnt);
                         sk[slot] = lk[r] & ~bit; sa[slot] = la[r];
                     }
                 }
@@ -283,7 +284,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
                     while (rows) {
                         const int r = __ffs(rows) - 1;
                         rows &= rows - 1;
-                        if ((unsigned)off < (unsigned)GP_ROUND) s_owner[off] = (unsigned short)(((e0 + v) << 4) | r);
+                        if ((unsigned)off < (unsigned)GP_ROUND) { SV_CHK(e0 + v < cnt); s_owner[off] = (unsigned short)(((e0 + v) << 4) | r); }
                         ++off;
                     }
                 }
@@ -306,6 +307,7 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
             for (int q = tid; q < m; q += SV_THREADS) {
                 const u32 code = s_owner[q];
                 const int e = (int)(code >> 4), r = (int)(code & 15u);
+                SV_CHK(e < cnt && r < NP);
                 const u64 k = sk[e];
                 double sr, si;
                 tuple_row(e, r, sr, si);

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                     if (e < cnt) {
                         const int aBefore = wc[r][warp] + __popc(balA[r] & ((1u << lane) - 1u));
                         const int slot = (lk[r] & bit) ? nA + (e - aBefore) : aBefore;
+                        SV_CHK(slot >= 0 && slot < cnt);
                         Wk[slot] = lk[r] & ~bit; Wi[slot] = (unsigned short)e;
                     }
                 }
@@ -224,6 +225,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             }
             i = lo; j = diag - lo;
         }
+        SV_CHK(i >= 0 && i <= nA && j >= 0 && j <= nB);
         const int endpos = min(diag + BP_VT, cnt);
         int pos = diag;
         // keys with bit p cleared never equal ~0: safe sentinels for an exhausted side
@@ -266,7 +268,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             __syncthreads();   // every read of A* | B* is done: stage by output position in the same arrays
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v)
-                if (opos[v] >= 0) { Wk[BP_SWK(opos[v])] = okey[v]; Wi[BP_SWK(opos[v])] = (unsigned short)osrc[v]; }
+                if (opos[v] >= 0) { SV_CHK(opos[v] < cnt && (osrc[v] & 0x7fff) < cnt); Wk[BP_SWK(opos[v])] = okey[v]; Wi[BP_SWK(opos[v])] = (unsigned short)osrc[v]; }
             __syncthreads();
             // ---- copy-out: gather the amplitude, apply a pending truncation and the phase, store coalesced ----
             const u64 base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
@@ -369,6 +371,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         const int excl = block_excl_scan1(nout, red, &total);   // its barriers also retire every read of A* | B* and of the amplitudes
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
         // BP_ROUND outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
+        SV_CHK(total >= 0 && total <= 2 * BP_TILE && excl >= 0 && excl + nout <= total);
         const bool park = PARK && total <= BP_ROUND;   // one round: its outputs wait in shared memory for the block's next tile
         if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);   // at once: the later tiles read it while this one stages
         for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {

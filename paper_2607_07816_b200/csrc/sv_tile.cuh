@@ -68,6 +68,7 @@ __device__ __forceinline__ Pieces3 pieces_of(const u64* w) {   // w: desc[tile] 
     if (q.oneblock) { q.ps0 = ia0; q.l0 = (int)(ia1 - ia0); q.ps1 = ib0; q.l1 = (int)(ib1 - ib0); q.ps2 = 0; q.l2 = 0; }
     else { q.ps0 = ia0; q.l0 = (int)(mid0 - ia0); q.ps1 = ib0; q.l1 = (int)(ia1 - ib0); q.ps2 = mid1; q.l2 = (int)(ib1 - mid1); }
     q.cnt = min(BP_TILE, q.l0 + q.l1 + q.l2);
+    SV_CHK(q.l0 >= 0 && q.l1 >= 0 && q.l2 >= 0 && q.l0 + q.l1 + q.l2 <= BP_TILE);
     return q;
 }
 
@@ -84,7 +85,9 @@ __device__ __forceinline__ Landing3 landing_of(const Pieces3& q) {
     return L;
 }
 __device__ __forceinline__ int landing_key_slot(const Pieces3& q, const Landing3& L, int e) {
-    return e + (e < q.l0 ? L.k0 : (e < q.l0 + q.l1 ? L.k1 : L.k2));
+    const int sl = e + (e < q.l0 ? L.k0 : (e < q.l0 + q.l1 ? L.k1 : L.k2));
+    SV_CHK(sl >= 0 && sl < BP_TILE + 8);
+    return sl;
 }
 // Issued by ONE thread: arm the barrier with the byte count, then the (up to six) copies.
 __device__ __forceinline__ void land_tile_bulk(const Pieces3& q, const u64* __restrict__ kin, const double2* __restrict__ ain,
