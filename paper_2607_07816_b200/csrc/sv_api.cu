@@ -418,13 +418,32 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     memset(&tab, 0, sizeof(tab));
     if (s->count == 0) { s->stats.gate_class = SV_CLASS_NONE; return SV_OK; }
 
-    // XOR class: U[r][c] != 0 iff r == c ^ x0 (then x0 = all active bits); pure relabelling + phases
+    // Relabelling class (rows a-3, f-4): U is monomial and its nonzero of column c sits in row sigma(c) = pi(c) ^ x0 with
+    // pi a PERMUTATION OF THE GATE'S QUBITS and x0 a constant pattern -- X, SWAP, any product of them, with phases.  Such a
+    // gate only renames qubits and flips bits: the lazy layout (phys_of_log, xmask) takes it, no data is touched
+    // ("just permutes the amplitudes"); phases, if any, go through the diagonal pass.
     bool xor_class = ma > 0, diag_nonzero = true, unit_phase = true;
-    for (int c = 0; c < d && xor_class; ++c)
-        for (int r = 0; r < d; ++r) {
-            const bool want = (r == (c ^ amask_l));
-            if (want == is_zero(U[r * d + c])) { xor_class = false; break; }
+    int sigma[16], pi[SV_MAX_M] = {0, 1, 2, 3}, x0 = 0;
+    for (int c = 0; c < d && xor_class; ++c) {
+        int nz = 0;
+        for (int r = 0; r < d; ++r) if (!is_zero(U[r * d + c])) { sigma[c] = r; ++nz; }
+        if (nz != 1) xor_class = false;
+    }
+    if (xor_class) {
+        x0 = sigma[0];
+        int used = 0;
+        for (int j = 0; j < m && xor_class; ++j) {
+            const int v = sigma[1 << j] ^ x0;
+            if (v == 0 || (v & (v - 1)) || (used & v)) { xor_class = false; break; }
+            used |= v;
+            pi[j] = __builtin_ctz((unsigned)v);
         }
+        for (int c = 0; c < d && xor_class; ++c) {
+            int pc = 0;
+            for (int j = 0; j < m; ++j) pc |= ((c >> j) & 1) << pi[j];
+            if (sigma[c] != (pc ^ x0)) xor_class = false;
+        }
+    }
     if (ma == 0)
         for (int c = 0; c < d; ++c) if (is_zero(U[c * d + c])) diag_nonzero = false;
 
@@ -436,12 +455,19 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         for (int j = 0; j < m; ++j) tab.ctrl_pos[j] = s->phys_of_log[qubits[j]];
         for (int cs = 0; cs < d; ++cs) {
             const int ct = cs ^ xm;                       // true pattern of the stored pattern
-            const sv_c128 z = U[(ct ^ (xor_class ? amask_l : 0)) * d + ct];
+            const sv_c128 z = U[(xor_class ? sigma[ct] : ct) * d + ct];
             tab.U[cs] = make_double2(z.re, z.im);
             if (!(z.re == 1.0 && z.im == 0.0)) unit_phase = false;
         }
-        if (xor_class)   // flip the lazy mask on the active bits: no data is touched
-            { for (int i = 0; i < ma; ++i) s->xmask ^= 1ull << s->phys_of_log[qubits[active[i]]]; s->lut_valid = false; }
+        if (xor_class) {   // new layout: qubit qubits[pi[j]] now lives where qubits[j] lived, flipped if x0 says so -- no data is touched
+            int oldp[SV_MAX_M];
+            for (int j = 0; j < m; ++j) oldp[j] = s->phys_of_log[qubits[j]];
+            for (int j = 0; j < m; ++j) {
+                s->phys_of_log[qubits[pi[j]]] = oldp[j];
+                if ((x0 >> pi[j]) & 1) s->xmask ^= 1ull << oldp[j];
+            }
+            s->lut_valid = false;
+        }
         s->stats.gate_class = xor_class ? SV_CLASS_XOR : SV_CLASS_DIAGONAL;
         if (!unit_phase) {
             CU(cudaMemcpyAsync(s->tab, &tab, sizeof(tab), cudaMemcpyHostToDevice, s->stream));
@@ -545,6 +571,18 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         const bool z00 = u[0].x == 0.0 && u[0].y == 0.0, z01 = u[1].x == 0.0 && u[1].y == 0.0;
         const bool z10 = u[2].x == 0.0 && u[2].y == 0.0, z11 = u[3].x == 0.0 && u[3].y == 0.0;
         monomial = (!z00 && !z11 && z01 && z10) || (z00 && z11 && !z01 && !z10);
+    }
+    if (ma == 1 && monomial && plast < 0) {
+        // the active bit already is the physical LSB: partners are stored neighbours, the gate is applied IN PLACE (row f-4)
+        prof_slot(s, SV_K_DIAG, 40.0 * (double)s->phys, &ge0, &ge1);
+        if (ge0) cudaEventRecord(ge0, s->stream);
+        s->stats.launches += svk_perm_lsb(s->keys[s->cur], s->amps[s->cur], s->phys, s->tab, s->defer, s->stream);
+        if (ge1) cudaEventRecord(ge1, s->stream);
+        CHECK_LAUNCH();
+        s->stats.passes += 1;
+        s->defer.active = 0;
+        s->stats.n_out = s->count;
+        return SV_OK;
     }
     if (ma == 1 && monomial && few_dead(s)) {
         prof_slot(s, SV_K_BITPASS, 48.0 * (double)s->phys, &ge0, &ge1);

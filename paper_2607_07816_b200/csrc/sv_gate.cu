@@ -7,7 +7,7 @@
 // streaming pass -- a segmented two-way merge of the bit=0 run and the bit=1 run of every block of
 // keys that agree above the moved bit (sv_pair.cu, sv_group.cu).  find_splits cuts such a pass into
 // tiles: merge-path splits, one thread per boundary.  Diagonal gates touch amplitudes only.
-#include "sv_device.cuh"
+#include "sv_tile.cuh"
 
 // ---------------------------------------------------------------------------------------
 // a-2 diagonal fast path: a <- U[c,c] * a, c = the key's pattern on the gate's qubits
@@ -41,6 +41,83 @@ int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStre
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
     if (blocks > (u64)sv_sm_count() * 16) blocks = (u64)sv_sm_count() * 16;
     diag_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, tab);
+    return 1;
+}
+
+// ---------------------------------------------------------------------------------------
+// a-3 / f-4: monomial one-bit gate (CNOT, Toffoli, C3X, controlled-Y ...) whose active bit ALREADY sits at the physical
+// LSB: partners are stored neighbours, so nothing moves.  PAPER.md:54-55: such a gate "just permutes the amplitudes".
+// In place: a tuple with both members and a swapping control pattern trades its two amplitudes (handled by the member
+// with bit 0 clear); a lone member of a swapping tuple gets its key's LSB flipped (the order of the array is unchanged:
+// its neighbours differ from it above bit 0); phases and a pending truncation (dropped -> dead entry, survivors scaled)
+// are applied on the way.  8 B per term when nothing is pending and the entries are unit, else 40 B per term -- against
+// 48 B per term for the position-preserving pass that has to move the bit first.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(SV_THREADS) perm_lsb_kernel(u64* __restrict__ keys, double2* __restrict__ amps, u64 n,
+                                                              const GateTab* __restrict__ gtab, PendPred pd) {
+    __shared__ double2 sU[64];
+    __shared__ int s_cpos[SV_MAX_M], s_mc, s_sw[16], s_unit;
+    if (threadIdx.x < 64) sU[threadIdx.x] = gtab->U[threadIdx.x];
+    if (threadIdx.x < SV_MAX_M) s_cpos[threadIdx.x] = gtab->ctrl_pos[threadIdx.x];
+    if (threadIdx.x == 0) {
+        s_mc = gtab->mc;
+        int unit = 1;
+        for (int cx = 0; cx < 16; ++cx) {
+            const double2* u = &gtab->U[(cx & 15) << 2];
+            const int sw = (u[0].x == 0.0 && u[0].y == 0.0) ? 1 : 0;
+            s_sw[cx] = sw;
+            const double2 x = sw ? u[1] : u[0], y = sw ? u[2] : u[3];
+            if (cx < (1 << gtab->mc) && !(x.x == 1.0 && x.y == 0.0 && y.x == 1.0 && y.y == 0.0)) unit = 0;
+        }
+        s_unit = unit;
+    }
+    __syncthreads();
+    const int mc = s_mc;
+    const bool touch_all = pd.active || !s_unit;     // every amplitude changes (scale / phase)
+    const u64 stride = (u64)gridDim.x * blockDim.x;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const u64 k = keys[i];
+        const int b = (int)(k & 1ull);
+        int cx = 0;
+        for (int q = 0; q < mc; ++q) cx |= (int)((k >> s_cpos[q]) & 1ull) << q;
+        const int sw = s_sw[cx];
+        bool paired = false;
+        if (b == 0) paired = (i + 1 < n) && keys[i + 1] == (k | 1ull);
+        else paired = (i > 0) && keys[i - 1] == (k & ~1ull);
+        auto load = [&](u64 idx, u64 key) {
+            double2 a = amps[idx];
+            if (pd.active) {
+                if (pend_keep(pd, key, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
+                else { a.x = 0.0; a.y = 0.0; }
+            }
+            return a;
+        };
+        auto times = [&](double2 u, double2 a) {
+            if (s_unit) return a;
+            const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
+            const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
+            return make_double2(__dadd_rn(0.0, pr), __dadd_rn(0.0, pi));
+        };
+        const double2* u = &sU[cx << 2];                 // u[row * 2 + col]
+        if (sw && paired) {
+            if (b == 0) {                                 // both members: trade the amplitudes
+                const double2 a0 = load(i, k), a1 = load(i + 1, k | 1ull);
+                amps[i] = times(u[1], a1);                // row 0 <- column 1
+                amps[i + 1] = times(u[2], a0);            // row 1 <- column 0
+            }
+        } else if (sw) {                                  // a lone member moves to the other key of its tuple
+            keys[i] = k ^ 1ull;
+            if (touch_all) amps[i] = times(u[((b ^ 1) << 1) | b], load(i, k));
+        } else if (touch_all) {
+            amps[i] = times(u[(b << 1) | b], load(i, k));
+        }
+    }
+}
+int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st) {
+    if (n == 0) return 0;
+    u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
+    if (blocks > (u64)sv_sm_count() * 16) blocks = (u64)sv_sm_count() * 16;
+    perm_lsb_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, tab, pend);
     return 1;
 }
 

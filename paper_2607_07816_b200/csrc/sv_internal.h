@@ -94,6 +94,8 @@ struct PendPred {
 #define SV_MAX_DEV 64
 int sv_cur_device(); // ordinal of the current device, clamped to SV_MAX_DEV - 1 (index of the per-device caches)
 int sv_sm_count();   // SMs of the current device (cached per device)
+// In place: monomial one-bit gate whose active bit is the physical LSB (partners are neighbours); applies a pending cut.
+int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st);
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----

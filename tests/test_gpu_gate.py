@@ -307,3 +307,88 @@ def test_gates_while_another_stream_keeps_the_sms_busy(eng):
     assert_truncation_parity(sv.export()[:2], o.export()[:2])
     assert sv.check_invariants()
     sv.close()
+
+
+def _perm_matrix(sigma, phases=None):
+    d = len(sigma)
+    U = np.zeros((d, d), dtype=np.complex128)
+    for c, r in enumerate(sigma):
+        U[r, c] = 1.0 if phases is None else phases[c]
+    return U
+
+
+def test_qubit_relabelling_gates_touch_no_data(eng):
+    """SWAP, X (x) SWAP, a cyclic shift of three qubits, iSWAP: monomial gates whose permutation of basis states is a
+    permutation of the gate's QUBITS (plus bit flips) only rename qubits: zero passes
+    when the entries are 1, one diagonal pass for phases.  Checked against the oracle, with gates of every other class
+    and truncations by logical key in between (the lazy layout must stay consistent)."""
+    rng = np.random.default_rng(17)
+    n = 48
+    keys, amps = W.random_state(rng, n, 20000, spread=1.0)
+    sv = eng.SparseSV(n, 1 << 17)
+    sv.set_option(eng.OPT_SAMPLE_MIN_TERMS, 512)
+    o = _oracle(n)
+    sv.load(keys, amps); o.load(keys, amps)
+    swap = _perm_matrix([0, 2, 1, 3])
+    xswap = _perm_matrix([1, 3, 0, 2])                       # r = swap(c) ^ 01
+    cyc3 = _perm_matrix([((c << 1) | (c >> 2)) & 7 for c in range(8)])
+    iswap = _perm_matrix([0, 2, 1, 3], [1, 1j, 1j, 1])
+    x3 = _perm_matrix([c ^ 5 for c in range(8)], np.exp(1j * rng.uniform(0, 6, 8)))
+    seq = [("relabel", [3, 40], swap), ("other", [40], W.mat_h()), ("relabel", [40, 3], xswap), ("other", [3, 17], W.mat_mcx(2)),
+           ("relabel", [47, 0, 21], cyc3), ("other", [0, 47], W.haar_unitary(rng, 4)), ("phase", [21, 9], iswap),
+           ("other", [9], W.mat_rz(0.4)), ("phase", [9, 21, 47], x3), ("relabel", [9, 47], swap), ("other", [47, 3, 9], W.mat_mcx(3))]
+    for kind, qs, U in seq:
+        sv.truncate(0, 0.9995); o.truncate(0, 0.9995)        # a cut stays pending on the engine's side
+        l0 = sv.stats()["launches"]
+        sv.apply_gate(qs, U); o.apply_gate(qs, U)
+        st = sv.stats()
+        if kind == "relabel":
+            assert st["class"] == "xor" and st["passes"] == 0 and st["launches"] == l0, (qs, st)
+        elif kind == "phase":
+            assert st["class"] == "xor" and st["passes"] == 1, (qs, st)
+        assert sv.num_terms() == o.num_terms()
+        assert_same_state(sv.export()[:2], o.export()[:2])
+        assert sv.check_invariants()
+    # ties by LOGICAL key after renaming: a flat state cut by the cap alone
+    sv2 = eng.SparseSV(20, 1 << 12); o2 = _oracle(20)
+    for q in range(10):
+        sv2.apply_gate([q], W.mat_h()); o2.apply_gate([q], W.mat_h())
+    for qs, U in (([0, 19], swap), ([5, 12, 18], cyc3), ([7, 15], xswap)):
+        sv2.apply_gate(qs, U); o2.apply_gate(qs, U)
+    kg, ko = sv2.truncate(300, 1.0), o2.truncate(300, 1.0)
+    assert abs(kg - ko) <= 1e-12
+    assert_same_state(sv2.export()[:2], o2.export()[:2])
+
+
+def test_controlled_permutation_in_place_when_target_is_lsb(eng):
+    """CNOT / Toffoli / controlled-Y whose target already sits at the physical LSB (the previous gate left it there) run
+    IN PLACE: partners are stored neighbours, pairs trade amplitudes, lone members get their key's LSB flipped (SURVEY
+    row f-4).  With pairs and lone members, phases, and a pending cut; against the oracle."""
+    rng = np.random.default_rng(23)
+    n = 52
+    keys, amps = W.random_state(rng, n, 60000, spread=1.0)
+    keys = np.unique(np.concatenate([keys, keys[:25000] ^ np.uint64(1 << 30)]))       # many stored partners on qubit 30
+    amps = (rng.standard_normal(keys.size) + 1j * rng.standard_normal(keys.size)) * np.exp(rng.standard_normal(keys.size))
+    amps /= np.sqrt(np.sum(np.abs(amps) ** 2))
+    sv = eng.SparseSV(n, 1 << 19)
+    sv.set_option(eng.OPT_SAMPLE_MIN_TERMS, 512)
+    o = _oracle(n)
+    sv.load(keys, amps); o.load(keys, amps)
+    cy = np.zeros((4, 4), dtype=np.complex128)       # controlled-Y, qubits = (control, target)
+    cy[0, 0] = cy[2, 2] = 1
+    cy[3, 1] = 1j
+    cy[1, 3] = -1j
+    sv.apply_gate([30], W.mat_rx(0.9)); o.apply_gate([30], W.mat_rx(0.9))              # qubit 30 is the physical LSB now
+    sv.profile(True)
+    for i, (qs, U) in enumerate([([11, 30], W.mat_mcx(2)), ([5, 44, 30], W.mat_mcx(3)), ([2, 30], cy), ([1, 7, 50, 30], W.mat_mcx(4)),
+                                 ([30, 11], W.mat_mcx(2))]):
+        if i % 2 == 0:
+            sv.truncate(0, 0.999); o.truncate(0, 0.999)
+        sv.apply_gate(qs, U); o.apply_gate(qs, U)
+        assert sv.stats()["class"] == "group"
+        assert sv.num_terms() == o.num_terms()
+        assert_same_state(sv.export()[:2], o.export()[:2])
+        assert sv.check_invariants()
+    pr = sv.profile_get()
+    assert pr["diag"]["launches"] == 4 and pr["bitpass"]["launches"] == 1, pr      # four in place, the last one moves qubit 11
+    sv.profile(False)
