@@ -74,49 +74,75 @@ __global__ void __launch_bounds__(SV_THREADS) perm_lsb_kernel(u64* __restrict__ 
     __syncthreads();
     const int mc = s_mc;
     const bool touch_all = pd.active || !s_unit;     // every amplitude changes (scale / phase)
-    const u64 stride = (u64)gridDim.x * blockDim.x;
-    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
-        const u64 k = keys[i];
-        const int b = (int)(k & 1ull);
-        int cx = 0;
-        for (int q = 0; q < mc; ++q) cx |= (int)((k >> s_cpos[q]) & 1ull) << q;
-        const int sw = s_sw[cx];
-        bool paired = false;
-        if (b == 0) paired = (i + 1 < n) && keys[i + 1] == (k | 1ull);
-        else paired = (i > 0) && keys[i - 1] == (k & ~1ull);
-        auto load = [&](u64 idx, u64 key) {
-            double2 a = amps[idx];
-            if (pd.active) {
-                if (pend_keep(pd, key, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
-                else { a.x = 0.0; a.y = 0.0; }
+    auto pended = [&](double2 a, u64 key) {
+        if (pd.active) {
+            if (pend_keep(pd, key, a)) { a.x = __dmul_rn(a.x, pd.scale); a.y = __dmul_rn(a.y, pd.scale); }
+            else { a.x = 0.0; a.y = 0.0; }
+        }
+        return a;
+    };
+    auto times = [&](double2 u, double2 a) {
+        if (s_unit) return a;
+        const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
+        const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
+        return make_double2(__dadd_rn(0.0, pr), __dadd_rn(0.0, pi));
+    };
+    // four elements per thread and iteration, all loads of a batch issued before anything is decided
+    const u64 chunk = (u64)SV_THREADS * 4;
+    const u64 nchunks = (n + chunk - 1) / chunk;
+    for (u64 c = blockIdx.x; c < nchunks; c += gridDim.x) {
+        u64 k[4], kn[4], kp[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            k[r] = kn[r] = kp[r] = 0;
+            if (i < n) { k[r] = keys[i]; kn[r] = (i + 1 < n) ? keys[i + 1] : ~k[r]; kp[r] = (i > 0) ? keys[i - 1] : ~k[r]; }
+        }
+        int code[4];            // bit 0: swap, bit 1: paired, bit 2: valid; bits 4..: control block
+        double2 a[4], an[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            int cx = 0;
+            for (int q = 0; q < mc; ++q) cx |= (int)((k[r] >> s_cpos[q]) & 1ull) << q;
+            const int b = (int)(k[r] & 1ull);
+            const bool paired = b ? (kp[r] == (k[r] & ~1ull)) : (kn[r] == (k[r] | 1ull));
+            const int sw = s_sw[cx];
+            code[r] = (i < n ? 4 : 0) | (paired ? 2 : 0) | sw | (cx << 4);
+            a[r] = an[r] = make_double2(0.0, 0.0);
+            if (i < n) {
+                const bool owner = sw && paired && !b;                       // trades the tuple's two amplitudes
+                const bool self = (sw && !paired) ? touch_all : (!sw && touch_all);
+                if (owner || self) a[r] = amps[i];
+                if (owner) an[r] = amps[i + 1];
             }
-            return a;
-        };
-        auto times = [&](double2 u, double2 a) {
-            if (s_unit) return a;
-            const double pr = __dsub_rn(__dmul_rn(u.x, a.x), __dmul_rn(u.y, a.y));
-            const double pi = __dadd_rn(__dmul_rn(u.x, a.y), __dmul_rn(u.y, a.x));
-            return make_double2(__dadd_rn(0.0, pr), __dadd_rn(0.0, pi));
-        };
-        const double2* u = &sU[cx << 2];                 // u[row * 2 + col]
-        if (sw && paired) {
-            if (b == 0) {                                 // both members: trade the amplitudes
-                const double2 a0 = load(i, k), a1 = load(i + 1, k | 1ull);
-                amps[i] = times(u[1], a1);                // row 0 <- column 1
-                amps[i + 1] = times(u[2], a0);            // row 1 <- column 0
+        }
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            if (!(code[r] & 4)) continue;
+            const u64 i = c * chunk + (u64)r * SV_THREADS + threadIdx.x;
+            const int sw = code[r] & 1, b = (int)(k[r] & 1ull);
+            const bool paired = (code[r] & 2) != 0;
+            const double2* u = &sU[(code[r] >> 4) << 2];                    // u[row * 2 + col]
+            if (sw && paired) {
+                if (!b) {
+                    const double2 a0 = pended(a[r], k[r]), a1 = pended(an[r], k[r] | 1ull);
+                    amps[i] = times(u[1], a1);                               // row 0 <- column 1
+                    amps[i + 1] = times(u[2], a0);                           // row 1 <- column 0
+                }
+            } else if (sw) {                                                 // a lone member moves to the other key of its tuple
+                keys[i] = k[r] ^ 1ull;
+                if (touch_all) amps[i] = times(u[((b ^ 1) << 1) | b], pended(a[r], k[r]));
+            } else if (touch_all) {
+                amps[i] = times(u[(b << 1) | b], pended(a[r], k[r]));
             }
-        } else if (sw) {                                  // a lone member moves to the other key of its tuple
-            keys[i] = k ^ 1ull;
-            if (touch_all) amps[i] = times(u[((b ^ 1) << 1) | b], load(i, k));
-        } else if (touch_all) {
-            amps[i] = times(u[(b << 1) | b], load(i, k));
         }
     }
 }
 int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st) {
     if (n == 0) return 0;
     u64 blocks = (n + SV_THREADS * 4 - 1) / (SV_THREADS * 4);
-    if (blocks > (u64)sv_sm_count() * 16) blocks = (u64)sv_sm_count() * 16;
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
     perm_lsb_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, tab, pend);
     return 1;
 }
@@ -156,6 +182,25 @@ __global__ void find_splits_kernel(const u64* __restrict__ keys, u64 n, int p, i
     u64 mlo = (kt & (1ull << p)) ? 0 : t + 1, mhi = (kt & (1ull << p)) ? t : n;
     u64 elo = has_e ? t + 1 : n, ehi = n;                       // keys[t] < nxt: e in [t + 1, n]
     if (!searching) { shi = slo; mhi = mlo; ehi = elo; }
+    // Bounded gallop from t first: when the blocks are small (the moved bit is low) all three bounds lie within a few
+    // elements of t, in cache lines this thread has just touched -- the full-range searches below would instead spend
+    // ~28 scattered reads each.  At most 10 doubling steps per bound; the binary searches then start from the brackets.
+    {
+        const bool mdown = (kt & (1ull << p)) != 0;          // mid lies at or below t
+        bool gs = slo < shi, gm = mlo < mhi, ge = elo < ehi;
+        for (u64 step = 1; step <= 1024 && (gs || gm || ge); step <<= 1) {
+            const u64 cs = (shi > slo + step) ? shi - step : slo;
+            const u64 cm = mdown ? ((mhi > mlo + step) ? mhi - step : mlo) : ((mlo + step - 1 < mhi) ? mlo + step - 1 : mhi - 1);
+            const u64 ce = (elo + step - 1 < ehi) ? elo + step - 1 : ehi - 1;
+            const u64 ks = gs ? keys[cs] : 0, km = gm ? keys[cm] : 0, ke = ge ? keys[ce] : 0;
+            if (gs) { if (ks >= blk) { shi = cs; gs = shi > slo; } else { slo = cs + 1; gs = false; } }
+            if (gm) {
+                if (mdown) { if (km >= vmid) { mhi = cm; gm = mhi > mlo; } else { mlo = cm + 1; gm = false; } }
+                else { if (km < vmid) { mlo = cm + 1; gm = mlo < mhi; } else { mhi = cm; gm = false; } }
+            }
+            if (ge) { if (ke < nxt) { elo = ce + 1; ge = elo < ehi; } else { ehi = ce; ge = false; } }
+        }
+    }
     while (slo < shi || mlo < mhi || elo < ehi) {
         const u64 sm = slo + ((shi - slo) >> 1), mm = mlo + ((mhi - mlo) >> 1), em = elo + ((ehi - elo) >> 1);
         const u64 ks = (slo < shi) ? keys[sm] : 0, km = (mlo < mhi) ? keys[mm] : 0, ke = (elo < ehi) ? keys[em] : 0;

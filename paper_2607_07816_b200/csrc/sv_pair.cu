@@ -274,7 +274,10 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             const u64 base = s_desc[par][0] + s_desc[par][1] - s_desc[par][2];   // merged rank of the tile's first term
             const int mc = PERM ? s_mc : 0;
             const bool phase = PERM && !s_unit;
-            for (int idx = tid; idx < cnt; idx += SV_THREADS) {
+#pragma unroll
+            for (int it = 0; it < BP_VT; ++it) {
+                const int idx = tid + it * SV_THREADS;
+                if (idx >= cnt) break;
                 const u64 key = Wk[BP_SWK(idx)];
                 const u32 code = Wi[BP_SWK(idx)];
                 double2 a = La[code & 0x7fffu];
