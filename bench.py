@@ -283,7 +283,8 @@ def run_ours(args):
             else:
                 sv.apply_gate(g.qubits, g.U)
                 if record:
-                    st = sv.stats(); e1.record()
+                    e1.record()              # (the apply step ends here; stats() is a host-side struct copy)
+                    st = sv.stats()
                 sv.truncate(c.max_terms, c.min_mass)
                 if record:
                     e2.record()

@@ -74,6 +74,19 @@ struct PreCut {
     double mass_hi, mass_lo;
 };
 
+// Small-state path (sv_small.cu): one thread block per gate, count on the device.
+#define SV_SMALL_CAP 4096
+struct SmallGate {
+    int m, xm;              // qubits; the lazy X mask restricted to them (stored local pattern = true pattern ^ xm)
+    int pos[SV_MAX_M];      // physical bit positions of the gate's qubits
+    double2 U[256];         // 2^m x 2^m, row-major in TRUE local indices, as the caller gave it
+};
+struct SmallCtl {
+    u64 count, n_pre;       // terms now; terms after the last gate before its cut
+    int status;             // 1: a gate's input or output did not fit -- the state is that before gate fail_gate
+    int fail_gate, done_gates, pad_;
+};
+
 // stored (physical) key -> logical key.  The map is a bit permutation plus the lazy X mask,
 // hence linear over GF(2): logical = XOR over the 8 bytes b of lut[b * 256 + byte_b(stored)]
 // (the mask is folded into table 0).  lut: DEVICE memory, 8 x 256 u64, built by the host.
@@ -96,6 +109,9 @@ int sv_cur_device(); // ordinal of the current device, clamped to SV_MAX_DEV - 1
 int sv_sm_count();   // SMs of the current device (cached per device)
 // In place: monomial one-bit gate whose active bit is the physical LSB (partners are neighbours); applies a pending cut.
 int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st);
+size_t svk_small_smem();
+int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
+                   double* kept_out, int gate_index, cudaStream_t st);
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----

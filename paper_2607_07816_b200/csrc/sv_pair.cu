@@ -202,9 +202,11 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             }
             __syncthreads();
             const u64 base = s_base;
-            for (int idx = tid; idx < pk_total; idx += SV_THREADS) {
+#pragma unroll
+            for (int it = 0; it < BP_ROUND / SV_THREADS; ++it) {
+                const int idx = tid + it * SV_THREADS;
                 const u64 g = base + (u64)idx;
-                if (g < cap) { st_stream_u64(kout + g, pk_keys[BP_SWK(idx)]); st_stream_d2(aout + g, pk_amps[BP_SWA(idx)]); }
+                if (idx < pk_total && g < cap) { st_stream_u64(kout + g, pk_keys[BP_SWK(idx)]); st_stream_d2(aout + g, pk_amps[BP_SWA(idx)]); }
             }
             __syncthreads();   // the parked arrays are free again (the next loads land in pk_amps)
             pk_valid = false;
@@ -408,9 +410,11 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             __syncthreads();
             const u64 base = s_base + (u64)h0;
             const int m = min(total - h0, BP_ROUND);
-            for (int idx = tid; idx < m; idx += SV_THREADS) {
+#pragma unroll
+            for (int it = 0; it < BP_ROUND / SV_THREADS; ++it) {
+                const int idx = tid + it * SV_THREADS;
                 const u64 g = base + (u64)idx;
-                if (g < cap) { st_stream_u64(kout + g, Wk[BP_SWK(idx)]); st_stream_d2(aout + g, La[BP_SWA(idx)]); }
+                if (idx < m && g < cap) { st_stream_u64(kout + g, Wk[BP_SWK(idx)]); st_stream_d2(aout + g, La[BP_SWA(idx)]); }
             }
         }
         if (!park) __syncthreads();   // A* | B* and this landing buffer are reused (a parked tile's are not, until it is stored)

@@ -1,0 +1,330 @@
+// Small-state path (SURVEY.md hard part H5; after reordering and fusion the paper's own circuit is
+// solved with fewer than 2^5 terms, and its GPU backend shows "a fixed overhead that is apparent at low values of k").
+//
+// A state of at most SV_SMALL_CAP terms whose gate output also fits SV_SMALL_CAP entries is processed by ONE thread
+// block, entirely in shared memory: gate + zero drop + truncation +
+// renormalisation in one launch, with the term count kept ON THE DEVICE.  A sequence of such launches needs no host
+// round trip: sv_apply_circuit (sv_api.cu) enqueues a whole batch of gates back to back and synchronises once.
+//
+// The kernel works on STORED keys in the handle's current layout (which it never changes): the gate's qubits are
+// given as physical bit positions, the lazy X mask as a pattern `xm` that is XORed into the local indices of U.
+//   1. every term finds the other members of its tuple (the terms that differ only in the gate's qubits)
+//      by binary search in the sorted key array; the member with the lowest stored pattern OWNS the tuple;
+//   2. owners compute the 2^m outputs (columns added in ascending logical index, every operation rounded separately:
+//      DESIGN.md D1) into slot (owner rank) * 2^m + row -- or, when every tuple is complete, straight into the
+//      positions of the tuple's own members (same keys, same order: nothing to sort);
+//   3. truncation, if it can cut: bitonic sort of (p descending, logical key ascending), prefix sums of p in that
+//      order, the smallest prefix reaching min_mass * S, capped at max_terms, at least one term; survivors scaled by
+//      1/sqrt(kept mass); nothing dropped -> amplitudes untouched (reading R7);
+//   4. exact zeros dropped, survivors sorted by stored key (bitonic), written back; count and kept
+//      fraction stay on the device.
+// If the input or the output does not fit, the kernel sets ctl->status and leaves the state untouched; every later
+// launch of the batch then does nothing, and the host continues with the streaming passes from that gate.
+// The mass sums here are fp64 tree sums (the streaming path uses exact integer sums, D3): the two agree to ~1e-16
+// relative, so a cut decision can differ only at a knife edge (R22).
+#include "sv_device.cuh"
+#include "sv_launch.cuh"
+
+#define SM_T 1024
+#define SM_PER (SV_SMALL_CAP / SM_T)
+
+struct SmallLayout {
+    u64* ik; double2* ia;      // input terms; later sort keys / scratch
+    u64* ok; double2* oa;      // output terms
+    unsigned short* oidx;      // sort payload
+};
+
+// bitonic sort of P (power of two) entries by (k1, k2) ascending with payload idx; entries with idx == 0xffff are pads
+// and sort last.  TWO: compare k2 on equal k1.
+template <bool TWO>
+__device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, int P) {
+    for (int k = 2; k <= P; k <<= 1) {
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            for (int t = threadIdx.x; t < (P >> 1); t += SM_T) {
+                const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
+                const int l = i | j;
+                const bool up = (i & k) == 0;
+                const u64 a1 = k1[i], b1 = k1[l];
+                const unsigned short ai = idx[i], bi = idx[l];
+                u64 a2 = 0, b2 = 0;
+                if (TWO) { a2 = k2[i]; b2 = k2[l]; }
+                bool a_gt_b;                                   // a sorts after b
+                if (ai == 0xffff || bi == 0xffff) a_gt_b = (ai == 0xffff) && (bi != 0xffff);
+                else a_gt_b = (a1 > b1) || (TWO && a1 == b1 && a2 > b2);
+                const bool b_gt_a = (ai == 0xffff || bi == 0xffff) ? ((bi == 0xffff) && (ai != 0xffff))
+                                                                    : ((b1 > a1) || (TWO && a1 == b1 && b2 > a2));
+                if (up ? a_gt_b : b_gt_a) {
+                    k1[i] = b1; k1[l] = a1; idx[i] = bi; idx[l] = ai;
+                    if (TWO) { k2[i] = b2; k2[l] = a2; }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+// exclusive scan of one int per thread over the block (1024 threads); returns the exclusive prefix, *total the sum
+__device__ __forceinline__ int scan1024(int v, int* red, int* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+    __syncthreads();
+    if (lane == 31) red[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const int w = red[lane];
+        int winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc += t; }
+        red[lane] = winc - w;
+        if (lane == 31) red[32] = winc;
+    }
+    __syncthreads();
+    *total = red[32];
+    return red[warp] + inc - v;
+}
+// the same for doubles, additions only, in a fixed tree (the same bits every run): returns the EXCLUSIVE prefix
+__device__ __forceinline__ double scan1024_excl_d(double v, double* red, double* total) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc = __dadd_rn(inc, t); }
+    double exl = __shfl_up_sync(0xffffffffu, inc, 1);
+    if (lane == 0) exl = 0.0;
+    __syncthreads();
+    if (lane == 31) red[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const double w = red[lane];
+        double winc = w;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc = __dadd_rn(winc, t); }
+        double wex = __shfl_up_sync(0xffffffffu, winc, 1);
+        if (lane == 0) wex = 0.0;
+        red[lane] = wex;
+        if (lane == 31) red[32] = winc;
+    }
+    __syncthreads();
+    *total = red[32];
+    return __dadd_rn(red[warp], exl);
+}
+
+__global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ keys, double2* __restrict__ amps, SmallCtl* __restrict__ ctl,
+                                                             const SmallGate* __restrict__ gate, KeyMap km, u64 max_terms, double min_mass,
+                                                             double* __restrict__ kept_out, int gate_index) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* ia = reinterpret_cast<double2*>(smem_raw);
+    double2* oa = ia + SV_SMALL_CAP;
+    u64* ik = reinterpret_cast<u64*>(oa + SV_SMALL_CAP);
+    u64* ok = ik + SV_SMALL_CAP;
+    unsigned short* oidx = reinterpret_cast<unsigned short*>(ok + SV_SMALL_CAP);
+    __shared__ double2 sU[256];
+    __shared__ int s_pos[SV_MAX_M];
+    __shared__ int red[33];
+    __shared__ double redd[33];
+    __shared__ int s_flag;
+    const int tid = threadIdx.x;
+    if (ctl->status != 0) return;                     // an earlier gate of the batch did not fit: nothing more is done
+    const u64 n64 = ctl->count;
+    if (n64 > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
+    const int n = (int)n64;
+    const int m = gate->m, NP = 1 << m, xm = gate->xm;
+    if (tid < 256) sU[tid] = gate->U[tid];
+    if (tid < SV_MAX_M) s_pos[tid] = gate->pos[tid];
+    if (tid == 0) s_flag = 0;
+    for (int e = tid; e < n; e += SM_T) { ik[e] = keys[e]; ia[e] = amps[e]; }
+    __syncthreads();
+    u64 mask = 0;
+    for (int j = 0; j < m; ++j) mask |= 1ull << s_pos[j];
+    auto scatter = [&](int pat) { u64 v = 0; for (int j = 0; j < m; ++j) v |= (u64)((pat >> j) & 1) << s_pos[j]; return v; };
+    auto find = [&](u64 key) {                        // index of key in ik[0..n), or -1
+        int lo = 0, hi = n;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (ik[mid] < key) lo = mid + 1; else hi = mid; }
+        return (lo < n && ik[lo] == key) ? lo : -1;
+    };
+
+    // ---- 1. owners ----
+    int own[SM_PER];        // 1: element tid + i * SM_T owns its tuple
+    int nown = 0;
+#pragma unroll
+    for (int i = 0; i < SM_PER; ++i) {
+        const int e = tid + i * SM_T;
+        own[i] = 0;
+        if (e < n) {
+            const u64 k = ik[e], base = k & ~mask;
+            int cs = 0;
+            for (int j = 0; j < m; ++j) cs |= (int)((k >> s_pos[j]) & 1ull) << j;
+            bool owner = true;
+            for (int y = 0; y < cs && owner; ++y) if (find(base | scatter(y)) >= 0) owner = false;
+            own[i] = owner ? 1 : 0;
+            nown += own[i];
+        }
+    }
+    // owner ranks in element order: elements are taken strided, so scan per i
+    int orank[SM_PER], n_owners = 0;
+#pragma unroll
+    for (int i = 0; i < SM_PER; ++i) {
+        int tot;
+        const int ex = scan1024(own[i], red, &tot);
+        orank[i] = n_owners + ex;
+        n_owners += tot;
+    }
+    const long long n_slots = (long long)n_owners << m;
+    if (n_slots > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
+    const bool in_place = (n_slots == n);             // every tuple complete: the outputs take the members' own positions
+    // ---- 2. outputs ----
+    int nz_mine = 0;
+#pragma unroll
+    for (int i = 0; i < SM_PER; ++i) {
+        const int e = tid + i * SM_T;
+        if (e < n && own[i]) {
+            const u64 base = ik[e] & ~mask;
+            int mem[16];
+            for (int y = 0; y < 16; ++y) mem[y] = (y < NP) ? find(base | scatter(y)) : -1;
+            for (int r = 0; r < NP; ++r) {             // r, c: TRUE local patterns; stored pattern = true ^ xm
+                double sr = 0.0, si = 0.0;
+                for (int c = 0; c < NP; ++c) {
+                    const int mi = mem[c ^ xm];
+                    if (mi >= 0) {
+                        const double2 a = ia[mi];
+                        const double2 u = sU[r * NP + c];
+                        cmul_acc(sr, si, u.x, u.y, a.x, a.y);
+                    }
+                }
+                const int rs = r ^ xm;
+                int slot;
+                if (in_place) slot = mem[rs];
+                else slot = (orank[i] << m) | rs;
+                ok[slot] = base | scatter(rs);
+                oa[slot] = make_double2(sr, si);
+                nz_mine += (sr == 0.0 && si == 0.0) ? 0 : 1;
+            }
+        }
+    }
+    int n_pre;                                        // nonzero outputs = terms after the gate
+    scan1024(nz_mine, red, &n_pre);
+    const int ns = (int)n_slots;                      // stored outputs (zeros among them)
+    __syncthreads();
+
+    // ---- 3. truncation ----
+    const bool needK = max_terms != 0 && max_terms < (u64)n_pre, needM = min_mass < 1.0;
+    double kept_fraction = 1.0;
+    if ((needK || needM) && n_pre > 0) {
+        int P = 2; while (P < ns) P <<= 1;
+        u64* s1 = ik;                                               // ~pattern of p  (the input arrays are free now)
+        u64* s2 = reinterpret_cast<u64*>(ia);                       // logical key
+        for (int e = tid; e < P; e += SM_T) {
+            if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) {
+                s1[e] = ~(u64)__double_as_longlong(prob_of(oa[e]));
+                s2[e] = logical_key(ok[e], km);
+                oidx[e] = (unsigned short)e;
+            } else { s1[e] = ~0ull; s2[e] = ~0ull; oidx[e] = 0xffff; }
+        }
+        __syncthreads();
+        bitonic<true>(s1, s2, oidx, P);
+        // masses in sorted order: thread t holds ranks t * per .. (consecutive), per = P / SM_T (>= 1) or one rank each
+        const int per = (P + SM_T - 1) / SM_T;
+        double loc = 0.0;
+        for (int q = 0; q < per; ++q) {
+            const int rnk = tid * per + q;
+            if (rnk < n_pre) loc = __dadd_rn(loc, __longlong_as_double((long long)~s1[rnk]));
+        }
+        double S;
+        const double excl = scan1024_excl_d(loc, redd, &S);
+        // j_mass: the smallest j with cum_j >= min_mass * S
+        const double thr = __dmul_rn(min_mass, S);
+        int jm_local = 0x7fffffff;
+        if (needM) {
+            double cum = excl;
+            for (int q = 0; q < per; ++q) {
+                const int rnk = tid * per + q;
+                if (rnk < n_pre) {
+                    cum = __dadd_rn(cum, __longlong_as_double((long long)~s1[rnk]));
+                    if (cum >= thr && jm_local == 0x7fffffff) jm_local = rnk + 1;
+                }
+            }
+        }
+        // block minimum of jm_local
+        if (tid == 0) s_flag = 0x7fffffff;
+        __syncthreads();
+        if (jm_local != 0x7fffffff) atomicMin(&s_flag, jm_local);
+        __syncthreads();
+        int j = n_pre;
+        if (needM && s_flag != 0x7fffffff) j = s_flag;
+        if (max_terms != 0 && (u64)j > max_terms) j = (int)max_terms;
+        if (j < 1) j = 1;
+        __syncthreads();
+        if (j < n_pre) {
+            // kept mass = cum_j
+            double cumj = 0.0;
+            {
+                double cum = excl;
+                bool mine = false;
+                for (int q = 0; q < per; ++q) {
+                    const int rnk = tid * per + q;
+                    if (rnk < n_pre) {
+                        cum = __dadd_rn(cum, __longlong_as_double((long long)~s1[rnk]));
+                        if (rnk + 1 == j) { cumj = cum; mine = true; }
+                    }
+                }
+                if (mine) redd[0] = cumj;
+            }
+            __syncthreads();
+            const double kept = redd[0];
+            const double scale = __ddiv_rn(1.0, __dsqrt_rn(kept));
+            kept_fraction = __ddiv_rn(kept, S);
+            for (int rnk = tid; rnk < n_pre; rnk += SM_T) {
+                const int e = oidx[rnk];
+                if (rnk < j) { oa[e].x = __dmul_rn(oa[e].x, scale); oa[e].y = __dmul_rn(oa[e].y, scale); }
+                else { oa[e].x = 0.0; oa[e].y = 0.0; }                 // dropped: squeezed out with the exact zeros below
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- 4. zero drop, order by stored key, write back ----
+    int n_final;
+    if (in_place) {       // slots are in key order already: stable compaction
+        // elements taken in CONSECUTIVE chunks here so that one scan gives the order
+        const int per = (ns + SM_T - 1) / SM_T;
+        int c = 0;
+        for (int q = 0; q < per; ++q) { const int e = tid * per + q; if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) ++c; }
+        const int ex = scan1024(c, red, &n_final);
+        int w = ex;
+        for (int q = 0; q < per; ++q) {
+            const int e = tid * per + q;
+            if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { keys[w] = ok[e]; amps[w] = oa[e]; ++w; }
+        }
+    } else {
+        int P = 2; while (P < ns) P <<= 1;
+        u64* s1 = ik;
+        for (int e = tid; e < P; e += SM_T) {
+            if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { s1[e] = ok[e]; oidx[e] = (unsigned short)e; }
+            else { s1[e] = ~0ull; oidx[e] = 0xffff; }
+        }
+        __syncthreads();
+        bitonic<false>(s1, nullptr, oidx, P);
+        int c = 0;
+        for (int e = tid; e < P; e += SM_T) c += (oidx[e] != 0xffff) ? 1 : 0;
+        scan1024(c, red, &n_final);
+        for (int e = tid; e < n_final; e += SM_T) { keys[e] = s1[e]; amps[e] = oa[oidx[e]]; }
+    }
+    if (tid == 0) {
+        ctl->count = (u64)n_final;
+        ctl->n_pre = (u64)n_pre;
+        ctl->done_gates = gate_index + 1;
+        if (kept_out) kept_out[gate_index] = kept_fraction;
+    }
+}
+
+size_t svk_small_smem() { return (size_t)SV_SMALL_CAP * (16 + 16 + 8 + 8 + 2); }
+
+int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
+                   double* kept_out, int gate_index, cudaStream_t st) {
+    static bool attr[SV_MAX_DEV];
+    const size_t smem = svk_small_smem();
+    sv_set_smem_once(small_gate_kernel, smem, attr);
+    small_gate_kernel<<<1, SM_T, smem, st>>>(keys, amps, ctl, gate, km, max_terms, min_mass, kept_out, gate_index);
+    return 1;
+}
