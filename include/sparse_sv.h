@@ -55,6 +55,7 @@ typedef struct {
     uint64_t fallbacks;    /* sampled estimates that missed: truncations that re-ran the full select, fused gates that re-ran without a floor */
     uint64_t n_mid;        /* sv_apply_gate_truncate: terms of the gate's output before the cut (logical; not all were written) */
     uint64_t pre_dropped;  /* outputs the last gate did not write because the cut that follows drops them (fused call)          */
+    uint64_t small_gates;  /* gates sv_apply_circuit has run through its single-block path since creation                       */
 } sv_stats;
 
 /* Bytes of device memory a state of this capacity needs (for sv_create_in_arena). */
@@ -101,6 +102,22 @@ int sv_truncate(sv_state *s, uint64_t max_terms, double min_mass, double *kept_f
  * gate, n_out = terms kept. */
 int sv_apply_gate_truncate(sv_state *s, const int *qubits, int m, const sv_c128 *U,
                            uint64_t max_terms, double min_mass, double *kept_fraction);
+
+/* A sequence of gates, each followed by the same truncation ("for each block ... apply ... truncate"), as ONE
+ * call: gate g has gate_m[g] qubits; qubit lists and row-major 2^m x 2^m matrices are concatenated in gate_qubits / gate_U
+ * (conventions of sv_apply_gate; fused blocks from sv_fuse_gates can be passed as they are).  The result is that of
+ * n_gates calls of sv_apply_gate_truncate(.., max_terms, min_mass, ..); kept_fractions (nullable, n_gates doubles) receives
+ * each step's kept mass / mass before.  Knowing the gates ahead, the engine does not return to the host between steps when
+ * it need not: while the state has at most 4096 terms and a gate's output fits 4096 entries, every step is one
+ * single-block kernel (gate + zero drop + cut + renormalisation in shared memory, the term count kept on the device) and a
+ * batch of up to 64 steps costs one synchronisation -- the regime the paper reports after reordering and fusion
+ * (< 2^5 terms; "a fixed overhead ... at low values of k").  Larger states take the streaming passes
+ * gate by gate.  The two paths agree up to the rounding of the mass sums (fp64 tree sums in the single-block kernel, exact
+ * integer sums in the streaming path): a cut can differ only at a knife edge (R22).  *n_done (nullable) receives
+ * the number of gates applied: n_gates on SV_OK; on an error the state is that after *n_done gates.  The whole list is
+ * validated first (SV_ERR_INVALID_ARG then changes nothing).  Synchronises the stream. */
+int sv_apply_circuit(sv_state *s, int n_gates, const int *gate_m, const int *gate_qubits, const sv_c128 *gate_U,
+                     uint64_t max_terms, double min_mass, double *kept_fractions, int *n_done);
 
 /* Gate fusion ("for each block of single- and two-qubit gates we fuse those gates into a
  * multi-qubit unitary operation", one state update and one truncation per block).  HOST ONLY: no device work.
@@ -155,7 +172,7 @@ int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amp
  * truncation cut with the sampled one-pass path (sv_sample_select.cu; default 2^21), smaller
  * ones with the full-state radix select.  Both are exact; tests force either.  The same threshold gates the
  * output floor of sv_apply_gate_truncate. */
-enum { SV_OPT_SAMPLE_MIN_TERMS = 0 };
+enum { SV_OPT_SAMPLE_MIN_TERMS = 0, SV_OPT_SMALL_STATE_PATH = 2 };   /* 2: 1 (default) / 0: sv_apply_circuit may / may not use its single-block path */
 int sv_set_option(sv_state *s, int option, uint64_t value);
 
 /* Statistics of the last call and the launch counter. */

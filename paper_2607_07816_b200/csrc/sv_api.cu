@@ -67,6 +67,9 @@ struct sv_state {
     bool fuse_on;           // sv_apply_gate runs on behalf of sv_apply_gate_truncate
     bool diag_deferred;     // the diagonal gate in s->tab (and the pending cut) has not been applied yet: the truncation's
                             // classification pass applies it in place (sv_sample_select.cu, XF)
+    bool small_on;          // SV_OPT_SMALL_STATE_PATH: sv_apply_circuit may use the single-block path (sv_small.cu)
+    u64 small_gates;        // gates it has taken so far
+    int circuit_done;       // gates the running / last sv_apply_circuit completed
     long long pre_slack;    // sv_test_set_pre_slack: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
@@ -256,6 +259,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->smp_scr = (u32*)(s->arena + L.smp_scr);
     s->seg_cnt = s->arena + L.seg_cnt;
     s->chunk_cnt = (u32*)(s->arena + L.chunk_cnt);
+    s->small_on = true;
     s->sample_min_terms = 1ull << 21;   // below ~2^21 terms the state sits in L2 and the full select has fewer launches
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
@@ -314,6 +318,7 @@ extern "C" int sv_profile_get(sv_state* s, int kernel, sv_kernel_prof* out) {
 extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
+    if (option == SV_OPT_SMALL_STATE_PATH) { s->small_on = value != 0; return SV_OK; }
     return fail(s, SV_ERR_INVALID_ARG, "unknown option");
 }
 // test hook (include/sparse_sv_test.h): sample points added to the margin of the fused call's output floor
@@ -324,6 +329,7 @@ extern "C" int sv_test_set_pre_slack(sv_state* s, long long slack) {
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
     if (!s || !out) return SV_ERR_INVALID_ARG;
+    s->stats.small_gates = s->small_gates;
     *out = s->stats;
     return SV_OK;
 }
@@ -690,6 +696,108 @@ extern "C" int sv_apply_gate_truncate(sv_state* s, const int* qubits, int m, con
     s->stats.passes += tp; s->stats.launches = launches; s->stats.fallbacks = fallbacks;
     s->stats.n_mid = g.n_out;
     if (rc == SV_OK) s->stats.n_out = n_kept;
+    return rc;
+}
+
+// ---------------------------------------------------------------------------------------
+// sv_apply_circuit: a sequence of (gate, truncate) steps with look-ahead (row f-2; small states: H5)
+// ---------------------------------------------------------------------------------------
+#define SV_SMALL_BATCH 64
+static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const int* gate_qubits, const sv_c128* gate_U,
+                              uint64_t max_terms, double min_mass, double* kept_fractions) {
+    // offsets + validation of the whole list up front: an invalid gate anywhere leaves the state untouched
+    size_t qoff = 0, uoff = 0;
+    for (int g = 0; g < n_gates; ++g) {
+        const int m = gate_m[g];
+        if (m < 1 || m > SV_MAX_M) return fail(s, SV_ERR_INVALID_ARG, "sv_apply_circuit: m must be 1..4");
+        u64 seen = 0;
+        for (int j = 0; j < m; ++j) {
+            const int q = gate_qubits[qoff + j];
+            if (q < 0 || q >= s->n || (seen & (1ull << q))) return fail(s, SV_ERR_INVALID_ARG, "sv_apply_circuit: qubit out of range or repeated");
+            seen |= 1ull << q;
+        }
+        qoff += m; uoff += (size_t)1 << (2 * m);
+    }
+    SmallGate* d_gates = reinterpret_cast<SmallGate*>(s->smp_k[0]);           // the sampling scratch is idle here
+    double* d_kept = reinterpret_cast<double*>(s->smp_k[1]);
+    SmallCtl* d_ctl = reinterpret_cast<SmallCtl*>(reinterpret_cast<unsigned char*>(s->smp_k[1]) + 1024);
+    static_assert(sizeof(SmallGate) * SV_SMALL_BATCH <= (size_t)SV_SAMPLE_MAX * 8, "gate batch does not fit the scratch");
+    SmallGate* h_gates = new (std::nothrow) SmallGate[SV_SMALL_BATCH];
+    if (!h_gates) return fail(s, SV_ERR_NOMEM, "sv_apply_circuit: host allocation failed");
+    int rc = SV_OK, g = 0;
+    qoff = 0; uoff = 0;
+    while (g < n_gates && rc == SV_OK) {
+        if (s->small_on && s->count > 0 && s->count <= SV_SMALL_CAP) {
+            // ---- small-state batch: one single-block launch per gate, the count stays on the device ----
+            rc = materialize(s);
+            if (rc != SV_OK) break;
+            const int B = (n_gates - g < SV_SMALL_BATCH) ? n_gates - g : SV_SMALL_BATCH;
+            size_t qo = qoff, uo = uoff;
+            for (int b = 0; b < B; ++b) {
+                const int m = gate_m[g + b], d = 1 << m;
+                SmallGate& sg = h_gates[b];
+                memset(&sg, 0, sizeof(int) * (2 + SV_MAX_M));
+                sg.m = m;
+                for (int j = 0; j < m; ++j) {
+                    const int ph = s->phys_of_log[gate_qubits[qo + j]];
+                    sg.pos[j] = ph;
+                    sg.xm |= (int)((s->xmask >> ph) & 1ull) << j;
+                }
+                for (int i = 0; i < d * d; ++i) sg.U[i] = make_double2(gate_U[uo + i].re, gate_U[uo + i].im);
+                qo += m; uo += (size_t)d * d;
+            }
+            SmallCtl hc;
+            memset(&hc, 0, sizeof(hc));
+            hc.count = s->count; hc.fail_gate = -1;
+            cudaStream_t st = s->stream;
+            const KeyMap km = keymap_of(s);
+            if (cudaMemcpyAsync(d_gates, h_gates, sizeof(SmallGate) * B, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+                cudaMemcpyAsync(d_ctl, &hc, sizeof(hc), cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = cuda_fail(s, cudaGetLastError(), "sv_apply_circuit: upload"); break; }
+            for (int b = 0; b < B; ++b)
+                s->stats.launches += svk_small_gate(s->keys[s->cur], s->amps[s->cur], d_ctl, d_gates + b, km, max_terms, min_mass, d_kept, b, s->cap, st);
+            if (cudaGetLastError() != cudaSuccess) { rc = fail(s, SV_ERR_CUDA, "sv_apply_circuit: kernel launch"); break; }
+            struct { SmallCtl c; double kept[SV_SMALL_BATCH]; } back;
+            // (ctl and the kept fractions are 1 KB apart in one scratch array: two small copies, one synchronisation)
+            if (cudaMemcpyAsync(&back.c, d_ctl, sizeof(SmallCtl), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaMemcpyAsync(back.kept, d_kept, sizeof(double) * B, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaStreamSynchronize(st) != cudaSuccess) { rc = cuda_fail(s, cudaGetLastError(), "sv_apply_circuit: read-back"); break; }
+            const int done = back.c.done_gates;
+            if (done > 0) {
+                s->stats.n_in = s->count; s->stats.n_mid = back.c.n_pre; s->stats.n_out = back.c.count;
+                s->stats.gate_class = SV_CLASS_GROUP; s->stats.m = gate_m[g + done - 1]; s->stats.passes = done; s->stats.pre_dropped = 0;
+                s->count = back.c.count; s->phys = back.c.count;
+                s->mass_est = nan("");
+                s->small_gates += (u64)done;
+            }
+            if (kept_fractions) for (int b = 0; b < done; ++b) kept_fractions[g + b] = back.kept[b];
+            for (int b = 0; b < done; ++b) { qoff += gate_m[g + b]; uoff += (size_t)1 << (2 * gate_m[g + b]); }
+            g += done;
+            if (g >= n_gates || !back.c.status) continue;
+            // gate g (or its output) does not fit one block: the streaming passes take it (and the loop comes back here
+            // if the cut brings the state down again)
+        }
+        double kf = 1.0;
+        rc = sv_apply_gate_truncate(s, gate_qubits + qoff, gate_m[g], gate_U + uoff, max_terms, min_mass, &kf);
+        if (rc != SV_OK) break;
+        if (kept_fractions) kept_fractions[g] = kf;
+        qoff += gate_m[g]; uoff += (size_t)1 << (2 * gate_m[g]);
+        g += 1;
+    }
+    delete[] h_gates;
+    s->circuit_done = g;
+    return rc;
+}
+
+extern "C" int sv_apply_circuit(sv_state* s, int n_gates, const int* gate_m, const int* gate_qubits, const sv_c128* gate_U,
+                                uint64_t max_terms, double min_mass, double* kept_fractions, int* n_done) {
+    if (n_done) *n_done = 0;
+    if (!s) return SV_ERR_INVALID_ARG;
+    if (n_gates < 0 || (n_gates && (!gate_m || !gate_qubits || !gate_U))) return fail(s, SV_ERR_INVALID_ARG, "null argument");
+    if (!(min_mass > 0.0)) return fail(s, SV_ERR_INVALID_ARG, "min_mass must be > 0");
+    s->err[0] = 0;
+    s->circuit_done = 0;
+    const int rc = apply_circuit_impl(s, n_gates, gate_m, gate_qubits, gate_U, max_terms, min_mass, kept_fractions);
+    if (n_done) *n_done = s->circuit_done;
     return rc;
 }
 

@@ -111,7 +111,7 @@ int sv_sm_count();   // SMs of the current device (cached per device)
 int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st);
 size_t svk_small_smem();
 int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
-                   double* kept_out, int gate_index, cudaStream_t st);
+                   double* kept_out, int gate_index, u64 cap, cudaStream_t st);
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----

@@ -28,12 +28,6 @@
 #define SM_T 1024
 #define SM_PER (SV_SMALL_CAP / SM_T)
 
-struct SmallLayout {
-    u64* ik; double2* ia;      // input terms; later sort keys / scratch
-    u64* ok; double2* oa;      // output terms
-    unsigned short* oidx;      // sort payload
-};
-
 // bitonic sort of P (power of two) entries by (k1, k2) ascending with payload idx; entries with idx == 0xffff are pads
 // and sort last.  TWO: compare k2 on equal k1.
 template <bool TWO>
@@ -112,7 +106,7 @@ __device__ __forceinline__ double scan1024_excl_d(double v, double* red, double*
 
 __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ keys, double2* __restrict__ amps, SmallCtl* __restrict__ ctl,
                                                              const SmallGate* __restrict__ gate, KeyMap km, u64 max_terms, double min_mass,
-                                                             double* __restrict__ kept_out, int gate_index) {
+                                                             double* __restrict__ kept_out, int gate_index, u64 cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* ia = reinterpret_cast<double2*>(smem_raw);
     double2* oa = ia + SV_SMALL_CAP;
@@ -205,6 +199,9 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     int n_pre;                                        // nonzero outputs = terms after the gate
     scan1024(nz_mine, red, &n_pre);
     const int ns = (int)n_slots;                      // stored outputs (zeros among them)
+    // (capacity bounds the terms that exist at any instant, a gate's output before its cut included: the streaming path
+    // reports SV_ERR_CAPACITY for this gate)
+    if ((u64)n_pre > cap) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
     __syncthreads();
 
     // ---- 3. truncation ----
@@ -321,10 +318,10 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
 size_t svk_small_smem() { return (size_t)SV_SMALL_CAP * (16 + 16 + 8 + 8 + 2); }
 
 int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
-                   double* kept_out, int gate_index, cudaStream_t st) {
+                   double* kept_out, int gate_index, u64 cap, cudaStream_t st) {
     static bool attr[SV_MAX_DEV];
     const size_t smem = svk_small_smem();
     sv_set_smem_once(small_gate_kernel, smem, attr);
-    small_gate_kernel<<<1, SM_T, smem, st>>>(keys, amps, ctl, gate, km, max_terms, min_mass, kept_out, gate_index);
+    small_gate_kernel<<<1, SM_T, smem, st>>>(keys, amps, ctl, gate, km, max_terms, min_mass, kept_out, gate_index, cap);
     return 1;
 }

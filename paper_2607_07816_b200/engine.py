@@ -19,16 +19,17 @@ CLASS_NAMES = {0: "none", 1: "diagonal", 2: "xor", 3: "group"}
 EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "sv_apply_gate", "sv_truncate",
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
-           "sv_apply_gate_truncate", "sv_fuse_gates", "sv_reorder_gates"]
+           "sv_apply_gate_truncate", "sv_fuse_gates", "sv_reorder_gates", "sv_apply_circuit"]
 TEST_EXPORTS = ["sv_test_set_pre_slack"]      # include/sparse_sv_test.h
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
+OPT_SMALL_STATE_PATH = 2
 
 
 class SvStats(C.Structure):
     _fields_ = [("gate_class", C.c_int), ("m", C.c_int), ("active_bits", C.c_int), ("passes", C.c_int),
                 ("n_in", C.c_uint64), ("n_out", C.c_uint64), ("launches", C.c_uint64), ("fallbacks", C.c_uint64),
-                ("n_mid", C.c_uint64), ("pre_dropped", C.c_uint64)]
+                ("n_mid", C.c_uint64), ("pre_dropped", C.c_uint64), ("small_gates", C.c_uint64)]
 
 
 class SvKernelProf(C.Structure):
@@ -65,6 +66,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_reorder_gates.argtypes = [i32, vp, vp, vp, vp, vp]
     lib.sv_apply_gate_truncate.restype = i32
     lib.sv_apply_gate_truncate.argtypes = [vp, vp, i32, vp, u64, dbl, C.POINTER(dbl)]
+    lib.sv_apply_circuit.restype = i32
+    lib.sv_apply_circuit.argtypes = [vp, i32, vp, vp, vp, u64, dbl, vp, C.POINTER(i32)]
     lib.sv_norm.restype = i32
     lib.sv_norm.argtypes = [vp, C.POINTER(dbl)]
     lib.sv_top.restype = i32
@@ -205,6 +208,24 @@ class SparseSV:
                                              C.byref(kept)))
         return kept.value
 
+    def apply_circuit(self, gates, max_terms: int = 0, min_mass: float = 1.0):
+        """sv_apply_circuit: gates = sequence of (qubits, U); every gate is followed by truncate(max_terms, min_mass).
+        Returns the kept fraction of every step (numpy array).  Argument marshalling only."""
+        gates = list(gates)
+        if not gates:
+            return np.zeros(0)
+        ms = np.array([len(q) for q, _ in gates], dtype=np.int32)
+        qs = np.ascontiguousarray(np.concatenate([np.asarray(q, dtype=np.int32) for q, _ in gates]))
+        for (q, U), m in zip(gates, ms):
+            if np.shape(U) != (1 << m, 1 << m):
+                raise ValueError("U must be 2^m x 2^m")
+        us = np.ascontiguousarray(np.concatenate([np.asarray(U, dtype=np.complex128).reshape(-1) for _, U in gates]))
+        kept = np.ones(len(gates), dtype=np.float64)
+        done = C.c_int(0)
+        self._chk(lib.sv_apply_circuit(self._h, len(gates), ms.ctypes.data, qs.ctypes.data, us.ctypes.data, int(max_terms),
+                                       float(min_mass), kept.ctypes.data, C.byref(done)))
+        return kept
+
     def truncate(self, max_terms: int = 0, min_mass: float = 1.0) -> float:
         kept = C.c_double(1.0)
         self._chk(lib.sv_truncate(self._h, int(max_terms), float(min_mass), C.byref(kept)))
@@ -253,7 +274,8 @@ class SparseSV:
         self._chk(lib.sv_get_stats(self._h, C.byref(st)))
         return {"class": CLASS_NAMES.get(st.gate_class, "?"), "m": st.m, "active_bits": st.active_bits,
                 "passes": st.passes, "n_in": int(st.n_in), "n_out": int(st.n_out), "launches": int(st.launches),
-                "fallbacks": int(st.fallbacks), "n_mid": int(st.n_mid), "pre_dropped": int(st.pre_dropped)}
+                "fallbacks": int(st.fallbacks), "n_mid": int(st.n_mid), "pre_dropped": int(st.pre_dropped),
+                "small_gates": int(st.small_gates)}
 
     def set_option(self, option: int, value: int):
         self._chk(lib.sv_set_option(self._h, int(option), int(value)))
