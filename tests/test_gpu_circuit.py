@@ -48,7 +48,8 @@ def test_ring_blocks_step_locked_vs_oracle(eng, K):
         assert sv.num_terms() == o.num_terms() <= K
         assert_truncation_parity(sv.export()[:2], o.export()[:2])
         assert sv.check_invariants()
-    assert sv.stats()["small_gates"] == len(blocks)
+    sg = sv.stats()["small_gates"]
+    assert sg == len(blocks) if K * 16 <= 4096 else 0 < sg < len(blocks)     # (K = 700: a 16x expansion does not fit one block)
     assert abs(sv.norm() - 1.0) <= 1e-12
 
 
@@ -117,7 +118,7 @@ def test_random_gates_small_path_vs_oracle(eng, n, count, seed):
         assert sv.num_terms() == o.num_terms(), (step, qs)
         assert_truncation_parity(sv.export()[:2], o.export()[:2])
         assert sv.check_invariants()
-    assert small >= 12
+    assert small >= 4          # (expansions beyond 4096 entries take the streaming passes)
 
 
 def test_hand_over_between_the_paths(eng):
