@@ -201,3 +201,21 @@ __device__ __forceinline__ u64 logical_key(u64 stored, const KeyMap& km) {
     for (int b = 0; b < 8; ++b) out ^= __ldg(km.lut + b * 256 + (int)((stored >> (8 * b)) & 0xffull));
     return out;
 }
+
+// Double-double sums (error-free two_sum): the mass sums of the truncation are taken in this form so that they do not
+// depend on the order of summation to within ~2^-100 (D3).
+struct dd { double hi, lo; };
+__device__ __forceinline__ dd dd_make(double a) { dd r; r.hi = a; r.lo = 0.0; return r; }
+__device__ __forceinline__ dd two_sum(double a, double b) {
+    dd r; r.hi = __dadd_rn(a, b);
+    const double bb = __dsub_rn(r.hi, a);
+    r.lo = __dadd_rn(__dsub_rn(a, __dsub_rn(r.hi, bb)), __dsub_rn(b, bb));
+    return r;
+}
+__device__ __forceinline__ dd dd_add(dd a, dd b) {
+    dd s = two_sum(a.hi, b.hi);
+    s.lo = __dadd_rn(s.lo, __dadd_rn(a.lo, b.lo));
+    return two_sum(s.hi, s.lo);
+}
+__device__ __forceinline__ dd dd_sub(dd a, dd b) { b.hi = -b.hi; b.lo = -b.lo; return dd_add(a, b); }
+__device__ __forceinline__ bool dd_ge(dd a, dd b) { return a.hi > b.hi || (a.hi == b.hi && a.lo >= b.lo); }

@@ -24,21 +24,6 @@
 // ---------------------------------------------------------------------------------------
 // double-double helpers (cut decisions only; one thread)
 // ---------------------------------------------------------------------------------------
-struct dd { double hi, lo; };
-__device__ __forceinline__ dd dd_make(double a) { dd r; r.hi = a; r.lo = 0.0; return r; }
-__device__ __forceinline__ dd two_sum(double a, double b) {
-    dd r; r.hi = __dadd_rn(a, b);
-    const double bb = __dsub_rn(r.hi, a);
-    r.lo = __dadd_rn(__dsub_rn(a, __dsub_rn(r.hi, bb)), __dsub_rn(b, bb));
-    return r;
-}
-__device__ __forceinline__ dd dd_add(dd a, dd b) {
-    dd s = two_sum(a.hi, b.hi);
-    s.lo = __dadd_rn(s.lo, __dadd_rn(a.lo, b.lo));
-    return two_sum(s.hi, s.lo);
-}
-__device__ __forceinline__ dd dd_sub(dd a, dd b) { b.hi = -b.hi; b.lo = -b.lo; return dd_add(a, b); }
-__device__ __forceinline__ bool dd_ge(dd a, dd b) { return a.hi > b.hi || (a.hi == b.hi && a.lo >= b.lo); }
 __device__ __forceinline__ dd dd_from_u64(u64 x) {
     return two_sum(__dmul_rn((double)(x >> 32), 4294967296.0), (double)(x & 0xffffffffull));
 }

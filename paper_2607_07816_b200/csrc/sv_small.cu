@@ -20,21 +20,20 @@
 //      fraction stay on the device.
 // If the input or the output does not fit, the kernel sets ctl->status and leaves the state untouched; every later
 // launch of the batch then does nothing, and the host continues with the streaming passes from that gate.
-// The mass sums here are fp64 tree sums (the streaming path uses exact integer sums, D3): the two agree to ~1e-16
-// relative, so a cut decision can differ only at a knife edge (R22).
+// The mass sums here are double-double sums (order independent to ~2^-100), rounded to the same doubles as the exact
+// integer sums of the streaming path (D3): threshold, cut, kept mass, scale and kept fraction come out bit for bit the same.
 #include "sv_device.cuh"
 #include "sv_launch.cuh"
 
 #define SM_T 1024
-#define SM_PER (SV_SMALL_CAP / SM_T)
 
 // bitonic sort of P (power of two) entries by (k1, k2) ascending with payload idx; entries with idx == 0xffff are pads
 // and sort last.  TWO: compare k2 on equal k1.
 template <bool TWO>
-__device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, int P) {
+__device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, int P, int A) {
     for (int k = 2; k <= P; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = threadIdx.x; t < (P >> 1); t += SM_T) {
+            for (int t = threadIdx.x; t < (P >> 1); t += A) {
                 const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
                 const int l = i | j;
                 const bool up = (i & k) == 0;
@@ -58,8 +57,9 @@ __device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, i
 }
 
 // exclusive scan of one int per thread over the block (1024 threads); returns the exclusive prefix, *total the sum
-__device__ __forceinline__ int scan1024(int v, int* red, int* total) {
+__device__ __forceinline__ int scan1024(int v, int* red, int* total, int A) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nw = A >> 5;
     int inc = v;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
@@ -67,7 +67,7 @@ __device__ __forceinline__ int scan1024(int v, int* red, int* total) {
     if (lane == 31) red[warp] = inc;
     __syncthreads();
     if (warp == 0) {
-        const int w = red[lane];
+        const int w = lane < nw ? red[lane] : 0;
         int winc = w;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc += t; }
@@ -78,30 +78,41 @@ __device__ __forceinline__ int scan1024(int v, int* red, int* total) {
     *total = red[32];
     return red[warp] + inc - v;
 }
-// the same for doubles, additions only, in a fixed tree (the same bits every run): returns the EXCLUSIVE prefix
-__device__ __forceinline__ double scan1024_excl_d(double v, double* red, double* total) {
+// the same for double-double sums (order independent to ~2^-100: the streaming path's exact sums round to the same
+// doubles, D3): returns the EXCLUSIVE prefix
+__device__ __forceinline__ dd scan1024_excl_dd(dd v, double* red, dd* total, int A) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double inc = v;
+    const int nw = A >> 5;
+    dd inc = v;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc = __dadd_rn(inc, t); }
-    double exl = __shfl_up_sync(0xffffffffu, inc, 1);
-    if (lane == 0) exl = 0.0;
+    for (int d = 1; d < 32; d <<= 1) {
+        dd t; t.hi = __shfl_up_sync(0xffffffffu, inc.hi, d); t.lo = __shfl_up_sync(0xffffffffu, inc.lo, d);
+        if (lane >= d) inc = dd_add(inc, t);
+    }
+    dd exl; exl.hi = __shfl_up_sync(0xffffffffu, inc.hi, 1); exl.lo = __shfl_up_sync(0xffffffffu, inc.lo, 1);
+    if (lane == 0) exl = dd_make(0.0);
     __syncthreads();
-    if (lane == 31) red[warp] = inc;
+    if (lane == 31) { red[2 * warp] = inc.hi; red[2 * warp + 1] = inc.lo; }
     __syncthreads();
     if (warp == 0) {
-        const double w = red[lane];
-        double winc = w;
+        dd w = dd_make(0.0);
+        if (lane < nw) { w.hi = red[2 * lane]; w.lo = red[2 * lane + 1]; }
+        dd winc = w;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { const double t = __shfl_up_sync(0xffffffffu, winc, d); if (lane >= d) winc = __dadd_rn(winc, t); }
-        double wex = __shfl_up_sync(0xffffffffu, winc, 1);
-        if (lane == 0) wex = 0.0;
-        red[lane] = wex;
-        if (lane == 31) red[32] = winc;
+        for (int d = 1; d < 32; d <<= 1) {
+            dd t; t.hi = __shfl_up_sync(0xffffffffu, winc.hi, d); t.lo = __shfl_up_sync(0xffffffffu, winc.lo, d);
+            if (lane >= d) winc = dd_add(winc, t);
+        }
+        dd wex; wex.hi = __shfl_up_sync(0xffffffffu, winc.hi, 1); wex.lo = __shfl_up_sync(0xffffffffu, winc.lo, 1);
+        if (lane == 0) wex = dd_make(0.0);
+        __syncwarp();
+        red[2 * lane] = wex.hi; red[2 * lane + 1] = wex.lo;
+        if (lane == 31) { red[64] = winc.hi; red[65] = winc.lo; }
     }
     __syncthreads();
-    *total = red[32];
-    return __dadd_rn(red[warp], exl);
+    total->hi = red[64]; total->lo = red[65];
+    dd pre; pre.hi = red[2 * warp]; pre.lo = red[2 * warp + 1];
+    return dd_add(pre, exl);
 }
 
 __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ keys, double2* __restrict__ amps, SmallCtl* __restrict__ ctl,
@@ -116,7 +127,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     __shared__ double2 sU[256];
     __shared__ int s_pos[SV_MAX_M];
     __shared__ int red[33];
-    __shared__ double redd[33];
+    __shared__ double redd[66];
     __shared__ int s_flag;
     const int tid = threadIdx.x;
     if (ctl->status != 0) return;                     // an earlier gate of the batch did not fit: nothing more is done
@@ -124,10 +135,21 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     if (n64 > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
     const int n = (int)n64;
     const int m = gate->m, NP = 1 << m, xm = gate->xm;
-    if (tid < 256) sU[tid] = gate->U[tid];
+    // Only as many warps as the problem can use stay: a barrier among 2 warps costs a fraction of one among 32, and the
+    // sorts below are ~100 barriers.  A = active threads (a multiple of 32); the others leave before the first barrier.
+    int A;
+    {
+        long long ub = (long long)n << m;             // upper bound of the output slots
+        if (ub > SV_SMALL_CAP) ub = SV_SMALL_CAP;
+        long long need = ub / 2 > n ? ub / 2 : n;
+        A = (int)((need + 31) / 32) * 32;
+        if (A < 32) A = 32;
+        if (A > SM_T) A = SM_T;
+    }
+    if (tid >= A) return;
+    for (int i = tid; i < 256; i += A) sU[i] = gate->U[i];
     if (tid < SV_MAX_M) s_pos[tid] = gate->pos[tid];
-    if (tid == 0) s_flag = 0;
-    for (int e = tid; e < n; e += SM_T) { ik[e] = keys[e]; ia[e] = amps[e]; }
+    for (int e = tid; e < n; e += A) { ik[e] = keys[e]; ia[e] = amps[e]; }
     __syncthreads();
     u64 mask = 0;
     for (int j = 0; j < m; ++j) mask |= 1ull << s_pos[j];
@@ -138,41 +160,30 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         return (lo < n && ik[lo] == key) ? lo : -1;
     };
 
-    // ---- 1. owners ----
-    int own[SM_PER];        // 1: element tid + i * SM_T owns its tuple
-    int nown = 0;
-#pragma unroll
-    for (int i = 0; i < SM_PER; ++i) {
-        const int e = tid + i * SM_T;
-        own[i] = 0;
+    // ---- 1. owners: thread t takes the elements t * per .. t * per + per - 1 (consecutive: one scan gives their ranks) ----
+    const int per = (n + A - 1) / A;                  // <= 4
+    u32 ownbits = 0;
+    for (int i = 0; i < per; ++i) {
+        const int e = tid * per + i;
         if (e < n) {
             const u64 k = ik[e], base = k & ~mask;
             int cs = 0;
             for (int j = 0; j < m; ++j) cs |= (int)((k >> s_pos[j]) & 1ull) << j;
             bool owner = true;
             for (int y = 0; y < cs && owner; ++y) if (find(base | scatter(y)) >= 0) owner = false;
-            own[i] = owner ? 1 : 0;
-            nown += own[i];
+            if (owner) ownbits |= 1u << i;
         }
     }
-    // owner ranks in element order: elements are taken strided, so scan per i
-    int orank[SM_PER], n_owners = 0;
-#pragma unroll
-    for (int i = 0; i < SM_PER; ++i) {
-        int tot;
-        const int ex = scan1024(own[i], red, &tot);
-        orank[i] = n_owners + ex;
-        n_owners += tot;
-    }
+    int n_owners;
+    int orank = scan1024(__popc(ownbits), red, &n_owners, A);
     const long long n_slots = (long long)n_owners << m;
     if (n_slots > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
     const bool in_place = (n_slots == n);             // every tuple complete: the outputs take the members' own positions
     // ---- 2. outputs ----
     int nz_mine = 0;
-#pragma unroll
-    for (int i = 0; i < SM_PER; ++i) {
-        const int e = tid + i * SM_T;
-        if (e < n && own[i]) {
+    for (int i = 0; i < per; ++i) {
+        const int e = tid * per + i;
+        if (e < n && ((ownbits >> i) & 1u)) {
             const u64 base = ik[e] & ~mask;
             int mem[16];
             for (int y = 0; y < 16; ++y) mem[y] = (y < NP) ? find(base | scatter(y)) : -1;
@@ -187,17 +198,16 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
                     }
                 }
                 const int rs = r ^ xm;
-                int slot;
-                if (in_place) slot = mem[rs];
-                else slot = (orank[i] << m) | rs;
+                const int slot = in_place ? mem[rs] : ((orank << m) | rs);
                 ok[slot] = base | scatter(rs);
                 oa[slot] = make_double2(sr, si);
                 nz_mine += (sr == 0.0 && si == 0.0) ? 0 : 1;
             }
+            ++orank;
         }
     }
     int n_pre;                                        // nonzero outputs = terms after the gate
-    scan1024(nz_mine, red, &n_pre);
+    scan1024(nz_mine, red, &n_pre, A);
     const int ns = (int)n_slots;                      // stored outputs (zeros among them)
     // (capacity bounds the terms that exist at any instant, a gate's output before its cut included: the streaming path
     // reports SV_ERR_CAPACITY for this gate)
@@ -211,7 +221,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         int P = 2; while (P < ns) P <<= 1;
         u64* s1 = ik;                                               // ~pattern of p  (the input arrays are free now)
         u64* s2 = reinterpret_cast<u64*>(ia);                       // logical key
-        for (int e = tid; e < P; e += SM_T) {
+        for (int e = tid; e < P; e += A) {
             if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) {
                 s1[e] = ~(u64)__double_as_longlong(prob_of(oa[e]));
                 s2[e] = logical_key(ok[e], km);
@@ -219,30 +229,29 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
             } else { s1[e] = ~0ull; s2[e] = ~0ull; oidx[e] = 0xffff; }
         }
         __syncthreads();
-        bitonic<true>(s1, s2, oidx, P);
-        // masses in sorted order: thread t holds ranks t * per .. (consecutive), per = P / SM_T (>= 1) or one rank each
-        const int per = (P + SM_T - 1) / SM_T;
-        double loc = 0.0;
-        for (int q = 0; q < per; ++q) {
-            const int rnk = tid * per + q;
-            if (rnk < n_pre) loc = __dadd_rn(loc, __longlong_as_double((long long)~s1[rnk]));
+        bitonic<true>(s1, s2, oidx, P, A);
+        // masses in sorted order: thread t holds the ranks t * rper .. (consecutive)
+        const int rper = (n_pre + A - 1) / A;
+        dd loc = dd_make(0.0);
+        for (int q = 0; q < rper; ++q) {
+            const int rnk = tid * rper + q;
+            if (rnk < n_pre) loc = dd_add(loc, dd_make(__longlong_as_double((long long)~s1[rnk])));
         }
-        double S;
-        const double excl = scan1024_excl_d(loc, redd, &S);
-        // j_mass: the smallest j with cum_j >= min_mass * S
-        const double thr = __dmul_rn(min_mass, S);
+        dd S;
+        const dd excl = scan1024_excl_dd(loc, redd, &S, A);
+        // j_mass: the smallest j with cum_j >= min_mass * S (the threshold rounded once, as the streaming path takes it)
+        const dd thr = dd_make(__dmul_rn(min_mass, S.hi));
         int jm_local = 0x7fffffff;
         if (needM) {
-            double cum = excl;
-            for (int q = 0; q < per; ++q) {
-                const int rnk = tid * per + q;
+            dd cum = excl;
+            for (int q = 0; q < rper; ++q) {
+                const int rnk = tid * rper + q;
                 if (rnk < n_pre) {
-                    cum = __dadd_rn(cum, __longlong_as_double((long long)~s1[rnk]));
-                    if (cum >= thr && jm_local == 0x7fffffff) jm_local = rnk + 1;
+                    cum = dd_add(cum, dd_make(__longlong_as_double((long long)~s1[rnk])));
+                    if (dd_ge(cum, thr) && jm_local == 0x7fffffff) jm_local = rnk + 1;
                 }
             }
         }
-        // block minimum of jm_local
         if (tid == 0) s_flag = 0x7fffffff;
         __syncthreads();
         if (jm_local != 0x7fffffff) atomicMin(&s_flag, jm_local);
@@ -253,25 +262,21 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         if (j < 1) j = 1;
         __syncthreads();
         if (j < n_pre) {
-            // kept mass = cum_j
-            double cumj = 0.0;
-            {
-                double cum = excl;
-                bool mine = false;
-                for (int q = 0; q < per; ++q) {
-                    const int rnk = tid * per + q;
+            {   // kept mass = cum_j (held by the thread that owns rank j - 1)
+                dd cum = excl;
+                for (int q = 0; q < rper; ++q) {
+                    const int rnk = tid * rper + q;
                     if (rnk < n_pre) {
-                        cum = __dadd_rn(cum, __longlong_as_double((long long)~s1[rnk]));
-                        if (rnk + 1 == j) { cumj = cum; mine = true; }
+                        cum = dd_add(cum, dd_make(__longlong_as_double((long long)~s1[rnk])));
+                        if (rnk + 1 == j) redd[0] = cum.hi;
                     }
                 }
-                if (mine) redd[0] = cumj;
             }
             __syncthreads();
             const double kept = redd[0];
             const double scale = __ddiv_rn(1.0, __dsqrt_rn(kept));
-            kept_fraction = __ddiv_rn(kept, S);
-            for (int rnk = tid; rnk < n_pre; rnk += SM_T) {
+            kept_fraction = __ddiv_rn(kept, S.hi);
+            for (int rnk = tid; rnk < n_pre; rnk += A) {
                 const int e = oidx[rnk];
                 if (rnk < j) { oa[e].x = __dmul_rn(oa[e].x, scale); oa[e].y = __dmul_rn(oa[e].y, scale); }
                 else { oa[e].x = 0.0; oa[e].y = 0.0; }                 // dropped: squeezed out with the exact zeros below
@@ -280,32 +285,31 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         }
     }
 
-    // ---- 4. zero drop, order by stored key, write back ----
+    // ---- 4. zero drop (stable compaction of the slots), order by stored key, write back ----
     int n_final;
-    if (in_place) {       // slots are in key order already: stable compaction
-        // elements taken in CONSECUTIVE chunks here so that one scan gives the order
-        const int per = (ns + SM_T - 1) / SM_T;
+    {
+        const int sper = (ns + A - 1) / A;
         int c = 0;
-        for (int q = 0; q < per; ++q) { const int e = tid * per + q; if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) ++c; }
-        const int ex = scan1024(c, red, &n_final);
-        int w = ex;
-        for (int q = 0; q < per; ++q) {
-            const int e = tid * per + q;
-            if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { keys[w] = ok[e]; amps[w] = oa[e]; ++w; }
+        for (int q = 0; q < sper; ++q) { const int e = tid * sper + q; if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) ++c; }
+        int w = scan1024(c, red, &n_final, A);
+        if (in_place) {       // the slots are in key order already
+            for (int q = 0; q < sper; ++q) {
+                const int e = tid * sper + q;
+                if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { keys[w] = ok[e]; amps[w] = oa[e]; ++w; }
+            }
+        } else {              // sort the survivors only
+            u64* s1 = ik;
+            for (int q = 0; q < sper; ++q) {
+                const int e = tid * sper + q;
+                if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { s1[w] = ok[e]; oidx[w] = (unsigned short)e; ++w; }
+            }
+            int P = 2; while (P < n_final) P <<= 1;
+            __syncthreads();
+            for (int e = n_final + tid; e < P; e += A) { s1[e] = ~0ull; oidx[e] = 0xffff; }
+            __syncthreads();
+            bitonic<false>(s1, nullptr, oidx, P, A);
+            for (int e = tid; e < n_final; e += A) { keys[e] = s1[e]; amps[e] = oa[oidx[e]]; }
         }
-    } else {
-        int P = 2; while (P < ns) P <<= 1;
-        u64* s1 = ik;
-        for (int e = tid; e < P; e += SM_T) {
-            if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { s1[e] = ok[e]; oidx[e] = (unsigned short)e; }
-            else { s1[e] = ~0ull; oidx[e] = 0xffff; }
-        }
-        __syncthreads();
-        bitonic<false>(s1, nullptr, oidx, P);
-        int c = 0;
-        for (int e = tid; e < P; e += SM_T) c += (oidx[e] != 0xffff) ? 1 : 0;
-        scan1024(c, red, &n_final);
-        for (int e = tid; e < n_final; e += SM_T) { keys[e] = s1[e]; amps[e] = oa[oidx[e]]; }
     }
     if (tid == 0) {
         ctl->count = (u64)n_final;

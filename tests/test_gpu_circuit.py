@@ -123,8 +123,9 @@ def test_random_gates_small_path_vs_oracle(eng, n, count, seed):
 
 def test_hand_over_between_the_paths(eng):
     """Scaled configs[4] (K = 2^13): the state grows through the small-state limit, is cut back, grows again.  One call for
-    the whole list must agree with the gate-by-gate streaming calls (small path off): same term counts after the list,
-    kept fractions to 1e-10, states to 1e-11 on the kept keys (the two paths round their mass sums differently)."""
+    the whole list must give THE BITS of the gate-by-gate streaming calls (small path off): the single-block kernel takes
+    its mass sums in double-double, which round to the doubles of the streaming path's exact sums (D3), so
+    threshold, cut, scale and every later exact cancellation are the same -- 160 gates free-running."""
     c = W.config5(num_gates=160, max_terms=1 << 13)
     gl = [(g.qubits, g.U) for g in c.gates]
     a, b = eng.SparseSV(c.n, 1 << 17), eng.SparseSV(c.n, 1 << 17)
@@ -132,9 +133,9 @@ def test_hand_over_between_the_paths(eng):
     ka = a.apply_circuit(gl, c.max_terms, c.min_mass)
     kb = b.apply_circuit(gl, c.max_terms, c.min_mass)
     assert 0 < a.stats()["small_gates"] < len(gl) and b.stats()["small_gates"] == 0
-    assert np.max(np.abs(ka - kb)) <= MASS_TOL
-    assert a.num_terms() == b.num_terms()
-    assert_truncation_parity(a.export()[:2], b.export()[:2])
+    assert np.array_equal(ka, kb)
+    ea, eb = a.export(), b.export()
+    assert np.array_equal(ea[0], eb[0]) and np.array_equal(ea[1], eb[1])
     assert a.check_invariants()
 
 
