@@ -174,7 +174,11 @@ def run_circuits(engine, W, dev, torch):
             torch.cuda.synchronize(); a.record()
             log_kept, peak_terms = 0.0, 1
             try:
-                for g in c.gates:
+                if name in ("cfg1", "cfg2"):     # small / mid-size states: the whole list as ONE call (sv_apply_circuit, look-ahead)
+                    kf = sv.apply_circuit([(g.qubits, g.U) for g in c.gates], c.max_terms if c.truncate_every_gate else 0,
+                                          c.min_mass if c.truncate_every_gate else 1.0)
+                    log_kept = float(np.sum(np.log(kf)))
+                for g in (c.gates if name not in ("cfg1", "cfg2") else []):
                     if c.truncate_every_gate:
                         kept = sv.apply_gate_truncate(g.qubits, g.U, c.max_terms, c.min_mass)
                         peak_terms = max(peak_terms, sv.stats()["n_mid"])
@@ -185,7 +189,7 @@ def run_circuits(engine, W, dev, torch):
                 k, _, p = sv.top(1)
                 res = {"n_qubits": c.n, "gates": len(c.gates), "wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(),
                        "peak_terms_before_cut": int(peak_terms), "log_retained_mass": log_kept, "top_p": float(p[0]),
-                       "norm": sv.norm(), "select_fallbacks": sv.stats()["fallbacks"],
+                       "norm": sv.norm(), "select_fallbacks": sv.stats()["fallbacks"], "small_path_gates": sv.stats()["small_gates"],
                        "top_is_secret": (int(k[0]) == c.secret) if c.secret is not None else None,
                        "variant": c.notes.get("variant")}
             except engine.SvError as ex:
@@ -217,13 +221,12 @@ def run_ring_scaling(engine, W, dev, torch):
                 sv = engine.SparseSV(c.n, 16 * K, device=dev)
                 a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 torch.cuda.synchronize(); a.record()
-                log_kept = 0.0
-                for q, U in blocks:
-                    log_kept += float(np.log(sv.apply_gate_truncate(q, U, K, 1.0)))
+                log_kept = float(np.sum(np.log(sv.apply_circuit(blocks, K, 1.0))))      # one call for the whole circuit
                 b.record(); torch.cuda.synchronize()
                 k, _, p = sv.top(1)
                 r = {"wall_ms": a.elapsed_time(b), "final_terms": sv.num_terms(), "log_retained_mass": log_kept,
-                     "top_p": float(p[0]), "top_is_secret": int(k[0]) == c.secret, "select_fallbacks": sv.stats()["fallbacks"]}
+                     "top_p": float(p[0]), "top_is_secret": int(k[0]) == c.secret, "select_fallbacks": sv.stats()["fallbacks"],
+                     "small_path_gates": sv.stats()["small_gates"]}
                 sv.close()
             res["by_K_log2"][str(klog)] = r
         except engine.SvError as ex:

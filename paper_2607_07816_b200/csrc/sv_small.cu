@@ -124,17 +124,25 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     u64* ik = reinterpret_cast<u64*>(oa + SV_SMALL_CAP);
     u64* ok = ik + SV_SMALL_CAP;
     unsigned short* oidx = reinterpret_cast<unsigned short*>(ok + SV_SMALL_CAP);
+    unsigned short* oelem = oidx + SV_SMALL_CAP;       // element index of the owner of every tuple
     __shared__ double2 sU[256];
     __shared__ int s_pos[SV_MAX_M];
     __shared__ int red[33];
     __shared__ double redd[66];
     __shared__ int s_flag;
     const int tid = threadIdx.x;
-    if (ctl->status != 0) return;                     // an earlier gate of the batch did not fit: nothing more is done
+    // (all the independent global reads of the prologue are issued together: each is a ~1 us round trip on its own)
+    const int status0 = ctl->status;
     const u64 n64 = ctl->count;
+    const int m = gate->m, xm = gate->xm;
+    const int pos_t = tid < SV_MAX_M ? gate->pos[tid] : 0;
+    const double2 u_t = tid < 256 ? gate->U[tid] : make_double2(0.0, 0.0);
+    if (status0 != 0) return;                         // an earlier gate of the batch did not fit: nothing more is done
     if (n64 > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
     const int n = (int)n64;
-    const int m = gate->m, NP = 1 << m, xm = gate->xm;
+    const int NP = 1 << m;
+    if (tid < 256) sU[tid] = u_t;
+    if (tid < SV_MAX_M) s_pos[tid] = pos_t;
     // Only as many warps as the problem can use stay: a barrier among 2 warps costs a fraction of one among 32, and the
     // sorts below are ~100 barriers.  A = active threads (a multiple of 32); the others leave before the first barrier.
     int A;
@@ -143,12 +151,10 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         if (ub > SV_SMALL_CAP) ub = SV_SMALL_CAP;
         long long need = ub / 2 > n ? ub / 2 : n;
         A = (int)((need + 31) / 32) * 32;
-        if (A < 32) A = 32;
+        if (A < 256) A = 256;                        // (the first 256 threads also fill the gate table)
         if (A > SM_T) A = SM_T;
     }
     if (tid >= A) return;
-    for (int i = tid; i < 256; i += A) sU[i] = gate->U[i];
-    if (tid < SV_MAX_M) s_pos[tid] = gate->pos[tid];
     for (int e = tid; e < n; e += A) { ik[e] = keys[e]; ia[e] = amps[e]; }
     __syncthreads();
     u64 mask = 0;
@@ -160,55 +166,60 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         return (lo < n && ik[lo] == key) ? lo : -1;
     };
 
-    // ---- 1. owners: thread t takes the elements t * per .. t * per + per - 1 (consecutive: one scan gives their ranks) ----
-    const int per = (n + A - 1) / A;                  // <= 4
-    u32 ownbits = 0;
-    for (int i = 0; i < per; ++i) {
-        const int e = tid * per + i;
-        if (e < n) {
-            const u64 k = ik[e], base = k & ~mask;
-            int cs = 0;
-            for (int j = 0; j < m; ++j) cs |= (int)((k >> s_pos[j]) & 1ull) << j;
-            bool owner = true;
-            for (int y = 0; y < cs && owner; ++y) if (find(base | scatter(y)) >= 0) owner = false;
-            if (owner) ownbits |= 1u << i;
-        }
+    // ---- 1. owners.  Every step is spread over all active threads (a few threads walking whole tuples serially would
+    // leave the other warps waiting at the barriers) ----
+    // 1a: element e is NOT an owner iff some member with a lower stored pattern exists: one search per (element, pattern)
+    for (int e = tid; e < n; e += A) oidx[e] = 0;
+    __syncthreads();
+    for (int t = tid; t < (n << m); t += A) {
+        const int e = t >> m, y = t & (NP - 1);
+        const u64 k = ik[e];
+        int cs = 0;
+        for (int j = 0; j < m; ++j) cs |= (int)((k >> s_pos[j]) & 1ull) << j;
+        if (y < cs && find((k & ~mask) | scatter(y)) >= 0) oidx[e] = 1;      // (racing writers all write 1)
     }
+    __syncthreads();
+    // 1b: owner ranks in key order (thread t takes the elements t * per .. consecutively: one scan)
+    const int per = (n + A - 1) / A;                  // <= 4
+    int cown = 0;
+    for (int i = 0; i < per; ++i) { const int e = tid * per + i; if (e < n && !oidx[e]) ++cown; }
     int n_owners;
-    int orank = scan1024(__popc(ownbits), red, &n_owners, A);
+    int orank = scan1024(cown, red, &n_owners, A);
     const long long n_slots = (long long)n_owners << m;
     if (n_slots > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
+    for (int i = 0; i < per; ++i) { const int e = tid * per + i; if (e < n && !oidx[e]) oelem[orank++] = (unsigned short)e; }
     const bool in_place = (n_slots == n);             // every tuple complete: the outputs take the members' own positions
-    // ---- 2. outputs ----
+    const int ns = (int)n_slots;                      // output slots (exact zeros among them)
+    __syncthreads();
+    // 1c: the members of every owner's tuple: memtab[owner * 2^m + stored pattern] = element index, 0xffff if absent
+    unsigned short* memtab = oidx;
+    for (int t = tid; t < ns; t += A) {
+        const int o = t >> m, y = t & (NP - 1);
+        const int f = find((ik[oelem[o]] & ~mask) | scatter(y));
+        memtab[t] = (unsigned short)(f < 0 ? 0xffff : f);
+    }
+    __syncthreads();
+    // ---- 2. outputs: one task per (tuple, row) ----
     int nz_mine = 0;
-    for (int i = 0; i < per; ++i) {
-        const int e = tid * per + i;
-        if (e < n && ((ownbits >> i) & 1u)) {
-            const u64 base = ik[e] & ~mask;
-            int mem[16];
-            for (int y = 0; y < 16; ++y) mem[y] = (y < NP) ? find(base | scatter(y)) : -1;
-            for (int r = 0; r < NP; ++r) {             // r, c: TRUE local patterns; stored pattern = true ^ xm
-                double sr = 0.0, si = 0.0;
-                for (int c = 0; c < NP; ++c) {
-                    const int mi = mem[c ^ xm];
-                    if (mi >= 0) {
-                        const double2 a = ia[mi];
-                        const double2 u = sU[r * NP + c];
-                        cmul_acc(sr, si, u.x, u.y, a.x, a.y);
-                    }
-                }
-                const int rs = r ^ xm;
-                const int slot = in_place ? mem[rs] : ((orank << m) | rs);
-                ok[slot] = base | scatter(rs);
-                oa[slot] = make_double2(sr, si);
-                nz_mine += (sr == 0.0 && si == 0.0) ? 0 : 1;
+    for (int t = tid; t < ns; t += A) {
+        const int o = t >> m, rs = t & (NP - 1), r = rs ^ xm;     // r, c: TRUE local patterns; stored pattern = true ^ xm
+        const u64 base = ik[oelem[o]] & ~mask;
+        double sr = 0.0, si = 0.0;
+        for (int c = 0; c < NP; ++c) {                             // ascending logical column (D1); absent members skipped
+            const unsigned short mi = memtab[(o << m) | (c ^ xm)];
+            if (mi != 0xffff) {
+                const double2 a = ia[mi];
+                const double2 u = sU[r * NP + c];
+                cmul_acc(sr, si, u.x, u.y, a.x, a.y);
             }
-            ++orank;
         }
+        const int slot = in_place ? (int)memtab[t] : t;
+        ok[slot] = base | scatter(rs);
+        oa[slot] = make_double2(sr, si);
+        nz_mine += (sr == 0.0 && si == 0.0) ? 0 : 1;
     }
     int n_pre;                                        // nonzero outputs = terms after the gate
     scan1024(nz_mine, red, &n_pre, A);
-    const int ns = (int)n_slots;                      // stored outputs (zeros among them)
     // (capacity bounds the terms that exist at any instant, a gate's output before its cut included: the streaming path
     // reports SV_ERR_CAPACITY for this gate)
     if ((u64)n_pre > cap) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
@@ -319,7 +330,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     }
 }
 
-size_t svk_small_smem() { return (size_t)SV_SMALL_CAP * (16 + 16 + 8 + 8 + 2); }
+size_t svk_small_smem() { return (size_t)SV_SMALL_CAP * (16 + 16 + 8 + 8 + 2 + 2); }
 
 int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
                    double* kept_out, int gate_index, u64 cap, cudaStream_t st) {
