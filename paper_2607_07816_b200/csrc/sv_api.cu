@@ -70,6 +70,7 @@ struct sv_state {
     bool small_on;          // SV_OPT_SMALL_STATE_PATH: sv_apply_circuit may use the single-block path (sv_small.cu)
     u64 small_gates;        // gates it has taken so far
     int circuit_done;       // gates the running / last sv_apply_circuit completed
+    int small_backoff, small_backoff_len;   // gates still to take the streaming passes after a gate that did not fit the small path
     long long pre_slack;    // sv_test_set_pre_slack: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
@@ -524,7 +525,11 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         for (int i = ma - 1; i >= 0; --i)
             if (s->phys_of_log[qubits[active[i]]] >= k) need[nneed++] = active[i];
     }
-    for (int t = 0; t + 1 < nneed; ++t) {   // pure moves: state preserving, committed one by one
+    static const bool allmoves_on = getenv("SV_ALLMOVES") != nullptr;   // EXPERIMENT
+    bool dense_early = allmoves_on && ma >= 2 && mc == 0;
+    for (int i = 0; i < d * d && dense_early; ++i) dense_early = !is_zero(U[i]);
+    const int npure = dense_early ? nneed : nneed - 1;
+    for (int t = 0; t < npure; ++t) {   // pure moves: state preserving, committed one by one
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;
         const int alt = s->cur ^ 1;
@@ -541,7 +546,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.passes += 1;
     }
     int plast = -1;
-    if (nneed > 0) {
+    if (nneed > 0 && !dense_early) {
         plast = s->phys_of_log[qubits[need[nneed - 1]]];
         if (plast == 0) plast = -1;
     }
@@ -727,7 +732,7 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
     int rc = SV_OK, g = 0;
     qoff = 0; uoff = 0;
     while (g < n_gates && rc == SV_OK) {
-        if (s->small_on && s->count > 0 && s->count <= SV_SMALL_CAP) {
+        if (s->small_on && s->count > 0 && s->count <= SV_SMALL_CAP && s->small_backoff == 0) {
             // ---- small-state batch: one single-block launch per gate, the count stays on the device ----
             rc = materialize(s);
             if (rc != SV_OK) break;
@@ -753,8 +758,18 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
             const KeyMap km = keymap_of(s);
             if (cudaMemcpyAsync(d_gates, h_gates, sizeof(SmallGate) * B, cudaMemcpyHostToDevice, st) != cudaSuccess ||
                 cudaMemcpyAsync(d_ctl, &hc, sizeof(hc), cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = cuda_fail(s, cudaGetLastError(), "sv_apply_circuit: upload"); break; }
-            for (int b = 0; b < B; ++b)
-                s->stats.launches += svk_small_gate(s->keys[s->cur], s->amps[s->cur], d_ctl, d_gates + b, km, max_terms, min_mass, d_kept, b, s->cap, st);
+            // block size: enough threads for the largest gate output this batch can see (count now or after a cap cut,
+            // times 2^m, two entries per thread in the sorts), no more: its ~100 barriers per gate get cheaper with fewer warps
+            u64 nmax = s->count;
+            if (max_terms != 0 && max_terms > nmax) nmax = max_terms;
+            if (max_terms == 0) nmax = SV_SMALL_CAP;
+            int mmax = 1;
+            for (int b = 0; b < B; ++b) if (gate_m[g + b] > mmax) mmax = gate_m[g + b];
+            u64 work = (nmax << mmax) / 2;
+            if (work < nmax) work = nmax;
+            if (work > 1024) work = 1024;
+            s->stats.launches += svk_small_gates(s->keys[s->cur], s->amps[s->cur], d_ctl, d_gates, B, km, max_terms, min_mass, d_kept, s->cap,
+                                                 (int)work, st);
             if (cudaGetLastError() != cudaSuccess) { rc = fail(s, SV_ERR_CUDA, "sv_apply_circuit: kernel launch"); break; }
             struct { SmallCtl c; double kept[SV_SMALL_BATCH]; } back;
             // (ctl and the kept fractions are 1 KB apart in one scratch array: two small copies, one synchronisation)
@@ -772,6 +787,11 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
             if (kept_fractions) for (int b = 0; b < done; ++b) kept_fractions[g + b] = back.kept[b];
             for (int b = 0; b < done; ++b) { qoff += gate_m[g + b]; uoff += (size_t)1 << (2 * gate_m[g + b]); }
             g += done;
+            // a gate that does not fit costs a wasted launch and round trip: after one, the next gates (twice as many after
+            // every failure in a row, up to 64) go straight to the streaming passes
+            if (back.c.status) s->small_backoff_len = s->small_backoff_len ? (s->small_backoff_len < 64 ? 2 * s->small_backoff_len : 64) : 4;
+            else s->small_backoff_len = 0;
+            s->small_backoff = back.c.status ? s->small_backoff_len : 0;
             if (g >= n_gates || !back.c.status) continue;
             // gate g (or its output) does not fit one block: the streaming passes take it (and the loop comes back here
             // if the cut brings the state down again)
@@ -782,6 +802,7 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
         if (kept_fractions) kept_fractions[g] = kf;
         qoff += gate_m[g]; uoff += (size_t)1 << (2 * gate_m[g]);
         g += 1;
+        if (s->small_backoff > 0) s->small_backoff -= 1;
     }
     delete[] h_gates;
     s->circuit_done = g;

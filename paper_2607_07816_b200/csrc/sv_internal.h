@@ -110,8 +110,8 @@ int sv_sm_count();   // SMs of the current device (cached per device)
 // In place: monomial one-bit gate whose active bit is the physical LSB (partners are neighbours); applies a pending cut.
 int svk_perm_lsb(u64* keys, double2* amps, u64 n, const GateTab* tab, const PendPred& pend, cudaStream_t st);
 size_t svk_small_smem();
-int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
-                   double* kept_out, int gate_index, u64 cap, cudaStream_t st);
+int svk_small_gates(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gates, int n_gates, KeyMap km, u64 max_terms, double min_mass,
+                    double* kept_out, u64 cap, int threads, cudaStream_t st);
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----

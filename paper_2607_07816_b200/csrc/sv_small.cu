@@ -116,8 +116,8 @@ __device__ __forceinline__ dd scan1024_excl_dd(dd v, double* red, dd* total, int
 }
 
 __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ keys, double2* __restrict__ amps, SmallCtl* __restrict__ ctl,
-                                                             const SmallGate* __restrict__ gate, KeyMap km, u64 max_terms, double min_mass,
-                                                             double* __restrict__ kept_out, int gate_index, u64 cap) {
+                                                             const SmallGate* __restrict__ gates, int n_gates, KeyMap km, u64 max_terms,
+                                                             double min_mass, double* __restrict__ kept_out, u64 cap) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* ia = reinterpret_cast<double2*>(smem_raw);
     double2* oa = ia + SV_SMALL_CAP;
@@ -131,31 +131,22 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     __shared__ double redd[66];
     __shared__ int s_flag;
     const int tid = threadIdx.x;
-    // (all the independent global reads of the prologue are issued together: each is a ~1 us round trip on its own)
-    const int status0 = ctl->status;
+    const int A = blockDim.x;                         // the host sizes the block to the work it expects (a barrier among few warps is cheap)
     const u64 n64 = ctl->count;
-    const int m = gate->m, xm = gate->xm;
-    const int pos_t = tid < SV_MAX_M ? gate->pos[tid] : 0;
-    const double2 u_t = tid < 256 ? gate->U[tid] : make_double2(0.0, 0.0);
-    if (status0 != 0) return;                         // an earlier gate of the batch did not fit: nothing more is done
-    if (n64 > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
-    const int n = (int)n64;
-    const int NP = 1 << m;
-    if (tid < 256) sU[tid] = u_t;
-    if (tid < SV_MAX_M) s_pos[tid] = pos_t;
-    // Only as many warps as the problem can use stay: a barrier among 2 warps costs a fraction of one among 32, and the
-    // sorts below are ~100 barriers.  A = active threads (a multiple of 32); the others leave before the first barrier.
-    int A;
-    {
-        long long ub = (long long)n << m;             // upper bound of the output slots
-        if (ub > SV_SMALL_CAP) ub = SV_SMALL_CAP;
-        long long need = ub / 2 > n ? ub / 2 : n;
-        A = (int)((need + 31) / 32) * 32;
-        if (A < 256) A = 256;                        // (the first 256 threads also fill the gate table)
-        if (A > SM_T) A = SM_T;
-    }
-    if (tid >= A) return;
+    if (n64 > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = 0; ctl->done_gates = 0; } return; }
+    int n = (int)n64;
+    // The state is loaded ONCE and stays in shared memory for the whole batch of gates: no launch, no global round trip
+    // and no reload between two gates.
     for (int e = tid; e < n; e += A) { ik[e] = keys[e]; ia[e] = amps[e]; }
+    int done = 0, failed = 0;
+    u64 last_pre = 0;
+    for (int gi = 0; gi < n_gates; ++gi) {
+    const SmallGate* gate = gates + gi;
+    const int m = gate->m, xm = gate->xm;
+    const int NP = 1 << m;
+    __syncthreads();                                  // the previous gate is complete (state in ik / ia, tables free)
+    for (int i = tid; i < 256; i += A) sU[i] = gate->U[i];
+    if (tid < SV_MAX_M) s_pos[tid] = gate->pos[tid];
     __syncthreads();
     u64 mask = 0;
     for (int j = 0; j < m; ++j) mask |= 1ull << s_pos[j];
@@ -186,7 +177,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     int n_owners;
     int orank = scan1024(cown, red, &n_owners, A);
     const long long n_slots = (long long)n_owners << m;
-    if (n_slots > SV_SMALL_CAP) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
+    if (n_slots > SV_SMALL_CAP) { failed = 1; break; }
     for (int i = 0; i < per; ++i) { const int e = tid * per + i; if (e < n && !oidx[e]) oelem[orank++] = (unsigned short)e; }
     const bool in_place = (n_slots == n);             // every tuple complete: the outputs take the members' own positions
     const int ns = (int)n_slots;                      // output slots (exact zeros among them)
@@ -222,7 +213,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
     scan1024(nz_mine, red, &n_pre, A);
     // (capacity bounds the terms that exist at any instant, a gate's output before its cut included: the streaming path
     // reports SV_ERR_CAPACITY for this gate)
-    if ((u64)n_pre > cap) { if (tid == 0) { ctl->status = 1; ctl->fail_gate = gate_index; } return; }
+    if ((u64)n_pre > cap) { failed = 1; break; }
     __syncthreads();
 
     // ---- 3. truncation ----
@@ -306,7 +297,7 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
         if (in_place) {       // the slots are in key order already
             for (int q = 0; q < sper; ++q) {
                 const int e = tid * sper + q;
-                if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { keys[w] = ok[e]; amps[w] = oa[e]; ++w; }
+                if (e < ns && !(oa[e].x == 0.0 && oa[e].y == 0.0)) { ik[w] = ok[e]; ia[w] = oa[e]; ++w; }
             }
         } else {              // sort the survivors only
             u64* s1 = ik;
@@ -319,24 +310,37 @@ __global__ void __launch_bounds__(SM_T, 1) small_gate_kernel(u64* __restrict__ k
             for (int e = n_final + tid; e < P; e += A) { s1[e] = ~0ull; oidx[e] = 0xffff; }
             __syncthreads();
             bitonic<false>(s1, nullptr, oidx, P, A);
-            for (int e = tid; e < n_final; e += A) { keys[e] = s1[e]; amps[e] = oa[oidx[e]]; }
+            for (int e = tid; e < n_final; e += A) ia[e] = oa[oidx[e]];          // (the sorted keys already sit in ik)
         }
     }
+    if (tid == 0 && kept_out) kept_out[gi] = kept_fraction;
+    n = n_final;
+    last_pre = (u64)n_pre;
+    done = gi + 1;
+    }   // gates
+    __syncthreads();
+    // write the state back (on a gate that did not fit: the state before that gate, untouched in ik / ia)
+    for (int e = tid; e < n; e += A) { keys[e] = ik[e]; amps[e] = ia[e]; }
     if (tid == 0) {
-        ctl->count = (u64)n_final;
-        ctl->n_pre = (u64)n_pre;
-        ctl->done_gates = gate_index + 1;
-        if (kept_out) kept_out[gate_index] = kept_fraction;
+        ctl->count = (u64)n;
+        ctl->n_pre = last_pre;
+        ctl->done_gates = done;
+        ctl->status = failed;
+        ctl->fail_gate = failed ? done : -1;
     }
 }
 
 size_t svk_small_smem() { return (size_t)SV_SMALL_CAP * (16 + 16 + 8 + 8 + 2 + 2); }
 
-int svk_small_gate(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gate, KeyMap km, u64 max_terms, double min_mass,
-                   double* kept_out, int gate_index, u64 cap, cudaStream_t st) {
+// `threads`: block size (a multiple of 32 in 256..1024), from the host's bound on the work of a gate
+int svk_small_gates(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gates, int n_gates, KeyMap km, u64 max_terms, double min_mass,
+                    double* kept_out, u64 cap, int threads, cudaStream_t st) {
     static bool attr[SV_MAX_DEV];
     const size_t smem = svk_small_smem();
     sv_set_smem_once(small_gate_kernel, smem, attr);
-    small_gate_kernel<<<1, SM_T, smem, st>>>(keys, amps, ctl, gate, km, max_terms, min_mass, kept_out, gate_index, cap);
+    if (threads < 256) threads = 256;
+    if (threads > SM_T) threads = SM_T;
+    threads = (threads + 31) & ~31;
+    small_gate_kernel<<<1, threads, smem, st>>>(keys, amps, ctl, gates, n_gates, km, max_terms, min_mass, kept_out, cap);
     return 1;
 }
