@@ -70,7 +70,8 @@ struct sv_state {
     bool small_on;          // SV_OPT_SMALL_STATE_PATH: sv_apply_circuit may use the single-block path (sv_small.cu)
     u64 small_gates;        // gates it has taken so far
     int circuit_done;       // gates the running / last sv_apply_circuit completed
-    int small_backoff, small_backoff_len;   // gates still to take the streaming passes after a gate that did not fit the small path
+    int small_backoff;      // gates still to take the streaming passes after a gate that did not fit the small path ...
+    u64 small_fail_work;    // ... unless their bound count * 2^m is below this one (that of the gate that failed)
     long long pre_slack;    // sv_test_set_pre_slack: sample points added to the floor's margin (tests force a failed margin with < 0)
 };
 #define SV_SAMPLE_MAX (1u << 16)
@@ -525,11 +526,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         for (int i = ma - 1; i >= 0; --i)
             if (s->phys_of_log[qubits[active[i]]] >= k) need[nneed++] = active[i];
     }
-    static const bool allmoves_on = getenv("SV_ALLMOVES") != nullptr;   // EXPERIMENT
-    bool dense_early = allmoves_on && ma >= 2 && mc == 0;
-    for (int i = 0; i < d * d && dense_early; ++i) dense_early = !is_zero(U[i]);
-    const int npure = dense_early ? nneed : nneed - 1;
-    for (int t = 0; t < npure; ++t) {   // pure moves: state preserving, committed one by one
+    for (int t = 0; t + 1 < nneed; ++t) {   // pure moves: state preserving, committed one by one
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;
         const int alt = s->cur ^ 1;
@@ -546,7 +543,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         s->stats.passes += 1;
     }
     int plast = -1;
-    if (nneed > 0 && !dense_early) {
+    if (nneed > 0) {
         plast = s->phys_of_log[qubits[need[nneed - 1]]];
         if (plast == 0) plast = -1;
     }
@@ -645,7 +642,8 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
             s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
                                                s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1,
                                                use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts, dense ? 1 : 0,
-                                               (s->defer.active || s->phys != s->count) ? 1 : 0);
+                                               few_dead(s) ? 0 : 1);   // few dead entries: they ride along as zero members (their
+                                                                       // products add +-0: the nonzero outputs keep their bits)
         }
         if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         CHECK_LAUNCH();
@@ -732,7 +730,10 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
     int rc = SV_OK, g = 0;
     qoff = 0; uoff = 0;
     while (g < n_gates && rc == SV_OK) {
-        if (s->small_on && s->count > 0 && s->count <= SV_SMALL_CAP && s->small_backoff == 0) {
+        // (after a gate that did not fit, a gate is tried on the small path again only if its bound count * 2^m is below that
+        // of the gate that failed, or 16 gates later: a wasted launch + round trip costs about a third of a streaming gate)
+        if (s->small_on && s->count > 0 && s->count <= SV_SMALL_CAP &&
+            (s->small_backoff == 0 || (s->count << gate_m[g]) < s->small_fail_work)) {
             // ---- small-state batch: one single-block launch per gate, the count stays on the device ----
             rc = materialize(s);
             if (rc != SV_OK) break;
@@ -787,11 +788,8 @@ static int apply_circuit_impl(sv_state* s, int n_gates, const int* gate_m, const
             if (kept_fractions) for (int b = 0; b < done; ++b) kept_fractions[g + b] = back.kept[b];
             for (int b = 0; b < done; ++b) { qoff += gate_m[g + b]; uoff += (size_t)1 << (2 * gate_m[g + b]); }
             g += done;
-            // a gate that does not fit costs a wasted launch and round trip: after one, the next gates (twice as many after
-            // every failure in a row, up to 64) go straight to the streaming passes
-            if (back.c.status) s->small_backoff_len = s->small_backoff_len ? (s->small_backoff_len < 64 ? 2 * s->small_backoff_len : 64) : 4;
-            else s->small_backoff_len = 0;
-            s->small_backoff = back.c.status ? s->small_backoff_len : 0;
+            if (back.c.status) { s->small_backoff = 16; s->small_fail_work = s->count << gate_m[g]; }
+            else s->small_backoff = 0;
             if (g >= n_gates || !back.c.status) continue;
             // gate g (or its output) does not fit one block: the streaming passes take it (and the loop comes back here
             // if the cut brings the state down again)
