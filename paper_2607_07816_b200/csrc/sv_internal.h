@@ -135,7 +135,8 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr,
-                const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr);
+                const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr,
+                u32 tnom = 0);   // tnom: nominal inputs per tile (0: the default, BP_TILE - 2)
 // fused apply + truncate: pre-sample of a one-bit gate's outputs -> (sort) -> floor; per-block partials -> totals (d_count[2] = count)
 int svk_pre_sample1(const u64* keys, const double2* amps, u64 n, int p, const GateTab* tab, const PendPred& pend, u32 M, u64* smp,
                     cudaStream_t st);

@@ -468,14 +468,16 @@ static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2
 int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int pair, int fixed,
                 const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u32* tile_counter,
                 u64* d_count, u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1, const PreCut* pre, double* pre_mass,
-                u64* pre_cnt, u32* pre_parts) {
+                u64* pre_cnt, u32* pre_parts, u32 tnom) {
     (void)tile_counter;
+    if (tnom == 0 || tnom > BP_TNOM) tnom = BP_TNOM;
+    if (tnom < 256) tnom = 256;
     if (pre_parts) *pre_parts = 0;
     if (n == 0) { cudaMemsetAsync(d_count, 0, sizeof(u64), st); return 0; }
-    const u32 ntiles = (u32)((n + BP_TNOM - 1) / BP_TNOM);
+    const u32 ntiles = (u32)((n + tnom - 1) / tnom);
     if (!(pair == 2 || (!pair && fixed)))   // the position-preserving variants have no scan
         cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);   // tile + group statuses
-    int launches = svk_find_splits(kin, n, p, 0, BP_TNOM, ntiles, desc, st);
+    int launches = svk_find_splits(kin, n, p, 0, tnom, ntiles, desc, st);
     if (e0) cudaEventRecord(e0, st);
 #define SV_BP(P_, F_) launch_bitpass<P_, F_, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st)
     if (pair == 2) SV_BP(2, true);                       // monomial blocks: always position preserving
