@@ -48,6 +48,9 @@
 #endif
 #define BP_WKN BP_TILE                         // entries of the key / slot work arrays
 #define BP_ROUND BP_TILE                       // outputs staged per round when amplitudes are staged too
+#ifndef BP_PARK_EXTRA
+#define BP_PARK_EXTRA 256                      // general one-bit pass of the FUSED call: a staging round holds this many outputs more than a tile has
+#endif                                         // inputs, so that the fused call's tiles (~1.02 outputs per input) fit one round and park
 // PRE (MODE 1 only; fused apply + truncate, sv_presample.cu): outputs whose probability pattern is below
 // pre->P_floor are not written; every block leaves the mass and the number of what it left out in
 // pre_mass / pre_cnt[blockIdx.x] (tiles are taken in a fixed order, so these sums are the same every run).
@@ -60,19 +63,21 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                                                                 double* __restrict__ pre_mass, u64* __restrict__ pre_cnt) {
     constexpr bool PAIR = (MODE == 1);
     constexpr bool PERM = (MODE == 2);
+    constexpr int STG = BP_TILE + ((!FIXED && MODE == 1 && PRE) ? BP_PARK_EXTRA : 0);   // entries of the amplitude buffers and key work arrays
+    constexpr int ROUND = STG;                                                   // outputs staged per round
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* La0 = reinterpret_cast<double2*>(smem_raw);       // landing amplitudes, double buffered
-    double2* La1 = La0 + BP_TILE;
-    u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);           // landing keys (consumed by prepare)
+    double2* La1 = La0 + STG;
+    u64* Lk = reinterpret_cast<u64*>(La1 + STG);           // landing keys (consumed by prepare)
     u64* Wk0 = Lk + BP_TILE + 8;                               // A* | B* keys with bit p cleared; later the staged output keys
-    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk0 + BP_WKN);   // their landing slots; later the staged source slots
+    unsigned short* Wi = reinterpret_cast<unsigned short*>(Wk0 + STG);   // their landing slots; later the staged source slots
     // PARK (general one-bit gate): a second key array, used in turns with the first, so that a tile whose outputs fit
     // one round leaves them parked in shared memory (keys there, amplitudes in the tile's landing buffer), publishes
     // its total at once and goes on with the block's next tile; its look-back is resolved after that tile's prepare
     // step: the chain of L2 round trips (tile totals -> group total -> reader) has run
     // behind that work instead of holding the whole block at a barrier.
     constexpr bool PARK = !FIXED && MODE == 1;   // (the compacting move keeps 4 resident blocks: no room for the array)
-    u64* Wk1 = PARK ? reinterpret_cast<u64*>(Wi + BP_WKN) : Wk0;
+    u64* Wk1 = PARK ? reinterpret_cast<u64*>(Wi + STG) : Wk0;
     bool pk_valid = false;      // uniform over the block
     u32 pk_tile = 0; int pk_total = 0;
     u64* pk_keys = Wk0; double2* pk_amps = La0;
@@ -203,7 +208,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             __syncthreads();
             const u64 base = s_base;
 #pragma unroll
-            for (int it = 0; it < BP_ROUND / SV_THREADS; ++it) {
+            for (int it = 0; it < ROUND / SV_THREADS; ++it) {
                 const int idx = tid + it * SV_THREADS;
                 const u64 g = base + (u64)idx;
                 if (idx < pk_total && g < cap) { st_stream_u64(kout + g, pk_keys[BP_SWK(idx)]); st_stream_d2(aout + g, pk_amps[BP_SWA(idx)]); }
@@ -377,9 +382,9 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
         // stage the outputs in output order (keys over A* | B*, amplitudes over this tile's landing buffer:
         // BP_ROUND outputs per round, a gate that doubles the tile is written in two rounds), store coalesced
         SV_CHK(total >= 0 && total <= 2 * BP_TILE && excl >= 0 && excl + nout <= total);
-        const bool park = PARK && total <= BP_ROUND;   // one round: its outputs wait in shared memory for the block's next tile
+        const bool park = PARK && total <= ROUND;   // one round: its outputs wait in shared memory for the block's next tile
         if (tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)total);   // at once: the later tiles read it while this one stages
-        for (int h0 = 0; h0 == 0 || h0 < total; h0 += BP_ROUND) {
+        for (int h0 = 0; h0 == 0 || h0 < total; h0 += ROUND) {
             if (h0 > 0) __syncthreads();
             {
                 int off = excl - h0;
@@ -387,11 +392,11 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                 for (int v = 0; v < BP_VT; ++v) {
                     const u32 f = (fl >> (2 * v)) & 3u;
                     if (f & 1u) {
-                        if ((unsigned)off < (unsigned)BP_ROUND) { Wk[BP_SWK(off)] = ok[v]; La[BP_SWA(off)] = make_double2(o0r[v], o0i[v]); }
+                        if ((unsigned)off < (unsigned)ROUND) { Wk[BP_SWK(off)] = ok[v]; La[BP_SWA(off)] = make_double2(o0r[v], o0i[v]); }
                         ++off;
                     }
                     if (PAIR && (f & 2u)) {
-                        if ((unsigned)off < (unsigned)BP_ROUND) { Wk[BP_SWK(off)] = ok[v] | 1ull; La[BP_SWA(off)] = make_double2(o1r[v], o1i[v]); }
+                        if ((unsigned)off < (unsigned)ROUND) { Wk[BP_SWK(off)] = ok[v] | 1ull; La[BP_SWA(off)] = make_double2(o1r[v], o1i[v]); }
                         ++off;
                     }
                 }
@@ -409,9 +414,9 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
             }
             __syncthreads();
             const u64 base = s_base + (u64)h0;
-            const int m = min(total - h0, BP_ROUND);
+            const int m = min(total - h0, ROUND);
 #pragma unroll
-            for (int it = 0; it < BP_ROUND / SV_THREADS; ++it) {
+            for (int it = 0; it < ROUND / SV_THREADS; ++it) {
                 const int idx = tid + it * SV_THREADS;
                 const u64 g = base + (u64)idx;
                 if (idx < m && g < cap) { st_stream_u64(kout + g, Wk[BP_SWK(idx)]); st_stream_d2(aout + g, La[BP_SWA(idx)]); }
@@ -457,8 +462,9 @@ template <int MODE, bool FIXED, bool PRE>
 static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                           const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
-    const size_t smem = (size_t)BP_TILE * (16 + 16 + 8) + 64 + (size_t)BP_WKN * (8 + 2) +
-                        ((!FIXED && MODE == 1) ? (size_t)BP_WKN * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
+    const size_t stg = (size_t)BP_TILE + ((!FIXED && MODE == 1 && PRE) ? BP_PARK_EXTRA : 0);
+    const size_t smem = stg * (16 + 16) + (size_t)BP_TILE * 8 + 64 + stg * (8 + 2) +
+                        ((!FIXED && MODE == 1) ? stg * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
     static int per_sm[SV_MAX_DEV];
     const u32 grid = sv_launch_persistent(bitpass_kernel<MODE, FIXED, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                           (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt);
