@@ -642,8 +642,10 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
             s->stats.launches += svk_grouppass(s->keys[s->cur], s->amps[s->cur], s->keys[alt], s->amps[alt], s->phys, plast, ma,
                                                s->tab, s->defer, s->desc, s->status, s->d_count, s->cap, s->stream, ge0, ge1,
                                                use_pre ? s->pre : nullptr, pmass, pcnt, &pre_parts, dense ? 1 : 0,
-                                               few_dead(s) ? 0 : 1);   // few dead entries: they ride along as zero members (their
-                                                                       // products add +-0: the nonzero outputs keep their bits)
+                                               // few dead entries: they ride along as zero members (their products add +-0: the
+                                                // nonzero outputs keep their bits) -- unless the dead-only tuples' zero outputs
+                                                // could then push a full-size output over the capacity
+                                               (few_dead(s) && (s->phys << ma) <= s->cap) ? 0 : 1);
         }
         if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         CHECK_LAUNCH();

@@ -25,12 +25,16 @@
 #include "sv_launch.cuh"
 #include <type_traits>
 
+#ifndef DP_NOPRE_BLOCKS
+#define DP_NOPRE_BLOCKS 3                  // resident blocks per SM of the two-call variant (ma <= 3)
+#endif
+#define DP_WENT 128                        // !PRE: entries of a warp's transposition buffer
 #ifndef DP_STAGE
 #define DP_STAGE 2048                      // PRE: staged survivors per tile (about twice the mean at the cap)
 #endif
 
 template <int MA, bool PRE>
-__global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+__global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLOCKS) densepass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                             u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                             const GateTab* __restrict__ gtab, PendPred pd,
                                                                             const TileDesc* __restrict__ desc, u64* status,
@@ -47,7 +51,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
     u64* sk = Lk + BP_TILE + 8;
     unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
     double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE: staged survivors, output order; else the warps' transposition buffers
-    u64* stg_k = reinterpret_cast<u64*>(stg_a + DP_STAGE);
+    u64* stg_k = reinterpret_cast<u64*>(stg_a + (PRE ? DP_STAGE : BP_WARPS * DP_WENT));
     __shared__ int wcA[BP_VT][BP_WARPS], wcB[BP_VT][BP_WARPS];
     __shared__ int s_nA, s_nB, s_nt;
     __shared__ int wtot[2][BP_WARPS];
@@ -299,10 +303,10 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
             // ---- two calls: every candidate is an output.  The rows a thread holds are consecutive outputs; each warp
             // transposes its round through its own 4 KB of shared memory (XOR-swizzled 16-byte entries: conflict free
             // both ways) so that consecutive lanes store consecutive entries ----
-            double2* W = stg_a + warp * 256;
+            double2* W = stg_a + warp * DP_WENT;
             u64* KB = stg_k + warp * (32 * TPR);
-            constexpr int TP = 256 / NP;                 // tuples per transposition phase
-            constexpr int PH = (32 * TPR) / TP;          // phases per round (2 for 16 rows, else 1)
+            constexpr int TP = DP_WENT / NP;             // tuples per transposition phase
+            constexpr int PH = (32 * TPR) / TP;          // phases per round
             constexpr int SWS = MA > 3 ? MA : 3;
             for (int h = 0; h < NT; h += SV_THREADS * TPR) {
                 const int hw = h + warp * (32 * TPR);
@@ -341,7 +345,7 @@ __global__ void __launch_bounds__(SV_THREADS, 2) densepass_kernel(const u64* __r
                     }
                     __syncwarp();
 #pragma unroll
-                    for (int s = 0; s < 8; ++s) {
+                    for (int s = 0; s < DP_WENT / 32; ++s) {
                         const int o = s * 32 + lane;
                         const int sl = ph * TP + (o >> MA), row = o & (NP - 1);
                         const int ti = hw + sl;
@@ -456,7 +460,8 @@ template <int MA, bool PRE>
 static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + 64 + (size_t)(BP_TILE + 8) * 2 + (size_t)DP_STAGE * 24;
+    const size_t smem = (size_t)2 * BP_TILE * 24 + 64 + (size_t)(BP_TILE + 8) * 2 +
+                        (PRE ? (size_t)DP_STAGE * 24 : (size_t)BP_WARPS * DP_WENT * 16 + (size_t)BP_WARPS * 64 * 8);
     static int per_sm[SV_MAX_DEV];
     return sv_launch_persistent(densepass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                 (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead);
