@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     u64* stg_k = reinterpret_cast<u64*>(stg_a + (PRE ? DP_STAGE : BP_WARPS * DP_WENT));
     __shared__ int wcA[BP_VT][BP_WARPS], wcB[BP_VT][BP_WARPS];
     __shared__ int s_nA, s_nB, s_nt;
+    __shared__ u64 s_last[BP_WARPS];        // last merged key of every warp (tuple starts across warps)
     __shared__ int wtot[2][BP_WARPS];
     __shared__ u64 s_desc[2][8];
     __shared__ u64 s_base;
@@ -213,15 +214,43 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
                 }
             }
+            // The tuples are found here, from the merged keys in registers: a thread's outputs are consecutive, its
+            // predecessor's last key comes by shuffle (across warps through shared memory, behind the barrier the
+            // merge needs anyway).  The tile's tuple count -- hence, two calls, its output count -- is known two
+            // barriers earlier than with a pass of its own over the merged tile, and is published at once.
+            u64 mylast = 0ull;
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v) if (diag + v < endpos) mylast = mk[v];
+            if (lane == 31) s_last[warp] = mylast;          // (a thread without elements sits behind the tile's end: never read)
             __syncthreads();   // every read of the partitioned tile is done
+            u64 prev = __shfl_up_sync(0xffffffffu, mylast, 1);
+            if (lane == 0 && warp > 0) prev = s_last[warp - 1];
+            u32 om = 0;        // bit v: merged element diag + v opens a tuple
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v) {
+                if (diag + v < endpos) {
+                    const u64 before = v == 0 ? prev : mk[v - 1];
+                    if ((diag + v == 0) || (before >> MA) != (mk[v] >> MA)) om |= 1u << v;
+                    sk[diag + v] = mk[v]; sa[diag + v] = ma_[v];
+                }
+            }
+            int cinc = __popc(om);
+            const int cmine = cinc;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, cinc, d); if (lane >= d) cinc += t; }
+            if (lane == 31) wcA[0][warp] = cinc;
+            __syncthreads();   // merged tile and the warps' tuple counts visible
+            int tbefore = 0, tall = 0;
+#pragma unroll
+            for (int w = 0; w < BP_WARPS; ++w) { const int c = wcA[0][w]; tall += c; if (w < warp) tbefore += c; }
+            if (!PRE && tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)tall << MA);   // known before any arithmetic
+            int tix = tbefore + cinc - cmine;
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v)
-                if (diag + v < endpos) { sk[diag + v] = mk[v]; sa[diag + v] = ma_[v]; }
-            __syncthreads();
-        }
-
-        // ---- phase 2: tuples (elements taken strided: conflict-free reads; counts scanned in element order) ----
-        {
+                if ((om >> v) & 1u) tst[tix++] = (unsigned short)(diag + v);
+            if (tid == 0) { tst[tall] = (unsigned short)nL; s_nt = tall; }
+        } else {
+        // ---- phase 2 (no move): tuples (elements taken strided: conflict-free reads; counts scanned in element order) ----
             u32 bs[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
@@ -245,12 +274,12 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             for (int r = 0; r < BP_VT; ++r)
                 if ((bs[r] >> lane) & 1u) tst[wcA[r][warp] + __popc(bs[r] & lt)] = (unsigned short)(tid + r * SV_THREADS);
             if (tid == 0) tst[s_nt] = (unsigned short)nL;
+            if (!PRE && tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)s_nt << MA);   // known before any arithmetic
         }
+        __syncthreads();              // tuple table complete
         const int NT = s_nt;
         SV_CHK(NT >= 0 && NT <= nL && nL <= BP_TILE);
         const int NC = NT << MA;      // candidates of the tile
-        if (!PRE && tid == 0) lookback_publish(status, gstat, tile, ntiles, (u64)NC);   // known before any arithmetic
-        __syncthreads();              // tuple table complete
         if (PRE && pk_valid) flush_parked();   // (the look-back of the previous tile has had the whole front end to resolve)
 
         // ---- back end: ONE THREAD PER TUPLE, all 2^MA rows in registers ----
