@@ -43,6 +43,13 @@
 // writes over the banks and keeps the copy-out reads of consecutive entries inside one row.
 #define BP_SWK(x) ((x) ^ (((x) >> 4) & 15))
 #define BP_SWA(x) ((x) ^ (((x) >> 3) & 7))
+#ifndef BP_GEN2_CTAS
+#define BP_GEN2_CTAS 4                         // resident blocks per SM of the general one-bit pass, two calls.  4 (64 registers, no second
+#endif                                         // key array, hence no parking): its tiles hold > 1024 outputs and could not park anyway; the
+                                               // fourth block hides their look-back wait better: H apply 5.07 -> 4.83 ms
+#ifndef BP_GENP_CTAS
+#define BP_GENP_CTAS 3                         // the same, fused call (3: tiles park, see BP_PARK_EXTRA)
+#endif
 #ifndef BP_GEN_CTAS
 #define BP_GEN_CTAS 3                          // resident blocks per SM of the general one-bit pass (0: BP_CTAS)
 #endif
@@ -55,7 +62,7 @@
 // pre->P_floor are not written; every block leaves the mass and the number of what it left out in
 // pre_mass / pre_cnt[blockIdx.x] (tiles are taken in a fixed order, so these sums are the same every run).
 template <int MODE, bool FIXED, bool PRE>
-__global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GEN_CTAS : BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
+__global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? (PRE ? BP_GENP_CTAS : BP_GEN2_CTAS) : BP_CTAS) bitpass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                 u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                 const GateTab* __restrict__ gtab, PendPred pd,
                                                                 const TileDesc* __restrict__ desc, u64* status,
@@ -63,7 +70,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
                                                                 double* __restrict__ pre_mass, u64* __restrict__ pre_cnt) {
     constexpr bool PAIR = (MODE == 1);
     constexpr bool PERM = (MODE == 2);
-    constexpr int STG = BP_TILE + ((!FIXED && MODE == 1 && PRE) ? BP_PARK_EXTRA : 0);   // entries of the amplitude buffers and key work arrays
+    constexpr int STG = BP_TILE + ((!FIXED && MODE == 1 && PRE && BP_GENP_CTAS < 4) ? BP_PARK_EXTRA : 0);   // entries of the amplitude buffers and key work arrays
     constexpr int ROUND = STG;                                                   // outputs staged per round
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* La0 = reinterpret_cast<double2*>(smem_raw);       // landing amplitudes, double buffered
@@ -76,7 +83,7 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? BP_GE
     // its total at once and goes on with the block's next tile; its look-back is resolved after that tile's prepare
     // step: the chain of L2 round trips (tile totals -> group total -> reader) has run
     // behind that work instead of holding the whole block at a barrier.
-    constexpr bool PARK = !FIXED && MODE == 1;   // (the compacting move keeps 4 resident blocks: no room for the array)
+    constexpr bool PARK = !FIXED && MODE == 1 && (PRE ? BP_GENP_CTAS < 4 : BP_GEN2_CTAS < 4);   // (the compacting move keeps 4 resident blocks: no room for the array)
     u64* Wk1 = PARK ? reinterpret_cast<u64*>(Wi + STG) : Wk0;
     bool pk_valid = false;      // uniform over the block
     u32 pk_tile = 0; int pk_total = 0;
@@ -462,9 +469,9 @@ template <int MODE, bool FIXED, bool PRE>
 static u32 launch_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                           const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                           const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr) {
-    const size_t stg = (size_t)BP_TILE + ((!FIXED && MODE == 1 && PRE) ? BP_PARK_EXTRA : 0);
+    const size_t stg = (size_t)BP_TILE + ((!FIXED && MODE == 1 && PRE && BP_GENP_CTAS < 4) ? BP_PARK_EXTRA : 0);
     const size_t smem = stg * (16 + 16) + (size_t)BP_TILE * 8 + 64 + stg * (8 + 2) +
-                        ((!FIXED && MODE == 1) ? stg * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
+                        ((!FIXED && MODE == 1 && (PRE ? BP_GENP_CTAS < 4 : BP_GEN2_CTAS < 4)) ? stg * 8 : 0);   // amplitudes x 2, landing keys, A* | B* keys, slots; general one-bit gate: second key array
     static int per_sm[SV_MAX_DEV];
     const u32 grid = sv_launch_persistent(bitpass_kernel<MODE, FIXED, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                           (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt);
