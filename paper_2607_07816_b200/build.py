@@ -25,7 +25,7 @@ def sources():
 
 def _headers():
     return glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + \
-        [os.path.join(os.path.dirname(HERE), "include", "sparse_sv.h")]
+        glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h"))
 
 
 def _compile(src, force, verbose, extra):
