@@ -19,6 +19,11 @@ extern "C" {
  * s: handle (host pointer).  Returns SV_OK, or SV_ERR_INVALID_ARG for a null handle.  No device work. */
 int sv_test_set_pre_slack(sv_state *s, long long slack);
 
+/* Diagnostic: bit q of *mask (host pointer) is set iff qubit q has the same value in every term of the state (a pending
+ * truncation is taken into account).  One pass over the state (24 B per term), synchronises the state's stream.
+ * Returns SV_OK, SV_ERR_INVALID_ARG (null pointer) or SV_ERR_CUDA. */
+int sv_test_definite_qubits(sv_state *s, uint64_t *mask);
+
 #ifdef __cplusplus
 }
 #endif

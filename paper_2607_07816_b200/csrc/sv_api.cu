@@ -68,6 +68,7 @@ struct sv_state {
     bool diag_deferred;     // the diagonal gate in s->tab (and the pending cut) has not been applied yet: the truncation's
                             // classification pass applies it in place (sv_sample_select.cu, XF)
     bool small_on;          // SV_OPT_SMALL_STATE_PATH: sv_apply_circuit may use the single-block path (sv_small.cu)
+    bool two_bit_on;        // SV_OPT_TWO_BIT_PASS: the final pass of a dense multi-qubit gate may move two bits at once
     u64 small_gates;        // gates it has taken so far
     int circuit_done;       // gates the running / last sv_apply_circuit completed
     int small_backoff;      // gates still to take the streaming passes after a gate that did not fit the small path ...
@@ -262,6 +263,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->seg_cnt = s->arena + L.seg_cnt;
     s->chunk_cnt = (u32*)(s->arena + L.chunk_cnt);
     s->small_on = true;
+    s->two_bit_on = false;
     s->sample_min_terms = 1ull << 21;   // below ~2^21 terms the state sits in L2 and the full select has fewer launches
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
@@ -321,12 +323,27 @@ extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
     if (option == SV_OPT_SMALL_STATE_PATH) { s->small_on = value != 0; return SV_OK; }
+    if (option == SV_OPT_TWO_BIT_PASS) { s->two_bit_on = value != 0; return SV_OK; }
     return fail(s, SV_ERR_INVALID_ARG, "unknown option");
 }
 // test hook (include/sparse_sv_test.h): sample points added to the margin of the fused call's output floor
 extern "C" int sv_test_set_pre_slack(sv_state* s, long long slack) {
     if (!s) return SV_ERR_INVALID_ARG;
     s->pre_slack = slack;
+    return SV_OK;
+}
+// test / diagnostic hook (include/sparse_sv_test.h): bit q of *mask is set iff qubit q has the same value in every term
+extern "C" int sv_test_definite_qubits(sv_state* s, uint64_t* mask) {
+    if (!s || !mask) return SV_ERR_INVALID_ARG;
+    svk_key_masks(s->keys[s->cur], s->amps[s->cur], s->phys, s->defer, 1, s->d_count + 4, s->stream);
+    u64 oa[2] = {0, 0};
+    CU(cudaMemcpyAsync(s->pinned, s->d_count + 4, sizeof(oa), cudaMemcpyDeviceToHost, s->stream));
+    CU(cudaStreamSynchronize(s->stream));
+    memcpy(oa, s->pinned, sizeof(oa));
+    const u64 same = ~(oa[0] ^ oa[1]);
+    u64 m = 0;
+    for (int q = 0; q < s->n; ++q) if ((same >> s->phys_of_log[q]) & 1ull) m |= 1ull << q;
+    *mask = (s->count == 0) ? 0 : m;
     return SV_OK;
 }
 extern "C" int sv_get_stats(sv_state* s, sv_stats* out) {
@@ -526,7 +543,12 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         for (int i = ma - 1; i >= 0; --i)
             if (s->phys_of_log[qubits[active[i]]] >= k) need[nneed++] = active[i];
     }
-    for (int t = 0; t + 1 < nneed; ++t) {   // pure moves: state preserving, committed one by one
+    // A dense gate (every entry of U nonzero: Haar SU(4), 8x8, 16x16) brings its LAST TWO missing bits down in the final pass
+    // itself (a four-way merge per tile, sv_dense.cu TWO): one full pass over the state less.
+    bool dense0 = (ma >= 2 && mc == 0);
+    for (int i = 0; i < d * d && dense0; ++i) dense0 = !is_zero(U[i]);
+    const bool two = s->two_bit_on && dense0 && nneed >= 2;
+    for (int t = 0; t + (two ? 2 : 1) < nneed; ++t) {   // pure moves: state preserving, committed one by one
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;
         const int alt = s->cur ^ 1;
@@ -542,14 +564,19 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
         layout_move(s, p);
         s->stats.passes += 1;
     }
-    int plast = -1;
+    int plast = -1, plast2 = -1;   // the bit(s) the final pass moves; two: plast > plast2
     if (nneed > 0) {
         plast = s->phys_of_log[qubits[need[nneed - 1]]];
         if (plast == 0) plast = -1;
     }
+    if (two) {
+        const int pa = s->phys_of_log[qubits[need[nneed - 2]]], pb = s->phys_of_log[qubits[need[nneed - 1]]];
+        plast = pa > pb ? pa : pb; plast2 = pa > pb ? pb : pa;
+    }
     // layout after the final move (on a copy: committed only on success)
     sv_state after = *s;
     if (plast > 0) layout_move(&after, plast);
+    if (two) layout_move(&after, plast2 + 1);   // (the lower bit has moved up by one)
     tab.ma = ma; tab.mc = mc;
     int fpos[SV_MAX_M];
     for (int i = 0; i < ma; ++i) fpos[i] = after.phys_of_log[qubits[active[i]]];   // in 0..ma-1
@@ -624,7 +651,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
                                                      s->smp_k[0], s->stream);
             else
                 s->stats.launches += svk_pre_sample_group(s->keys[s->cur], s->amps[s->cur], s->phys, plast, ma, s->tab, s->defer, M,
-                                                          s->smp_k[0], s->stream);
+                                                          s->smp_k[0], s->stream, plast2);
             int in_alt = 0;
             s->stats.launches += svk_sort_pairs(s->smp_k[0], s->smp_v[0], s->smp_k[1], s->smp_v[1], M, 24, s->smp_scr, s->stream, &in_alt);
             s->stats.launches += svk_pre_pivot(s->smp_k[in_alt ? 1 : 0], M, s->phys, 1u << ma, s->fuse_K, s->pre_slack, s->pre, s->stream);
@@ -645,7 +672,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
                                                // few dead entries: they ride along as zero members (their products add +-0: the
                                                 // nonzero outputs keep their bits) -- unless the dead-only tuples' zero outputs
                                                 // could then push a full-size output over the capacity
-                                               (few_dead(s) && (s->phys << ma) <= s->cap) ? 0 : 1);
+                                               (few_dead(s) && (s->phys << ma) <= s->cap) ? 0 : 1, plast2);
         }
         if (use_pre) s->stats.launches += svk_pre_finish(pmass, pcnt, pre_parts, s->pre, s->d_count, s->stream);
         CHECK_LAUNCH();

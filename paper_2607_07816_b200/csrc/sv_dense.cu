@@ -29,26 +29,39 @@
 #define DP_NOPRE_BLOCKS 3                  // resident blocks per SM of the two-call variant (ma <= 3)
 #endif
 #define DP_WENT 128                        // !PRE: entries of a warp's transposition buffer
+// The tile arrays (keys sk, amplitudes sa) are addressed through an XOR swizzle of the entry index with its 128-byte row
+// (16 keys / 8 amplitudes per row), as the staging arrays of sv_pair.cu: threads that own a few CONSECUTIVE entries each
+// (the merges write 4 per thread, read ~2 apart per lane) would otherwise hit the same banks 4 to 16 ways -- measured: a
+// third of the kernel's shared-memory wavefronts were such replays and the shared-memory pipe its busiest unit (72 %).
+#define DK(x) ((x) ^ (((x) >> 4) & 15))
+#define DA(x) ((x) ^ (((x) >> 3) & 7))
 #ifndef DP_STAGE
 #define DP_STAGE 2048                      // PRE: staged survivors per tile (about twice the mean at the cap)
 #endif
 
-template <int MA, bool PRE>
+// TWO: the pass moves TWO bits (p > p2) to the two least-significant positions at once.  A tile (TileDesc2, find_splits2 in
+// sv_gate.cu) is then up to seven contiguous pieces of the input; its live entries are partitioned into the four classes of
+// (bH, bL) -- each sorted by the rest of the key -- and merged in two levels: the bL = 0 / 1 classes of either bH (two
+// merges side by side, one merge-path split per thread), then the two results by bH.  The state comes out as the two
+// single-bit passes (p, then p2 + 1) would leave it, without the intermediate trip through HBM.
+#define DP_MAXPIECES 8
+template <int MA, bool PRE, bool TWO>
 __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLOCKS) densepass_kernel(const u64* __restrict__ kin, const double2* __restrict__ ain,
                                                                             u64* __restrict__ kout, double2* __restrict__ aout, int p,
                                                                             const GateTab* __restrict__ gtab, PendPred pd,
                                                                             const TileDesc* __restrict__ desc, u64* status,
                                                                             u64* d_count, u64 cap, u32 ntiles, const PreCut* __restrict__ pre,
                                                                             double* __restrict__ pre_mass, u64* __restrict__ pre_cnt,
-                                                                            int maybe_dead) {
+                                                                            int maybe_dead, int p2) {
     constexpr int NP = 1 << MA;
+    constexpr int LKX = TWO ? 16 : 8;            // over-fetched keys the landing array has room for (two per piece)
     constexpr u64 AM = (u64)NP - 1;
     constexpr int TPR = NP >= 8 ? 1 : 8 / NP;   // tuples per thread and round
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
     double2* sa = La + BP_TILE;                                // the tile: partitioned, then in its new order
     u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
-    u64* sk = Lk + BP_TILE + 8;
+    u64* sk = Lk + BP_TILE + LKX;
     unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
     double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE: staged survivors, output order; else the warps' transposition buffers
     u64* stg_k = reinterpret_cast<u64*>(stg_a + (PRE ? DP_STAGE : BP_WARPS * DP_WENT));
@@ -56,7 +69,9 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     __shared__ int s_nA, s_nB, s_nt;
     __shared__ u64 s_last[BP_WARPS];        // last merged key of every warp (tuple starts across warps)
     __shared__ int wtot[2][BP_WARPS];
-    __shared__ u64 s_desc[2][8];
+    __shared__ u64 s_desc[2][TWO ? 16 : 8];
+    __shared__ int s_pcum[2][TWO ? DP_MAXPIECES + 1 : 1], s_pko[2][TWO ? DP_MAXPIECES : 1];   // TWO: first load-order index of every piece (+ total), key slot offset
+    __shared__ int wc4[TWO ? 4 : 1][BP_VT][BP_WARPS], s_n4[4];                                 // TWO: class counts per (round, warp); class totals
     __shared__ u64 s_base;
     __shared__ __align__(8) u64 s_bar;   // mbarrier of the landing bulk copies
     __shared__ double2 Us[NP * NP];          // Us[r * NP + x] = U[r][x] (physical patterns): lanes differ in x -> different banks
@@ -81,6 +96,9 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
 
     const u64 bit = mv ? (1ull << p) : 0ull;
     const u64 himask = (!mv || p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
+    // TWO: stored key (high, bH, mid, bL, low) -> (high, mid, low, 0, 0)
+    const u64 bit2 = TWO ? (1ull << p2) : 0ull;
+    const u64 midmask = TWO ? ((bit - 1) & ~((bit2 << 1) - 1)) : 0ull, lowmask2 = TWO ? (bit2 - 1) : 0ull;
     u64* gstat = status + ntiles;
     // parked tile (PRE): its staged outputs wait for the look-back while the next tile is prepared
     bool pk_valid = false;  // uniform over the block
@@ -89,6 +107,52 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     // The tile lands by bulk copies (TMA): one thread arms the barrier and issues up to six copies (sv_tile.cuh).
     auto issue_loads = [&](const Pieces3& q) {
         if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
+    };
+    // TWO, called by ONE thread: the tile between the boundaries w[0..6] and w[8..14] as contiguous pieces of the input -- the
+    // difference of two sets of four stored ranges each (TileDesc2) --, their table for the pick-up (s_pcum / s_pko[slot])
+    // and the bulk copies.  A key piece that starts at an odd index is fetched from the even index before it (sv_tile.cuh).
+    auto issue_loads2 = [&](const u64* w, int slot) {
+        const u64 as_[4] = {0, w[1], w[3], w[5]}, ae_[4] = {w[0], w[2], w[4], w[6]};
+        const u64 bs_[4] = {0, w[9], w[11], w[13]}, be_[4] = {w[8], w[10], w[12], w[14]};
+        u64 ps[DP_MAXPIECES]; int pl[DP_MAXPIECES];
+        int np = 0;
+        auto emit = [&](u64 a, u64 b) {
+            if (b <= a) return;
+            if (np > 0 && ps[np - 1] + (u64)pl[np - 1] == a) { pl[np - 1] += (int)(b - a); return; }
+            SV_CHK(np < DP_MAXPIECES);
+            if (np < DP_MAXPIECES) { ps[np] = a; pl[np] = (int)(b - a); ++np; }
+        };
+        for (int bi = 0; bi < 4; ++bi) {
+            u64 cur = bs_[bi];
+            const u64 be = be_[bi];
+            for (int ai = 0; ai < 4 && cur < be; ++ai) {
+                const u64 a0 = as_[ai], a1 = ae_[ai];
+                if (a1 <= a0 || a1 <= cur || a0 >= be) continue;
+                if (a0 > cur) emit(cur, a0);
+                cur = a1 < be ? a1 : be;
+            }
+            emit(cur, be);
+        }
+        int cum = 0, slots = 0;
+        u32 bytes = 0;
+        for (int q = 0; q < np; ++q) {
+            const int o = (int)(ps[q] & 1ull), c = (pl[q] + o + 1) & ~1;
+            s_pcum[slot][q] = cum; s_pko[slot][q] = slots + o - cum;
+            bytes += (u32)c * 8u + (u32)pl[q] * 16u;
+            cum += pl[q]; slots += c;
+        }
+        for (int q = np; q <= DP_MAXPIECES; ++q) s_pcum[slot][q] = cum;
+        for (int q = np; q < DP_MAXPIECES; ++q) s_pko[slot][q] = 0;
+        SV_CHK(cum <= BP_TILE && slots <= BP_TILE + LKX);
+        fence_proxy_async_smem();
+        mbar_expect_tx(&s_bar, bytes);
+        cum = 0; slots = 0;
+        for (int q = 0; q < np; ++q) {
+            const int o = (int)(ps[q] & 1ull), c = (pl[q] + o + 1) & ~1;
+            bulk_g2s(Lk + slots, kin + (ps[q] & ~1ull), (u32)c * 8u, &s_bar);
+            bulk_g2s(La + cum, ain + ps[q], (u32)pl[q] * 16u, &s_bar);
+            cum += pl[q]; slots += c;
+        }
     };
     if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
     u32 bar_phase = 0;
@@ -110,27 +174,47 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
         pk_valid = false;
     };
 
-    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
-    __syncthreads();
-    issue_loads(pieces_of(s_desc[0]));
+    if constexpr (TWO) {
+        if (tid < 16) s_desc[0][tid] = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + blockIdx.x)[tid];
+        __syncthreads();
+        if (tid == 0) issue_loads2(s_desc[0], 0);
+        __syncthreads();      // the piece table of the first tile is visible
+    } else {
+        if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+        __syncthreads();
+        issue_loads(pieces_of(s_desc[0]));
+    }
     int par = 0;
     for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
         const u32 next = tile + gridDim.x;
         u64 dnext = 0;
-        if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];
-        const Pieces3 pc = pieces_of(s_desc[par]);
+        if constexpr (TWO) { if (tid < 16 && next < ntiles) dnext = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + next)[tid]; }
+        else { if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid]; }
+        Pieces3 pc;
+        if constexpr (!TWO) pc = pieces_of(s_desc[par]); else { pc.cnt = s_pcum[par][DP_MAXPIECES]; pc.oneblock = false; pc.l0 = 0; }
         const int cnt = pc.cnt;
         int nA, nL;
         {   // pick up this thread's landed elements, apply a pending truncation, partition the LIVE ones into A* | B*
             mbar_wait(&s_bar, bar_phase);      // the tile has landed
             bar_phase ^= 1u;
-            const Landing3 ld = landing_of(pc);
+            Landing3 ld;
+            if constexpr (!TWO) ld = landing_of(pc);
             u64 lk[BP_VT]; double2 la[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
                 lk[r] = 0; la[r] = make_double2(0.0, 0.0);
-                if (e < cnt) { lk[r] = Lk[landing_key_slot(pc, ld, e)]; la[r] = La[e]; }
+                if (e < cnt) {
+                    if constexpr (TWO) {
+                        int q = 0;
+#pragma unroll
+                        for (int i = 1; i < DP_MAXPIECES; ++i) q += (e >= s_pcum[par][i]) ? 1 : 0;
+                        const int sl = e + s_pko[par][q];
+                        SV_CHK(sl >= 0 && sl < BP_TILE + LKX);
+                        lk[r] = Lk[sl];
+                    } else lk[r] = Lk[landing_key_slot(pc, ld, e)];
+                    la[r] = La[e];
+                }
             }
             if (pd.active) {
 #pragma unroll
@@ -141,12 +225,51 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     }
                 }
             }
-            if (!maybe_dead && (!mv || pc.oneblock)) {   // load order = A* | B* already and nothing to squeeze out
+            if constexpr (TWO) {
+                // the live entries by class (bH, bL), each class in load order = ascending rest; keys -> (high, mid, low, 0, 0)
+                u32 bal[4][BP_VT];
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    const bool live = (tid + r * SV_THREADS < cnt) && !(la[r].x == 0.0 && la[r].y == 0.0);
+                    const u32 bl = __ballot_sync(0xffffffffu, live);
+                    const u32 bh = __ballot_sync(0xffffffffu, (lk[r] & bit) != 0), b2 = __ballot_sync(0xffffffffu, (lk[r] & bit2) != 0);
+                    bal[0][r] = bl & ~bh & ~b2; bal[1][r] = bl & ~bh & b2; bal[2][r] = bl & bh & ~b2; bal[3][r] = bl & bh & b2;
+                    const u32 mine = lane == 0 ? bal[0][r] : (lane == 1 ? bal[1][r] : (lane == 2 ? bal[2][r] : bal[3][r]));
+                    if (lane < 4) wc4[lane][r][warp] = __popc(mine);
+                }
+                __syncthreads();
+                if (warp < 4) {   // lane = r * 8 + w: exclusive scan of the 32 counts of class `warp` in load order
+                    int* wv = &wc4[warp][0][0];
+                    const int c = wv[lane];
+                    int inc = c;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, d); if (lane >= d) inc += t; }
+                    wv[lane] = inc - c;
+                    if (lane == 31) s_n4[warp] = inc;
+                }
+                __syncthreads();
+                const int n00 = s_n4[0], n01 = s_n4[1], n10 = s_n4[2];
+                nA = n00 + n01; nL = nA + n10 + s_n4[3];
+                const int cb[4] = {0, n00, nA, nA + n10};
+#pragma unroll
+                for (int r = 0; r < BP_VT; ++r) {
+                    int slot = -1;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c)
+                        if ((bal[c][r] >> lane) & 1u) slot = cb[c] + wc4[c][r][warp] + __popc(bal[c][r] & lt);
+                    SV_CHK(slot < nL);
+                    if (slot >= 0) {
+                        const u64 k = lk[r];
+                        sk[DK(slot)] = (k & himask) | ((k & midmask) << 1) | ((k & lowmask2) << 2);
+                        sa[DA(slot)] = la[r];
+                    }
+                }
+            } else if (!maybe_dead && (!mv || pc.oneblock)) {   // load order = A* | B* already and nothing to squeeze out
                 nA = mv ? pc.l0 : cnt; nL = cnt;
 #pragma unroll
                 for (int r = 0; r < BP_VT; ++r) {
                     const int e = tid + r * SV_THREADS;
-                    if (e < cnt) { sk[e] = lk[r] & ~bit; sa[e] = la[r]; }
+                    if (e < cnt) { sk[DK(e)] = lk[r] & ~bit; sa[DA(e)] = la[r]; }
                 }
             } else {
                 u32 balA[BP_VT], balB[BP_VT];
@@ -176,42 +299,83 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if ((balA[r] >> lane) & 1u) slot = wcA[r][warp] + __popc(balA[r] & lt);
                     else if ((balB[r] >> lane) & 1u) slot = nA + wcB[r][warp] + __popc(balB[r] & lt);
                     SV_CHK(slot < nL);
-                    if (slot >= 0) { sk[slot] = lk[r] & ~bit; sa[slot] = la[r]; }
+                    if (slot >= 0) { sk[DK(slot)] = lk[r] & ~bit; sa[DA(slot)] = la[r]; }
                 }
             }
         }
-        if (tid < 8 && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+        if (tid < (TWO ? 16 : 8) && next < ntiles) s_desc[par ^ 1][tid] = dnext;
         __syncthreads();
-        if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]));
+        if constexpr (TWO) { if (next < ntiles && tid == 0) issue_loads2(s_desc[par ^ 1], par ^ 1); }
+        else { if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1])); }
+
+        // ---- TWO, level 1: inside either bH class, merge its bL = 0 and bL = 1 entries by the rest of the key (two merges
+        // side by side over the output positions [0, nA) and [nA, nL)); bL goes to bit 0 ----
+        if constexpr (TWO) {
+            const int n00 = s_n4[0], n10 = s_n4[2];
+            const int d0 = min(tid * BP_VT, nL);
+            int seg = (d0 >= nA) ? 1 : 0;
+            int ob = seg ? nA : 0;          // first entry of this thread's pair of classes
+            int na = seg ? n10 : n00, nb = seg ? (nL - nA - n10) : (nA - n00);
+            const int dg = d0 - (seg ? nA : 0);
+            int i, j;
+            {
+                int lo = max(0, dg - nb), hi = min(dg, na);
+                while (lo < hi) {   // bL = 0 first on ties
+                    const int mid = (lo + hi) >> 1;
+                    if (sk[DK(ob + mid)] <= sk[DK(ob + na + dg - 1 - mid)]) lo = mid + 1; else hi = mid;
+                }
+                i = lo; j = dg - lo;
+            }
+            u64 ka = (i < na) ? sk[DK(ob + i)] : ~0ull, kb = (j < nb) ? sk[DK(ob + na + j)] : ~0ull;
+            u64 mk[BP_VT]; double2 ma_[BP_VT];
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v) {
+                mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
+                if (d0 + v < nL) {
+                    if (seg == 0 && d0 + v == nA) {   // this thread's outputs run over into the bH = 1 merge: it starts there
+                        seg = 1; ob = nA; na = n10; nb = nL - nA - n10; i = 0; j = 0;
+                        ka = (0 < na) ? sk[DK(ob)] : ~0ull; kb = (0 < nb) ? sk[DK(ob + na)] : ~0ull;
+                    }
+                    const bool takeA = ka <= kb;
+                    mk[v] = (takeA ? ka : kb) | (takeA ? 0ull : 1ull);
+                    ma_[v] = sa[DA(takeA ? ob + i : ob + na + j)];
+                    if (takeA) { ++i; ka = (i < na) ? sk[DK(ob + i)] : ~0ull; } else { ++j; kb = (j < nb) ? sk[DK(ob + na + j)] : ~0ull; }
+                }
+            }
+            __syncthreads();   // every read of the partitioned tile is done
+#pragma unroll
+            for (int v = 0; v < BP_VT; ++v)
+                if (d0 + v < nL) { sk[DK(d0 + v)] = mk[v]; sa[DA(d0 + v)] = ma_[v]; }
+            __syncthreads();
+        }
 
         // ---- phase 1: bring the tile into its new order (moved bit at the LSB) ----
         if (mv) {
             const int nB = nL - nA;
-            const u64* skB = sk + nA;
-            const double2* saB = sa + nA;
             const int diag = min(tid * BP_VT, nL);
             int i, j;
             {
                 int lo = max(0, diag - nB), hi = min(diag, nA);
-                while (lo < hi) {   // A first on ties
+                while (lo < hi) {   // A first on ties (TWO: bit 0 holds bL, not part of the comparison)
                     const int mid = (lo + hi) >> 1;
-                    if (sk[mid] <= skB[diag - 1 - mid]) lo = mid + 1; else hi = mid;
+                    const u64 xa = sk[DK(mid)], xb = sk[DK(nA + diag - 1 - mid)];
+                    if (TWO ? ((xa | 1ull) <= (xb | 1ull)) : (xa <= xb)) lo = mid + 1; else hi = mid;
                 }
                 i = lo; j = diag - lo;
             }
             SV_CHK(i >= 0 && i <= nA && j >= 0 && j <= nB);
             const int endpos = min(diag + BP_VT, nL);
-            u64 ka = (i < nA) ? sk[i] : ~0ull, kb = (j < nB) ? skB[j] : ~0ull;
+            u64 ka = (i < nA) ? sk[DK(i)] : ~0ull, kb = (j < nB) ? sk[DK(nA + j)] : ~0ull;
             u64 mk[BP_VT]; double2 ma_[BP_VT];
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v) {
                 mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
                 if (diag + v < endpos) {
-                    const bool takeA = ka <= kb;
+                    const bool takeA = TWO ? ((ka | 1ull) <= (kb | 1ull)) : (ka <= kb);
                     const u64 k = takeA ? ka : kb;
-                    ma_[v] = takeA ? sa[i] : saB[j];
-                    mk[v] = (k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull);
-                    if (takeA) { ++i; ka = (i < nA) ? sk[i] : ~0ull; } else { ++j; kb = (j < nB) ? skB[j] : ~0ull; }
+                    ma_[v] = sa[DA(takeA ? i : nA + j)];
+                    mk[v] = TWO ? (k | (takeA ? 0ull : 2ull)) : ((k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull));
+                    if (takeA) { ++i; ka = (i < nA) ? sk[DK(i)] : ~0ull; } else { ++j; kb = (j < nB) ? sk[DK(nA + j)] : ~0ull; }
                 }
             }
             // The tuples are found here, from the merged keys in registers: a thread's outputs are consecutive, its
@@ -231,7 +395,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 if (diag + v < endpos) {
                     const u64 before = v == 0 ? prev : mk[v - 1];
                     if ((diag + v == 0) || (before >> MA) != (mk[v] >> MA)) om |= 1u << v;
-                    sk[diag + v] = mk[v]; sa[diag + v] = ma_[v];
+                    sk[DK(diag + v)] = mk[v]; sa[DA(diag + v)] = ma_[v];
                 }
             }
             int cinc = __popc(om);
@@ -255,7 +419,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
                 const int e = tid + r * SV_THREADS;
-                const bool opens = (e < nL) && (e == 0 || (sk[e - 1] >> MA) != (sk[e] >> MA));
+                const bool opens = (e < nL) && (e == 0 || (sk[DK(e - 1)] >> MA) != (sk[DK(e)] >> MA));
                 bs[r] = __ballot_sync(0xffffffffu, opens);
                 if (lane == 0) wcA[r][warp] = __popc(bs[r]);
             }
@@ -299,11 +463,11 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 if (valid[u]) {
                     const int e = tst[ti], nm = (int)tst[ti + 1] - e;
                     SV_CHK(nm >= 1 && nm <= NP && e + nm <= nL);
-                    kb[u] = sk[e] & ~AM;
+                    kb[u] = sk[DK(e)] & ~AM;
                     if (col_ident || nm <= 2) {          // members in stored order = ascending logical column (or the order cannot matter)
                         for (int j = 0; j < nm; ++j) {
-                            const int x = (int)(sk[e + j] & AM);
-                            const double2 a = sa[e + j];
+                            const int x = (int)(sk[DK(e + j)] & AM);
+                            const double2 a = sa[DA(e + j)];
 #pragma unroll
                             for (int r = 0; r < NP; ++r) {
                                 const double2 uu = Us[r * NP + x];
@@ -312,11 +476,11 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                         }
                     } else {                              // ascending LOGICAL column index (D1)
                         u32 pk = 0;
-                        for (int j = 0; j < nm; ++j) pk |= 1u << (int)(sk[e + j] & AM);
+                        for (int j = 0; j < nm; ++j) pk |= 1u << (int)(sk[DK(e + j)] & AM);
                         for (int t = 0; t < NP; ++t) {
                             const int x = (int)((colpack >> (4 * t)) & 15ull);
                             if ((pk >> x) & 1u) {
-                                const double2 a = sa[e + __popc(pk & ((1u << x) - 1u))];
+                                const double2 a = sa[DA(e + __popc(pk & ((1u << x) - 1u)))];
 #pragma unroll
                                 for (int r = 0; r < NP; ++r) {
                                     const double2 uu = Us[r * NP + x];
@@ -485,22 +649,30 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     }
 }
 
-template <int MA, bool PRE>
+template <int MA, bool PRE, bool TWO>
 static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
-                            const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + 64 + (size_t)(BP_TILE + 8) * 2 +
+                            const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2) {
+    const size_t smem = (size_t)2 * BP_TILE * 24 + (TWO ? 128 : 64) + (size_t)(BP_TILE + 8) * 2 +
                         (PRE ? (size_t)DP_STAGE * 24 : (size_t)BP_WARPS * DP_WENT * 16 + (size_t)BP_WARPS * 64 * 8);
     static int per_sm[SV_MAX_DEV];
-    return sv_launch_persistent(densepass_kernel<MA, PRE>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
-                                (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead);
+    return sv_launch_persistent(densepass_kernel<MA, PRE, TWO>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
+                                (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead, p2);
 }
 
 // Dispatch for svk_grouppass (sv_group.cu): the final pass of a dense gate.  Returns the grid size.
 u32 svk_densepass_launch(int ma, bool use_pre, const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                          const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
-                         const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead) {
-#define SV_DP(MA_, PRE_) launch_densepass<MA_, PRE_>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt, maybe_dead)
+                         const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2) {
+#define SV_DP(MA_, PRE_) launch_densepass<MA_, PRE_, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt, maybe_dead, p2)
+    if (p2 >= 0) {   // two bits moved by this pass (desc: TileDesc2)
+        if (use_pre) {
+            switch (ma) { case 2: return SV_DP(2, true); case 3: return SV_DP(3, true); case 4: return SV_DP(4, true); default: return 0; }
+        }
+        switch (ma) { case 2: return SV_DP(2, false); case 3: return SV_DP(3, false); case 4: return SV_DP(4, false); default: return 0; }
+    }
+#undef SV_DP
+#define SV_DP(MA_, PRE_) launch_densepass<MA_, PRE_, false>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt, maybe_dead, -1)
     if (use_pre) {
         switch (ma) { case 2: return SV_DP(2, true); case 3: return SV_DP(3, true); case 4: return SV_DP(4, true); default: return 0; }
     }

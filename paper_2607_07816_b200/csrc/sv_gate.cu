@@ -242,3 +242,225 @@ int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, 
     return 1;
 }
 
+
+// ---------------------------------------------------------------------------------------
+// tile boundaries of a TWO-bit pass (bits pH > pL moved to the two least-significant positions by ONE streaming pass:
+// a four-way merge per tile, sv_dense.cu).  One thread per boundary.
+//
+// Read a stored key as (high, bH, mid, bL, low) and let rest = (high, mid, low): the pass emits the state in (rest, bH, bL)
+// order, so tile j holds the entries whose rank in REST order is in [j tnom, (j + 1) tnom) -- pulled back to the start of a
+// tuple.  The boundary is the value R = (h, m, l) of rest with that rank (a selection over the four sorted sub-sequences
+// the patterns of (bH, bL) form), found in four steps that only ever take lower bounds over the stored (sorted) keys:
+//   (1) the block h of keys that agree above pH, its halves A = [s1, mid1), B = [mid1, e1): the stored position T = j tnom lies
+//       in it, and the block holds the same entries in either order, so the rank inside the block is T - s1;
+//   (2) m: both halves are sorted by mid -- a merge-path co-rank search on the mid bits gives the mid value of that rank;
+//   (3) the sub-blocks (h, 0, m) and (h, 1, m), each a bL = 0 run followed by a bL = 1 run, all four sorted by low;
+//   (4) l: the low value of the remaining rank among the four runs, by descent over the bits of low (bits on which all
+//       entries still in question agree are skipped; one partition point per run and bit, found together).
+// The entries before R are then four stored ranges (TileDesc2); a tile is the difference of two such sets: at most seven
+// contiguous pieces.
+// ---------------------------------------------------------------------------------------
+// K lower bounds over the sorted keys advanced TOGETHER (their dependent loads overlap).  On entry lo[k] <= answer <= hi[k],
+// answer = first index in [lo, hi) whose key is >= v[k] (hi if none); hint[k] is a position near it: a bounded gallop from
+// the hint brackets the answer before the binary search starts.  On return lo[k] == hi[k] == answer.
+template <int K>
+__device__ __forceinline__ void multi_lower_bound(const u64* __restrict__ keys, u64 (&lo)[K], u64 (&hi)[K], const u64 (&v)[K],
+                                                  const u64 (&hint)[K]) {
+    bool go[K], up[K];
+    u64 c[K], kk[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        go[k] = lo[k] < hi[k];
+        u64 h = hint[k] < lo[k] ? lo[k] : hint[k];
+        if (go[k] && h >= hi[k]) h = hi[k] - 1;
+        c[k] = h;
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) kk[k] = go[k] ? keys[c[k]] : 0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        up[k] = false;
+        if (go[k]) {
+            if (kk[k] < v[k]) { lo[k] = c[k] + 1; up[k] = true; } else hi[k] = c[k];
+            go[k] = lo[k] < hi[k];
+        }
+    }
+    for (u64 step = 1; step <= 2048; step <<= 1) {
+        bool any = false;
+#pragma unroll
+        for (int k = 0; k < K; ++k) any = any || go[k];
+        if (!any) break;
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+            c[k] = up[k] ? ((lo[k] + step - 1 < hi[k]) ? lo[k] + step - 1 : hi[k] - 1) : ((hi[k] - lo[k] > step) ? hi[k] - step : lo[k]);
+#pragma unroll
+        for (int k = 0; k < K; ++k) kk[k] = go[k] ? keys[c[k]] : 0;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            if (go[k]) {
+                if (kk[k] < v[k]) { lo[k] = c[k] + 1; go[k] = up[k] && lo[k] < hi[k]; }
+                else { hi[k] = c[k]; go[k] = !up[k] && lo[k] < hi[k]; }
+            }
+        }
+    }
+    for (;;) {
+        bool any = false;
+#pragma unroll
+        for (int k = 0; k < K; ++k) any = any || (lo[k] < hi[k]);
+        if (!any) break;
+#pragma unroll
+        for (int k = 0; k < K; ++k) c[k] = lo[k] + ((hi[k] - lo[k]) >> 1);
+#pragma unroll
+        for (int k = 0; k < K; ++k) kk[k] = (lo[k] < hi[k]) ? keys[c[k]] : 0;
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+            if (lo[k] < hi[k]) { if (kk[k] < v[k]) lo[k] = c[k] + 1; else hi[k] = c[k]; }
+    }
+}
+
+__global__ void find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles,
+                                    TileDesc2* __restrict__ desc) {
+    const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j > ntiles) return;
+    TileDesc2 d;
+    d.pad_ = 0;
+    const u64 T = (u64)j * tnom;
+    if (j == ntiles || T >= n) { d.p00 = d.m2a = d.p01 = d.m1 = d.p10 = d.m2b = d.p11 = n; desc[j] = d; return; }
+    const u64 bitH = 1ull << pH, bitL = 1ull << pL;             // pL < pH <= 63
+    const u64 maskH = (pH == 63) ? 0ull : ~((2ull << pH) - 1);
+    const u64 maskL = bitL - 1;
+    const u64 maskM = (bitH - 1) & ~((2ull << pL) - 1);
+    const u64 kt = keys[T];
+    const u64 hb = kt & maskH;
+    // (1) the block of keys that agree above pH
+    u64 s1, mid1, e1;
+    {
+        const u64 nxt = hb + (bitH << 1);                        // pH == 63: 0
+        const bool has_e = (pH < 63) && nxt != 0;                // nxt == 0: wrapped, last block
+        const bool inB = (kt & bitH) != 0;
+        u64 lo[3] = {0, inB ? 0 : T + 1, has_e ? T + 1 : n};
+        u64 hi[3] = {(pH == 63) ? 0 : T, inB ? T : n, n};
+        const u64 v[3] = {hb, hb | bitH, nxt};
+        const u64 hint[3] = {T, T, T + 1};
+        multi_lower_bound<3>(keys, lo, hi, v, hint);
+        s1 = lo[0]; mid1 = lo[1]; e1 = lo[2];
+    }
+    // (2) co-rank on the mid bits (the bH = 0 half first on ties): the mid value of rank diag inside the block
+    const u64 lenA = mid1 - s1, lenB = e1 - mid1, diag = T - s1;
+    u64 ia, jb, m;
+    {
+        u64 lo = diag > lenB ? diag - lenB : 0, hi = diag < lenA ? diag : lenA;
+        while (lo < hi) {
+            const u64 i = lo + ((hi - lo) >> 1);
+            const u64 ka = keys[s1 + i] & maskM, kb = keys[mid1 + (diag - 1 - i)] & maskM;
+            if (ka <= kb) lo = i + 1; else hi = i;
+        }
+        ia = lo; jb = diag - lo;
+        const bool hasA = ia < lenA, hasB = jb < lenB;           // (one of them: diag < lenA + lenB)
+        const u64 ka = hasA ? (keys[s1 + ia] & maskM) : 0, kb = hasB ? (keys[mid1 + jb] & maskM) : 0;
+        m = (hasA && (!hasB || ka <= kb)) ? ka : kb;
+    }
+    // (3) the sub-blocks (h, 0, m) and (h, 1, m): start, start of the bL = 1 run, end
+    u64 st[4], en[4];
+    {
+        const u64 b0 = hb | m, b1 = b0 | bitH;
+        u64 lo[6] = {s1, s1, s1, mid1, mid1, mid1};
+        u64 hi[6] = {mid1, mid1, mid1, e1, e1, e1};
+        const u64 v[6] = {b0, b0 | bitL, b0 + (bitL << 1), b1, b1 | bitL, b1 + (bitL << 1)};
+        if (v[5] < b1) lo[5] = hi[5];                            // wrapped: the sub-block ends with the half
+        const u64 hint[6] = {s1 + ia, s1 + ia, s1 + ia, mid1 + jb, mid1 + jb, mid1 + jb};
+        multi_lower_bound<6>(keys, lo, hi, v, hint);
+        st[0] = lo[0]; en[0] = lo[1]; st[1] = lo[1]; en[1] = lo[2];
+        st[2] = lo[3]; en[2] = lo[4]; st[3] = lo[4]; en[3] = lo[5];
+    }
+    const u64 diag2 = diag - (st[0] - s1) - (st[2] - mid1);      // rank among the entries of the two sub-blocks, by low
+    // (4) the low value of that rank among the four runs
+    u64 x[4] = {st[0], st[1], st[2], st[3]};
+    u64 l = 0;
+    if (pL > 0) {
+        u64 lo4[4], hi4[4], fk[4], lk[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) { lo4[c] = st[c]; hi4[c] = en[c]; }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const bool ne = lo4[c] < hi4[c];
+            fk[c] = ne ? (keys[lo4[c]] & maskL) : 0; lk[c] = ne ? (keys[hi4[c] - 1] & maskL) : 0;
+        }
+        u64 prefix = 0;
+        int q = pL - 1;
+        while (q >= 0) {
+            u64 ref = 0, diff = 0;
+            bool have = false;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if (lo4[c] < hi4[c]) {
+                    if (!have) { ref = fk[c]; have = true; }
+                    diff |= (fk[c] ^ ref) | (lk[c] ^ ref);
+                }
+            const u64 below_q = (2ull << q) - 1;                 // q <= 61
+            diff &= below_q;
+            if (diff == 0) { prefix |= ref & below_q; break; }   // every entry still in question has the same low value
+            const int nq = 63 - __clzll((long long)diff);
+            prefix |= ref & below_q & ~((2ull << nq) - 1);       // the bits they agree on
+            q = nq;
+            const u64 qb = 1ull << q;
+            u64 a[4], b[4];                                      // partition point of every run on bit q: first entry with the bit set
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                a[c] = lo4[c]; b[c] = hi4[c];
+                if (a[c] < b[c]) {
+                    if (fk[c] & qb) b[c] = a[c];
+                    else if (!(lk[c] & qb)) a[c] = b[c];
+                    else { a[c] += 1; b[c] -= 1; }
+                }
+            }
+            for (;;) {
+                bool any = false;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) any = any || (a[c] < b[c]);
+                if (!any) break;
+                u64 mm[4], kk[4];
+#pragma unroll
+                for (int c = 0; c < 4; ++c) mm[c] = a[c] + ((b[c] - a[c]) >> 1);
+#pragma unroll
+                for (int c = 0; c < 4; ++c) kk[c] = (a[c] < b[c]) ? keys[mm[c]] : 0;
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    if (a[c] < b[c]) { if (kk[c] & qb) b[c] = mm[c]; else a[c] = mm[c] + 1; }
+            }
+            u64 below = 0;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) below += a[c] - st[c];
+            const bool one = below <= diag2;                     // the wanted entry has bit q set
+            if (one) prefix |= qb;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                if (one) lo4[c] = a[c]; else hi4[c] = a[c];
+            }
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const bool ne = lo4[c] < hi4[c];
+                if (one) fk[c] = ne ? (keys[lo4[c]] & maskL) : 0; else lk[c] = ne ? (keys[hi4[c] - 1] & maskL) : 0;
+            }
+            --q;
+        }
+        l = prefix;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) x[c] = lo4[c];
+        // never split a tuple: its members differ in bH, bL and in the w lowest bits
+        const u64 l_al = l & ~((1ull << w) - 1);
+        if (l_al != l) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                while (x[c] > st[c] && (keys[x[c] - 1] & maskL) >= l_al) --x[c];
+        }
+    }
+    d.p00 = x[0]; d.m2a = st[1]; d.p01 = x[1]; d.m1 = mid1; d.p10 = x[2]; d.m2b = st[3]; d.p11 = x[3];
+    desc[j] = d;
+}
+
+int svk_find_splits2(const u64* keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles, TileDesc2* desc, cudaStream_t st) {
+    const u32 nb = (ntiles + 1 + 127) / 128;
+    find_splits2_kernel<<<nb, 128, 0, st>>>(keys, n, pH, pL, w, tnom, ntiles, desc);
+    return 1;
+}

@@ -371,12 +371,12 @@ static u32 launch_grouppass(const u64* kin, const double2* ain, u64* kout, doubl
 // stored outputs to d_count[0] and the number of dead ones among them (exact cancellations) to d_count[1].
 u32 svk_densepass_launch(int ma, bool use_pre, const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                          const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
-                         const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead);   // sv_dense.cu
+                         const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2);   // sv_dense.cu
 
 int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, int p, int ma,
                   const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
                   u64 cap, cudaStream_t st, cudaEvent_t e0, cudaEvent_t e1, const PreCut* pre, double* pre_mass, u64* pre_cnt,
-                  u32* pre_parts, int dense, int maybe_dead) {
+                  u32* pre_parts, int dense, int maybe_dead, int p2) {
     cudaMemsetAsync(d_count, 0, 2 * sizeof(u64), st);
     if (pre_parts) *pre_parts = 0;
     if (n == 0) return 0;
@@ -384,12 +384,14 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
     const u32 ntiles = (u32)((n + tnom - 1) / tnom);
     cudaMemsetAsync(status, 0, ((size_t)ntiles + (ntiles + 31) / 32 + 8) * sizeof(u64), st);
     int launches = 1;
-    if (p >= 0) launches += svk_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
+    const bool two = dense && p >= 0 && p2 >= 0 && p2 < p && ma >= 2 && ma <= 4;   // two bits moved by this pass (sv_dense.cu)
+    if (two) launches += svk_find_splits2(kin, n, p, p2, ma - 2, tnom, ntiles, reinterpret_cast<TileDesc2*>(desc), st);
+    else if (p >= 0) launches += svk_find_splits(kin, n, p, ma - 1, tnom, ntiles, desc, st);
     else { find_starts_kernel<<<(ntiles + 1 + 127) / 128, 128, 0, st>>>(kin, n, ma, tnom, ntiles, desc); launches += 1; }
     if (e0) cudaEventRecord(e0, st);
     if (dense && ma >= 2 && ma <= 4) {   // every entry of U nonzero, no control-like bit: sv_dense.cu
         const u32 g = svk_densepass_launch(ma, pre != nullptr, kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st,
-                                           pre, pre_mass, pre_cnt, maybe_dead);
+                                           pre, pre_mass, pre_cnt, maybe_dead, two ? p2 : -1);
         if (pre && pre_parts) *pre_parts = g;
     } else if (pre) {
         u32 g = 0;

@@ -29,6 +29,16 @@ struct TileDesc {
     u64 e;    // end of the block
 };
 
+// One tile boundary of a TWO-bit pass (bits pH > pL go to the two least-significant positions in one pass; sv_gate.cu
+// find_splits2, sv_dense.cu).  With the stored key read as (high, bH, mid, bL, low) and rest = (high, mid, low), the
+// boundary is a value R = (h, m, l) of rest; the entries with rest < R are the stored ranges
+//   [0, p00)  [m2a, p01)  [m1, p10)  [m2b, p11)
+// p00 / p01 / p10 / p11: lower bounds of (h, bH, m, bL, l) for the four patterns of (bH, bL); m1: start of the bH = 1
+// half of block h; m2a / m2b: start of the bL = 1 run of the sub-block (h, bH, m) of either half.
+struct TileDesc2 {
+    u64 p00, m2a, p01, m1, p10, m2b, p11, pad_;
+};
+
 // Radix-select state (device resident; one per handle).  See sv_radix_select.cu.
 struct SelState {
     int phase;           // 0 exponent level, 1 adaptive pattern levels, 2 tie keys to be extracted, 3 key levels
@@ -113,6 +123,8 @@ size_t svk_small_smem();
 int svk_small_gates(u64* keys, double2* amps, SmallCtl* ctl, const SmallGate* gates, int n_gates, KeyMap km, u64 max_terms, double min_mass,
                     double* kept_out, u64 cap, int threads, cudaStream_t st);
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st);
+// out[0] = OR, out[1] = AND of the stored keys of the live entries (amps == nullptr: of all stored entries)
+int svk_key_masks(const u64* keys, const double2* amps, u64 n, const PendPred& pd, int with_pend, u64* out, cudaStream_t st);
 
 // ---- launchers (each enqueues on `st` and returns the number of kernels launched) ----
 int svk_diag(const u64* keys, double2* amps, u64 n, const GateTab* tab, cudaStream_t st);
@@ -124,7 +136,8 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
                   const GateTab* tab, const PendPred& pend, TileDesc* desc, u64* status, u64* d_count,
                   u64 cap, cudaStream_t st, cudaEvent_t e0 = nullptr, cudaEvent_t e1 = nullptr,
                   const PreCut* pre = nullptr, double* pre_mass = nullptr, u64* pre_cnt = nullptr, u32* pre_parts = nullptr,
-                  int dense = 0, int maybe_dead = 1);   // dense: U has no zero entry and no control-like bit (sv_dense.cu)
+                  int dense = 0, int maybe_dead = 1,    // dense: U has no zero entry and no control-like bit (sv_dense.cu)
+                  int p2 = -1);                         // dense only: a SECOND bit (p2 < p) moved by the same pass, see TileDesc2
 
 // Lean single-bit pass (sv_pair.cu): moves physical bit p to the LSB in one streaming pass.
 // pair != 0: final pass of a gate with ONE active bit (tuple mat-vec + zero drop fused);
@@ -141,10 +154,12 @@ int svk_bitpass(const u64* kin, const double2* ain, u64* kout, double2* aout, u6
 int svk_pre_sample1(const u64* keys, const double2* amps, u64 n, int p, const GateTab* tab, const PendPred& pend, u32 M, u64* smp,
                     cudaStream_t st);
 int svk_pre_sample_group(const u64* keys, const double2* amps, u64 n, int p, int ma, const GateTab* tab, const PendPred& pend, u32 M,
-                         u64* smp, cudaStream_t st);
+                         u64* smp, cudaStream_t st, int p2 = -1);
 int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u32 mult, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st);
 int svk_pre_finish(const double* part_mass, const u64* part_cnt, u32 nparts, PreCut* pre, u64* d_count, cudaStream_t st);
 int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
+// boundaries of a two-bit pass: bits pH > pL; w low bits of the key belong to the tuple (boundaries are aligned to it)
+int svk_find_splits2(const u64* keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles, TileDesc2* desc, cudaStream_t st);
 // Diagonal gate fused with a pending truncation (out of place, compacting).
 int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
                      const PendPred& pend, u64* status, u32* tile_counter, u64* d_count, cudaStream_t st);

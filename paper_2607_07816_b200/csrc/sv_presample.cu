@@ -91,16 +91,22 @@ __global__ void __launch_bounds__(SV_THREADS) pre_sample1_kernel(const u64* __re
 // ONE of the 2^ma output rows: every (tuple, row) pair has the probability 1 / (2^ma n).
 __global__ void __launch_bounds__(SV_THREADS) pre_sample_group_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps,
                                                                       u64 n, int p, int ma, const GateTab* __restrict__ gtab, PendPred pd,
-                                                                      u32 M, u64* __restrict__ smp) {
+                                                                      u32 M, u64* __restrict__ smp, int p2) {
     const u32 t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= M) return;
     const u64 i = ps_position(t, n, M);
     const bool mv = p >= 0;
+    const bool two = mv && p2 >= 0;        // the final pass moves two bits (p > p2): the members sit in four runs
     const int np = 1 << ma;
     const u64 AM = (u64)np - 1;
     const u64 bit = mv ? (1ull << p) : 0ull;
     const u64 himask = (!mv || p == 63) ? 0 : ~((2ull << p) - 1), lowmask = bit - 1;
-    auto new_key = [&](u64 k) { return mv ? ((k & himask) | ((k & lowmask) << 1) | ((k >> p) & 1ull)) : k; };
+    const u64 bit2 = two ? (1ull << p2) : 0ull;
+    const u64 midmask = two ? ((bit - 1) & ~((bit2 << 1) - 1)) : 0ull, lowmask2 = two ? (bit2 - 1) : 0ull;
+    auto new_key = [&](u64 k) {
+        if (two) return (k & himask) | ((k & midmask) << 1) | ((k & lowmask2) << 2) | (((k >> p) & 1ull) << 1) | ((k >> p2) & 1ull);
+        return mv ? ((k & himask) | ((k & lowmask) << 1) | ((k >> p) & 1ull)) : k;
+    };
     auto live_amp = [&](u64 idx, u64 key) {
         double2 a = amps[idx];
         if (pd.active) {
@@ -117,10 +123,11 @@ __global__ void __launch_bounds__(SV_THREADS) pre_sample_group_kernel(const u64*
         double2 av[16];
         u32 pm = 0;
         // the runs of stored keys that hold the tuple's members
-        const u64 low = mv ? (((u64)np >> 1) - 1) : AM;           // stored low bits that vary inside a run
-        const int nruns = mv ? 2 : 1;
+        const u64 low = two ? (((u64)np >> 2) - 1) : (mv ? (((u64)np >> 1) - 1) : AM);   // stored low bits that vary inside a run
+        const int nruns = two ? 4 : (mv ? 2 : 1);
         for (int rr = 0; rr < nruns; ++rr) {
-            const u64 base = mv ? (((k & ~bit) & ~low) | (rr ? bit : 0ull)) : (k & ~low);
+            const u64 base = two ? (((k & ~bit & ~bit2) & ~low) | ((rr & 2) ? bit : 0ull) | ((rr & 1) ? bit2 : 0ull))
+                                 : (mv ? (((k & ~bit) & ~low) | (rr ? bit : 0ull)) : (k & ~low));
             u64 lo = 0, hi = n;
             while (lo < hi) { const u64 mid = (lo + hi) >> 1; if (keys[mid] < base) lo = mid + 1; else hi = mid; }
             for (u64 j = lo; j < n && j <= lo + low; ++j) {
@@ -203,8 +210,8 @@ int svk_pre_sample1(const u64* keys, const double2* amps, u64 n, int p, const Ga
     return 1;
 }
 int svk_pre_sample_group(const u64* keys, const double2* amps, u64 n, int p, int ma, const GateTab* tab, const PendPred& pend, u32 M,
-                         u64* smp, cudaStream_t st) {
-    pre_sample_group_kernel<<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(keys, amps, n, p, ma, tab, pend, M, smp);
+                         u64* smp, cudaStream_t st, int p2) {
+    pre_sample_group_kernel<<<(M + SV_THREADS - 1) / SV_THREADS, SV_THREADS, 0, st>>>(keys, amps, n, p, ma, tab, pend, M, smp, p2);
     return 1;
 }
 int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u32 mult, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st) {

@@ -1,7 +1,7 @@
 // Norm, the compaction pass of a truncation (row a-9, also fused with a
 // diagonal gate), readout gather and structural checks.  The cut itself is found by the
 // radix select in sv_radix_select.cu.
-#include "sv_device.cuh"
+#include "sv_tile.cuh"
 
 // ---------------------------------------------------------------------------------------
 // a-10 norm: fixed-order two-stage reduction (deterministic)
@@ -55,6 +55,38 @@ __global__ void __launch_bounds__(SV_THREADS) count_live_kernel(const double2* _
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(reinterpret_cast<unsigned long long*>(d_count), (unsigned long long)c);
+}
+// OR and AND of the stored keys of the live entries (a pending truncation applied when with_pend): a stored bit on which
+// the two agree has the same value in every term -- the qubit it holds is in a definite state, and bringing it to another
+// bit position does not change the order of the keys (sv_api.cu "definite qubits").  out[0] = OR, out[1] = AND.
+__global__ void __launch_bounds__(SV_THREADS) key_masks_kernel(const u64* __restrict__ keys, const double2* __restrict__ amps, u64 n,
+                                                               PendPred pd, int with_pend, u64* __restrict__ out) {
+    u64 o = 0, a = ~0ull;
+    const u64 stride = (u64)gridDim.x * blockDim.x;
+    for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+        const u64 k = ld_stream_u64(keys + i);
+        bool live = true;
+        if (amps) {
+            const double2 v = ld_stream_d2(amps + i);
+            live = (with_pend && pd.active) ? pend_keep(pd, k, v) : !(v.x == 0.0 && v.y == 0.0);
+        }
+        if (live) { o |= k; a &= k; }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { o |= __shfl_xor_sync(0xffffffffu, o, d); a &= __shfl_xor_sync(0xffffffffu, a, d); }
+    if ((threadIdx.x & 31) == 0) {
+        atomicOr(reinterpret_cast<unsigned long long*>(&out[0]), (unsigned long long)o);
+        atomicAnd(reinterpret_cast<unsigned long long*>(&out[1]), (unsigned long long)a);
+    }
+}
+int svk_key_masks(const u64* keys, const double2* amps, u64 n, const PendPred& pd, int with_pend, u64* out, cudaStream_t st) {
+    const u64 init[2] = {0ull, ~0ull};
+    cudaMemcpyAsync(out, init, sizeof(init), cudaMemcpyHostToDevice, st);
+    if (n == 0) return 0;
+    u64 blocks = (n + SV_THREADS * 8 - 1) / (SV_THREADS * 8);
+    if (blocks > (u64)sv_sm_count() * 8) blocks = (u64)sv_sm_count() * 8;
+    key_masks_kernel<<<(unsigned)blocks, SV_THREADS, 0, st>>>(keys, amps, n, pd, with_pend, out);
+    return 1;
 }
 int svk_count_live(const double2* amps, u64 n, u64* d_count, cudaStream_t st) {
     cudaMemsetAsync(d_count, 0, sizeof(u64), st);

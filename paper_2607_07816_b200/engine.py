@@ -20,10 +20,11 @@ EXPORTS = ["sv_arena_bytes", "sv_create", "sv_create_in_arena", "sv_destroy", "s
            "sv_norm", "sv_top", "sv_num_terms", "sv_load", "sv_load_device", "sv_get_stats",
            "sv_check_invariants", "sv_last_error", "sv_sync", "sv_profile", "sv_profile_get", "sv_set_option",
            "sv_apply_gate_truncate", "sv_fuse_gates", "sv_reorder_gates", "sv_apply_circuit"]
-TEST_EXPORTS = ["sv_test_set_pre_slack"]      # include/sparse_sv_test.h
+TEST_EXPORTS = ["sv_test_set_pre_slack", "sv_test_definite_qubits"]      # include/sparse_sv_test.h
 KERNELS = ["diag", "move", "bitpass", "sel_hist", "compact", "classify", "grouppass", "bitpass_gen"]
 OPT_SAMPLE_MIN_TERMS = 0
 OPT_SMALL_STATE_PATH = 2
+OPT_TWO_BIT_PASS = 3
 
 
 class SvStats(C.Structure):
@@ -94,6 +95,8 @@ def load_library(path: str = _LIBPATH):
     lib.sv_set_option.argtypes = [vp, i32, u64]
     lib.sv_test_set_pre_slack.restype = i32
     lib.sv_test_set_pre_slack.argtypes = [vp, C.c_longlong]
+    lib.sv_test_definite_qubits.restype = i32
+    lib.sv_test_definite_qubits.argtypes = [vp, C.POINTER(C.c_uint64)]
     return lib
 
 
@@ -283,6 +286,12 @@ class SparseSV:
     def test_set_pre_slack(self, slack: int):
         """Test hook (include/sparse_sv_test.h)."""
         self._chk(lib.sv_test_set_pre_slack(self._h, int(slack)))
+
+    def test_definite_qubits(self) -> int:
+        """Test hook (include/sparse_sv_test.h): bit q set iff qubit q has the same value in every term."""
+        m = C.c_uint64(0)
+        self._chk(lib.sv_test_definite_qubits(self._h, C.byref(m)))
+        return int(m.value)
 
     def check_invariants(self) -> bool:
         ok = C.c_int(0)
