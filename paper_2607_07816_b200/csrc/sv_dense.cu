@@ -26,7 +26,7 @@
 #include <type_traits>
 
 #ifndef DP_NOPRE_BLOCKS
-#define DP_NOPRE_BLOCKS 3                  // resident blocks per SM of the two-call variant (ma <= 3)
+#define DP_NOPRE_BLOCKS 4                  // resident blocks per SM of the two-call variant (ma <= 3): 64 registers, ~51 KB of shared memory
 #endif
 #define DP_WENT 128                        // !PRE: entries of a warp's transposition buffer
 // The tile arrays (keys sk, amplitudes sa) are addressed through an XOR swizzle of the entry index with its 128-byte row
@@ -63,8 +63,8 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
     u64* sk = Lk + BP_TILE + LKX;
     unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
-    double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE: staged survivors, output order; else the warps' transposition buffers
-    u64* stg_k = reinterpret_cast<u64*>(stg_a + (PRE ? DP_STAGE : BP_WARPS * DP_WENT));
+    double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE only: staged survivors, output order
+    u64* stg_k = reinterpret_cast<u64*>(stg_a + DP_STAGE);
     __shared__ int wcA[BP_VT][BP_WARPS], wcB[BP_VT][BP_WARPS];
     __shared__ int s_nA, s_nB, s_nt;
     __shared__ u64 s_last[BP_WARPS];        // last merged key of every warp (tuple starts across warps)
@@ -493,14 +493,11 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             }
         };
         if constexpr (!PRE) {
-            // ---- two calls: every candidate is an output.  The rows a thread holds are consecutive outputs; each warp
-            // transposes its round through its own 4 KB of shared memory (XOR-swizzled 16-byte entries: conflict free
-            // both ways) so that consecutive lanes store consecutive entries ----
-            double2* W = stg_a + warp * DP_WENT;
-            u64* KB = stg_k + warp * (32 * TPR);
-            constexpr int TP = DP_WENT / NP;             // tuples per transposition phase
-            constexpr int PH = (32 * TPR) / TP;          // phases per round
-            constexpr int SWS = MA > 3 ? MA : 3;
+            // ---- two calls: every candidate is an output.  The 2^MA rows a thread holds are CONSECUTIVE outputs (64 bytes of
+            // amplitudes, 32 of keys for MA = 2), the tuples of consecutive lanes follow one another, and a tile's first
+            // output is a multiple of 2^MA: every thread stores its rows straight from registers with 256-bit stores, each a
+            // whole 32-byte sector.  (Until round 2 every warp transposed its round through shared memory so that
+            // consecutive lanes stored consecutive 16-byte entries: a third of the pass's shared-memory wavefronts.) ----
             for (int h = 0; h < NT; h += SV_THREADS * TPR) {
                 const int hw = h + warp * (32 * TPR);
                 double accr[TPR][NP], acci[TPR][NP]; u64 kb[TPR]; bool valid[TPR];
@@ -522,30 +519,21 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     base = s_base; have_base = true;
                 }
 #pragma unroll
-                for (int ph = 0; ph < PH; ++ph) {
+                for (int u = 0; u < TPR; ++u) {
+                    if (!valid[u]) continue;
+                    const u64 g0 = base + ((u64)(hw + u * 32 + lane) << MA);
+                    if (g0 + (u64)NP <= cap) {
 #pragma unroll
-                    for (int u = 0; u < TPR; ++u) {
-                        const int sl = u * 32 + lane;                  // this thread's tuple slot in the warp's round
-                        if (sl / TP == ph) {
-                            const int tl = sl % TP;
-                            KB[sl] = kb[u];
+                        for (int r = 0; r < NP; r += 4)
+                            st_stream_u64x4(kout + g0 + r, kb[u] | (u64)r, kb[u] | (u64)(r + 1), kb[u] | (u64)(r + 2), kb[u] | (u64)(r + 3));
 #pragma unroll
-                            for (int r = 0; r < NP; ++r) {
-                                const int en = tl * NP + r;
-                                W[en ^ ((en >> SWS) & 7)] = make_double2(accr[u][r], acci[u][r]);
-                            }
-                        }
+                        for (int r = 0; r < NP; r += 2)
+                            st_stream_d2x2(aout + g0 + r, accr[u][r], acci[u][r], accr[u][r + 1], acci[u][r + 1]);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < NP; ++r)
+                            if (g0 + (u64)r < cap) { st_stream_u64(kout + g0 + r, kb[u] | (u64)r); st_stream_d2(aout + g0 + r, make_double2(accr[u][r], acci[u][r])); }
                     }
-                    __syncwarp();
-#pragma unroll
-                    for (int s = 0; s < DP_WENT / 32; ++s) {
-                        const int o = s * 32 + lane;
-                        const int sl = ph * TP + (o >> MA), row = o & (NP - 1);
-                        const int ti = hw + sl;
-                        const u64 g = base + ((u64)ti << MA) + (u64)row;
-                        if (ti < NT && g < cap) { st_stream_u64(kout + g, KB[sl] | (u64)row); st_stream_d2(aout + g, W[o ^ ((o >> SWS) & 7)]); }
-                    }
-                    __syncwarp();
                 }
             }
             if (!have_base) {   // (a tile without a live term still takes part in the chain)
@@ -654,7 +642,7 @@ static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, doubl
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2) {
     const size_t smem = (size_t)2 * BP_TILE * 24 + (TWO ? 128 : 64) + (size_t)(BP_TILE + 8) * 2 +
-                        (PRE ? (size_t)DP_STAGE * 24 : (size_t)BP_WARPS * DP_WENT * 16 + (size_t)BP_WARPS * 64 * 8);
+                        (PRE ? (size_t)DP_STAGE * 24 : 0);   // (two calls: the outputs are stored straight from registers)
     static int per_sm[SV_MAX_DEV];
     return sv_launch_persistent(densepass_kernel<MA, PRE, TWO>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
                                 (const TileDesc*)desc, status, d_count, cap, ntiles, pre, pre_mass, pre_cnt, maybe_dead, p2);

@@ -40,6 +40,13 @@ __device__ __forceinline__ u64 ld_stream_u64(const u64* p) {
 __device__ __forceinline__ void st_stream_d2(double2* p, double2 v) {
     asm volatile("st.global.L1::no_allocate.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(v.x), "d"(v.y) : "memory");
 }
+// 256-bit streaming stores (sm_100: STG.256): four keys / two amplitudes, the address 32-byte aligned -- one whole sector
+__device__ __forceinline__ void st_stream_u64x4(u64* p, u64 a, u64 b, u64 c, u64 d) {
+    asm volatile("st.global.L1::no_allocate.v4.b64 [%0], {%1, %2, %3, %4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
+}
+__device__ __forceinline__ void st_stream_d2x2(double2* p, double ax, double ay, double bx, double by) {
+    asm volatile("st.global.L1::no_allocate.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(ax), "d"(ay), "d"(bx), "d"(by) : "memory");
+}
 __device__ __forceinline__ void st_stream_u64(u64* p, u64 v) {
     asm volatile("st.global.L1::no_allocate.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
