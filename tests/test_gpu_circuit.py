@@ -151,3 +151,42 @@ def test_circuit_call_errors(eng):
     with pytest.raises(eng.SvError) as ei:
         sv.apply_circuit([([q], W.mat_h()) for q in range(10)], 0, 1.0)
     assert ei.value.code in (eng.SV_ERR_CAPACITY,)
+
+
+def test_qasm_text_through_the_circuit_call(eng):
+    """OpenQASM 2.0 text in the shape of the paper's excerpt (u3 + cz on a ring; own seeded angles) ->
+    qasm.loads -> reorder + fuse -> ONE sv_apply_circuit call with top-k after every block, against the oracle running
+    the same blocks, and the peak is found."""
+    from paper_2607_07816_b200 import qasm
+    import math
+    rng = np.random.default_rng(21)
+    n, layers = 16, 3
+    ring, ops = [], []
+    for layer in range(layers):
+        for a in range(layer % 2, n - 1 + layer % 2, 2):
+            b = (a + 1) % n
+            ring += [("u3", a, float(rng.uniform(0, math.pi)), 0.0, -0.5 * math.pi), ("u3", b, float(rng.uniform(0, math.pi)), 0.0, 0.5 * math.pi), ("cz", a, b)]
+    ops += ring
+    ops += [("u3", q, float(rng.normal(0.0, 0.3)), 0.0, 0.0) for q in range(n)]
+    for o in reversed(ring):          # R^dagger: cz is its own inverse, u3(t, p, l)^-1 = u3(-t, -l, -p)
+        ops.append(o if o[0] == "cz" else ("u3", o[1], -o[2], -o[4], -o[3]))
+    secret = int(rng.integers(0, 1 << n))
+    ops += [("u3", q, math.pi, 0.0, math.pi) for q in range(n) if (secret >> q) & 1]
+    c = qasm.loads(qasm.dumps_u3_cz(n, ops))
+    assert c.n == n and len(c.gates) == len(ops)
+    gates = [(list(g.qubits), g.U) for g in c.gates]
+    order = eng.reorder_gates(gates, [W.is_diagonal(U) for _, U in gates])
+    blocks = eng.fuse_gates([gates[i] for i in order], 4)
+    K = 128
+    sv = eng.SparseSV(n, 1 << 14)
+    kf = sv.apply_circuit(blocks, K, 1.0)
+    o = _oracle(n)
+    ko = []
+    for q, U in blocks:
+        o.apply_gate(q, U)
+        ko.append(o.truncate(K, 1.0))
+    assert np.allclose(kf, ko, atol=1e-9, rtol=0)
+    k, _, p = sv.top(1)
+    k2, _, p2 = o.top(1)
+    assert int(k[0]) == int(k2[0]) == secret
+    assert abs(p[0] - p2[0]) <= 1e-9
