@@ -174,18 +174,19 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
         pk_valid = false;
     };
 
+    const u32 tile0 = first_tile_of_block<!PRE>();
     if constexpr (TWO) {
-        if (tid < 16) s_desc[0][tid] = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + blockIdx.x)[tid];
+        if (tid < 16) s_desc[0][tid] = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + tile0)[tid];
         __syncthreads();
         if (tid == 0) issue_loads2(s_desc[0], 0);
         __syncthreads();      // the piece table of the first tile is visible
     } else {
-        if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+        if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + tile0)[tid];
         __syncthreads();
         issue_loads(pieces_of(s_desc[0]));
     }
     int par = 0;
-    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+    for (u32 tile = tile0; tile < ntiles; tile += gridDim.x, par ^= 1) {
         const u32 next = tile + gridDim.x;
         u64 dnext = 0;
         if constexpr (TWO) { if (tid < 16 && next < ntiles) dnext = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + next)[tid]; }

@@ -80,11 +80,12 @@ __global__ void __launch_bounds__(SV_THREADS, 3) grouppass_kernel(const u64* __r
     };
     if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
     u32 bar_phase = 0;
-    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+    const u32 tile0 = first_tile_of_block<!PRE>();
+    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + tile0)[tid];
     __syncthreads();
     issue_loads(pieces_of(s_desc[0]));
     int par = 0;
-    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+    for (u32 tile = tile0; tile < ntiles; tile += gridDim.x, par ^= 1) {
         const u32 next = tile + gridDim.x;
         u64 dnext = 0;
         if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid];

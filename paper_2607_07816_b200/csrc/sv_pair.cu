@@ -140,11 +140,12 @@ __global__ void __launch_bounds__(SV_THREADS, (MODE == 1 && BP_GEN_CTAS) ? (PRE 
     };
     if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
     u32 bar_phase = 0;
-    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + blockIdx.x)[tid];
+    const u32 tile0 = first_tile_of_block<(MODE == 1 && !FIXED && !PRE)>();
+    if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + tile0)[tid];
     __syncthreads();
     issue_loads(pieces_of(s_desc[0]), La0);
     int par = 0;
-    for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x, par ^= 1) {
+    for (u32 tile = tile0; tile < ntiles; tile += gridDim.x, par ^= 1) {
         double2* La = par ? La1 : La0;          // this tile's amplitudes (by landing slot)
         double2* Lnext = par ? La0 : La1;
         u64* Wk = par ? Wk1 : Wk0;
