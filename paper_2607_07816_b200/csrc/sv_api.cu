@@ -68,7 +68,7 @@ struct sv_state {
     bool diag_deferred;     // the diagonal gate in s->tab (and the pending cut) has not been applied yet: the truncation's
                             // classification pass applies it in place (sv_sample_select.cu, XF)
     bool small_on;          // SV_OPT_SMALL_STATE_PATH: sv_apply_circuit may use the single-block path (sv_small.cu)
-    bool two_bit_on;        // SV_OPT_TWO_BIT_PASS: the final pass of a dense multi-qubit gate may move two bits at once
+    int two_bit_min_ma;     // SV_OPT_TWO_BIT_PASS: the final pass of a dense gate with at least this many active qubits moves two bits at once (0: never)
     u64 small_gates;        // gates it has taken so far
     int circuit_done;       // gates the running / last sv_apply_circuit completed
     int small_backoff;      // gates still to take the streaming passes after a gate that did not fit the small path ...
@@ -263,7 +263,7 @@ static int create_common(int n_qubits, uint64_t capacity, void* arena, size_t ar
     s->seg_cnt = s->arena + L.seg_cnt;
     s->chunk_cnt = (u32*)(s->arena + L.chunk_cnt);
     s->small_on = true;
-    s->two_bit_on = false;
+    s->two_bit_min_ma = 3;
     s->sample_min_terms = 1ull << 21;   // below ~2^21 terms the state sits in L2 and the full select has fewer launches
     if (cudaMallocHost(&s->pinned, 1024) != cudaSuccess) { if (own) { cudaFree(arena); cudaStreamDestroy(s->stream); } delete s; return SV_ERR_NOMEM; }
     if (cudaMemsetAsync(s->hist, 0, 3 * SV_SEL_BINS * 8, s->stream) != cudaSuccess || init_state(s) != SV_OK) {
@@ -323,7 +323,7 @@ extern "C" int sv_set_option(sv_state* s, int option, uint64_t value) {
     if (!s) return SV_ERR_INVALID_ARG;
     if (option == SV_OPT_SAMPLE_MIN_TERMS) { s->sample_min_terms = value; return SV_OK; }
     if (option == SV_OPT_SMALL_STATE_PATH) { s->small_on = value != 0; return SV_OK; }
-    if (option == SV_OPT_TWO_BIT_PASS) { s->two_bit_on = value != 0; return SV_OK; }
+    if (option == SV_OPT_TWO_BIT_PASS) { s->two_bit_min_ma = value == 0 ? 0 : (value == 1 ? 2 : 3); return SV_OK; }
     return fail(s, SV_ERR_INVALID_ARG, "unknown option");
 }
 // test hook (include/sparse_sv_test.h): sample points added to the margin of the fused call's output floor
@@ -547,7 +547,7 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     // itself (a four-way merge per tile, sv_dense.cu TWO): one full pass over the state less.
     bool dense0 = (ma >= 2 && mc == 0);
     for (int i = 0; i < d * d && dense0; ++i) dense0 = !is_zero(U[i]);
-    const bool two = s->two_bit_on && dense0 && nneed >= 2;
+    const bool two = s->two_bit_min_ma != 0 && ma >= s->two_bit_min_ma && dense0 && nneed >= 2;
     for (int t = 0; t + (two ? 2 : 1) < nneed; ++t) {   // pure moves: state preserving, committed one by one
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;

@@ -108,50 +108,40 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     auto issue_loads = [&](const Pieces3& q) {
         if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
     };
-    // TWO, called by ONE thread: the tile between the boundaries w[0..6] and w[8..14] as contiguous pieces of the input -- the
-    // difference of two sets of four stored ranges each (TileDesc2) --, their table for the pick-up (s_pcum / s_pko[slot])
-    // and the bulk copies.  A key piece that starts at an odd index is fetched from the even index before it (sv_tile.cuh).
+    // TWO, called by ONE thread: w = the tile's entry of the piece table (make_pieces2 in sv_gate.cu: start index and length
+    // of its up to seven contiguous pieces of the input).  Fills the table the pick-up reads (s_pcum / s_pko[slot]) and
+    // issues the bulk copies.  A key piece that starts at an odd index is fetched from the even index before it (sv_tile.cuh).
     auto issue_loads2 = [&](const u64* w, int slot) {
-        const u64 as_[4] = {0, w[1], w[3], w[5]}, ae_[4] = {w[0], w[2], w[4], w[6]};
-        const u64 bs_[4] = {0, w[9], w[11], w[13]}, be_[4] = {w[8], w[10], w[12], w[14]};
         u64 ps[DP_MAXPIECES]; int pl[DP_MAXPIECES];
         int np = 0;
-        auto emit = [&](u64 a, u64 b) {
-            if (b <= a) return;
-            if (np > 0 && ps[np - 1] + (u64)pl[np - 1] == a) { pl[np - 1] += (int)(b - a); return; }
-            SV_CHK(np < DP_MAXPIECES);
-            if (np < DP_MAXPIECES) { ps[np] = a; pl[np] = (int)(b - a); ++np; }
-        };
-        for (int bi = 0; bi < 4; ++bi) {
-            u64 cur = bs_[bi];
-            const u64 be = be_[bi];
-            for (int ai = 0; ai < 4 && cur < be; ++ai) {
-                const u64 a0 = as_[ai], a1 = ae_[ai];
-                if (a1 <= a0 || a1 <= cur || a0 >= be) continue;
-                if (a0 > cur) emit(cur, a0);
-                cur = a1 < be ? a1 : be;
-            }
-            emit(cur, be);
+#pragma unroll
+        for (int q = 0; q < DP_MAXPIECES; ++q) {
+            ps[q] = w[q];
+            pl[q] = (int)(u32)(w[DP_MAXPIECES + q / 2] >> (32 * (q & 1)));
+            np += pl[q] ? 1 : 0;
         }
         int cum = 0, slots = 0;
         u32 bytes = 0;
-        for (int q = 0; q < np; ++q) {
-            const int o = (int)(ps[q] & 1ull), c = (pl[q] + o + 1) & ~1;
-            s_pcum[slot][q] = cum; s_pko[slot][q] = slots + o - cum;
+#pragma unroll
+        for (int q = 0; q < DP_MAXPIECES; ++q) {     // (unused pieces have length 0: they start where the tile ends)
+            const int o = (int)(ps[q] & 1ull), c = pl[q] ? ((pl[q] + o + 1) & ~1) : 0;
+            s_pcum[slot][q] = cum; s_pko[slot][q] = pl[q] ? (slots + o - cum) : 0;
             bytes += (u32)c * 8u + (u32)pl[q] * 16u;
             cum += pl[q]; slots += c;
         }
-        for (int q = np; q <= DP_MAXPIECES; ++q) s_pcum[slot][q] = cum;
-        for (int q = np; q < DP_MAXPIECES; ++q) s_pko[slot][q] = 0;
-        SV_CHK(cum <= BP_TILE && slots <= BP_TILE + LKX);
+        s_pcum[slot][DP_MAXPIECES] = cum;
+        SV_CHK(np <= DP_MAXPIECES && cum <= BP_TILE && slots <= BP_TILE + LKX);
         fence_proxy_async_smem();
         mbar_expect_tx(&s_bar, bytes);
         cum = 0; slots = 0;
-        for (int q = 0; q < np; ++q) {
-            const int o = (int)(ps[q] & 1ull), c = (pl[q] + o + 1) & ~1;
-            bulk_g2s(Lk + slots, kin + (ps[q] & ~1ull), (u32)c * 8u, &s_bar);
-            bulk_g2s(La + cum, ain + ps[q], (u32)pl[q] * 16u, &s_bar);
-            cum += pl[q]; slots += c;
+#pragma unroll
+        for (int q = 0; q < DP_MAXPIECES; ++q) {
+            if (pl[q]) {
+                const int o = (int)(ps[q] & 1ull), c = (pl[q] + o + 1) & ~1;
+                bulk_g2s(Lk + slots, kin + (ps[q] & ~1ull), (u32)c * 8u, &s_bar);
+                bulk_g2s(La + cum, ain + ps[q], (u32)pl[q] * 16u, &s_bar);
+                cum += pl[q]; slots += c;
+            }
         }
     };
     if (tid == 0) { mbar_init(&s_bar, 1); fence_proxy_async_smem(); }
@@ -176,7 +166,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
 
     const u32 tile0 = first_tile_of_block<!PRE>();
     if constexpr (TWO) {
-        if (tid < 16) s_desc[0][tid] = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + tile0)[tid];
+        if (tid < SV_PIECES2_WORDS) s_desc[0][tid] = (reinterpret_cast<const u64*>(desc) + (size_t)tile0 * SV_PIECES2_WORDS)[tid];
         __syncthreads();
         if (tid == 0) issue_loads2(s_desc[0], 0);
         __syncthreads();      // the piece table of the first tile is visible
@@ -189,7 +179,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     for (u32 tile = tile0; tile < ntiles; tile += gridDim.x, par ^= 1) {
         const u32 next = tile + gridDim.x;
         u64 dnext = 0;
-        if constexpr (TWO) { if (tid < 16 && next < ntiles) dnext = reinterpret_cast<const u64*>(reinterpret_cast<const TileDesc2*>(desc) + next)[tid]; }
+        if constexpr (TWO) { if (tid < SV_PIECES2_WORDS && next < ntiles) dnext = (reinterpret_cast<const u64*>(desc) + (size_t)next * SV_PIECES2_WORDS)[tid]; }
         else { if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid]; }
         Pieces3 pc;
         if constexpr (!TWO) pc = pieces_of(s_desc[par]); else { pc.cnt = s_pcum[par][DP_MAXPIECES]; pc.oneblock = false; pc.l0 = 0; }
@@ -200,6 +190,11 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             bar_phase ^= 1u;
             Landing3 ld;
             if constexpr (!TWO) ld = landing_of(pc);
+            int pcs[TWO ? DP_MAXPIECES : 1];          // TWO: first load-order index of pieces 1 .. 7
+            if constexpr (TWO) {
+#pragma unroll
+                for (int i = 1; i < DP_MAXPIECES; ++i) pcs[i] = s_pcum[par][i];
+            }
             u64 lk[BP_VT]; double2 la[BP_VT];
 #pragma unroll
             for (int r = 0; r < BP_VT; ++r) {
@@ -209,7 +204,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if constexpr (TWO) {
                         int q = 0;
 #pragma unroll
-                        for (int i = 1; i < DP_MAXPIECES; ++i) q += (e >= s_pcum[par][i]) ? 1 : 0;
+                        for (int i = 1; i < DP_MAXPIECES; ++i) q += (e >= pcs[i]) ? 1 : 0;
                         const int sl = e + s_pko[par][q];
                         SV_CHK(sl >= 0 && sl < BP_TILE + LKX);
                         lk[r] = Lk[sl];
@@ -227,7 +222,8 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 }
             }
             if constexpr (TWO) {
-                // the live entries by class (bH, bL), each class in load order = ascending rest; keys -> (high, mid, low, 0, 0)
+                // the live entries by class (bH, bL), each class in load order = ascending rest; keys -> (high, mid, low, bH, bL):
+                // with the two bits at the bottom a plain comparison orders both merges (equal rest: bL = 0, bH = 0 first)
                 u32 bal[4][BP_VT];
 #pragma unroll
                 for (int r = 0; r < BP_VT; ++r) {
@@ -261,7 +257,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     SV_CHK(slot < nL);
                     if (slot >= 0) {
                         const u64 k = lk[r];
-                        sk[DK(slot)] = (k & himask) | ((k & midmask) << 1) | ((k & lowmask2) << 2);
+                        sk[DK(slot)] = (k & himask) | ((k & midmask) << 1) | ((k & lowmask2) << 2) | ((k & bit) ? 2ull : 0ull) | ((k & bit2) ? 1ull : 0ull);
                         sa[DA(slot)] = la[r];
                     }
                 }
@@ -304,7 +300,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 }
             }
         }
-        if (tid < (TWO ? 16 : 8) && next < ntiles) s_desc[par ^ 1][tid] = dnext;
+        if (tid < (TWO ? SV_PIECES2_WORDS : 8) && next < ntiles) s_desc[par ^ 1][tid] = dnext;
         __syncthreads();
         if constexpr (TWO) { if (next < ntiles && tid == 0) issue_loads2(s_desc[par ^ 1], par ^ 1); }
         else { if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1])); }
@@ -338,7 +334,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                         ka = (0 < na) ? sk[DK(ob)] : ~0ull; kb = (0 < nb) ? sk[DK(ob + na)] : ~0ull;
                     }
                     const bool takeA = ka <= kb;
-                    mk[v] = (takeA ? ka : kb) | (takeA ? 0ull : 1ull);
+                    mk[v] = takeA ? ka : kb;
                     ma_[v] = sa[DA(takeA ? ob + i : ob + na + j)];
                     if (takeA) { ++i; ka = (i < na) ? sk[DK(ob + i)] : ~0ull; } else { ++j; kb = (j < nb) ? sk[DK(ob + na + j)] : ~0ull; }
                 }
@@ -357,10 +353,9 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             int i, j;
             {
                 int lo = max(0, diag - nB), hi = min(diag, nA);
-                while (lo < hi) {   // A first on ties (TWO: bit 0 holds bL, not part of the comparison)
+                while (lo < hi) {   // A first on ties
                     const int mid = (lo + hi) >> 1;
-                    const u64 xa = sk[DK(mid)], xb = sk[DK(nA + diag - 1 - mid)];
-                    if (TWO ? ((xa | 1ull) <= (xb | 1ull)) : (xa <= xb)) lo = mid + 1; else hi = mid;
+                    if (sk[DK(mid)] <= sk[DK(nA + diag - 1 - mid)]) lo = mid + 1; else hi = mid;
                 }
                 i = lo; j = diag - lo;
             }
@@ -372,10 +367,10 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             for (int v = 0; v < BP_VT; ++v) {
                 mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
                 if (diag + v < endpos) {
-                    const bool takeA = TWO ? ((ka | 1ull) <= (kb | 1ull)) : (ka <= kb);
+                    const bool takeA = ka <= kb;
                     const u64 k = takeA ? ka : kb;
                     ma_[v] = sa[DA(takeA ? i : nA + j)];
-                    mk[v] = TWO ? (k | (takeA ? 0ull : 2ull)) : ((k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull));
+                    mk[v] = TWO ? k : ((k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull));
                     if (takeA) { ++i; ka = (i < nA) ? sk[DK(i)] : ~0ull; } else { ++j; kb = (j < nB) ? sk[DK(nA + j)] : ~0ull; }
                 }
             }

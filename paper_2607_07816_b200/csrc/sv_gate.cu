@@ -321,34 +321,42 @@ __device__ __forceinline__ void multi_lower_bound(const u64* __restrict__ keys, 
 __global__ void find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles,
                                     TileDesc2* __restrict__ desc) {
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j > ntiles) return;
     TileDesc2 d;
     d.pad_ = 0;
     const u64 T = (u64)j * tnom;
-    if (j == ntiles || T >= n) { d.p00 = d.m2a = d.p01 = d.m1 = d.p10 = d.m2b = d.p11 = n; desc[j] = d; return; }
+    // (no early return: the boundaries of a warp that fall into the same block / sub-blocks share those searches)
+    const bool real = j < ntiles && T < n;
+    const int lane = threadIdx.x & 31;
+    if (!real && j <= ntiles) { d.p00 = d.m2a = d.p01 = d.m1 = d.p10 = d.m2b = d.p11 = n; desc[j] = d; }
     const u64 bitH = 1ull << pH, bitL = 1ull << pL;             // pL < pH <= 63
     const u64 maskH = (pH == 63) ? 0ull : ~((2ull << pH) - 1);
     const u64 maskL = bitL - 1;
     const u64 maskM = (bitH - 1) & ~((2ull << pL) - 1);
-    const u64 kt = keys[T];
+    const u64 kt = real ? keys[T] : 0;
     const u64 hb = kt & maskH;
-    // (1) the block of keys that agree above pH
+    // (1) the block of keys that agree above pH.  Only the first lane of every block searches (its brackets, taken from its own
+    // T, hold for the block as a whole: s1 <= T', mid1 and e1 anywhere), the others take its result.
     u64 s1, mid1, e1;
     {
+        const unsigned peers = __match_any_sync(0xffffffffu, real ? hb : (~0ull - (u64)lane));
+        const int leader = __ffs(peers) - 1;
+        const bool searching = real && lane == leader;
         const u64 nxt = hb + (bitH << 1);                        // pH == 63: 0
         const bool has_e = (pH < 63) && nxt != 0;                // nxt == 0: wrapped, last block
         const bool inB = (kt & bitH) != 0;
         u64 lo[3] = {0, inB ? 0 : T + 1, has_e ? T + 1 : n};
         u64 hi[3] = {(pH == 63) ? 0 : T, inB ? T : n, n};
+        if (!searching) { hi[0] = lo[0]; hi[1] = lo[1]; hi[2] = lo[2]; }
         const u64 v[3] = {hb, hb | bitH, nxt};
         const u64 hint[3] = {T, T, T + 1};
         multi_lower_bound<3>(keys, lo, hi, v, hint);
-        s1 = lo[0]; mid1 = lo[1]; e1 = lo[2];
+        s1 = __shfl_sync(0xffffffffu, lo[0], leader); mid1 = __shfl_sync(0xffffffffu, lo[1], leader); e1 = __shfl_sync(0xffffffffu, lo[2], leader);
     }
+    if (!real) { s1 = 0; mid1 = 0; e1 = 0; }                     // (idle lanes keep taking part in the shuffles below)
     // (2) co-rank on the mid bits (the bH = 0 half first on ties): the mid value of rank diag inside the block
-    const u64 lenA = mid1 - s1, lenB = e1 - mid1, diag = T - s1;
-    u64 ia, jb, m;
-    {
+    const u64 lenA = mid1 - s1, lenB = e1 - mid1, diag = real ? T - s1 : 0;
+    u64 ia = 0, jb = 0, m = 0;
+    if (real) {
         u64 lo = diag > lenB ? diag - lenB : 0, hi = diag < lenA ? diag : lenA;
         while (lo < hi) {
             const u64 i = lo + ((hi - lo) >> 1);
@@ -362,17 +370,27 @@ __global__ void find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH,
     }
     // (3) the sub-blocks (h, 0, m) and (h, 1, m): start, start of the bL = 1 run, end
     u64 st[4], en[4];
-    {
+    {   // (shared by the boundaries of the warp that fall into the same pair of sub-blocks, as in (1))
         const u64 b0 = hb | m, b1 = b0 | bitH;
+        const unsigned peers = __match_any_sync(0xffffffffu, real ? b0 : (~0ull - (u64)lane));
+        const int leader = __ffs(peers) - 1;
+        const bool searching = real && lane == leader;
         u64 lo[6] = {s1, s1, s1, mid1, mid1, mid1};
         u64 hi[6] = {mid1, mid1, mid1, e1, e1, e1};
         const u64 v[6] = {b0, b0 | bitL, b0 + (bitL << 1), b1, b1 | bitL, b1 + (bitL << 1)};
         if (v[5] < b1) lo[5] = hi[5];                            // wrapped: the sub-block ends with the half
+        if (!searching) {
+#pragma unroll
+            for (int k = 0; k < 6; ++k) hi[k] = lo[k];
+        }
         const u64 hint[6] = {s1 + ia, s1 + ia, s1 + ia, mid1 + jb, mid1 + jb, mid1 + jb};
         multi_lower_bound<6>(keys, lo, hi, v, hint);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) lo[k] = __shfl_sync(0xffffffffu, lo[k], leader);
         st[0] = lo[0]; en[0] = lo[1]; st[1] = lo[1]; en[1] = lo[2];
         st[2] = lo[3]; en[2] = lo[4]; st[3] = lo[4]; en[3] = lo[5];
     }
+    if (!real) return;
     const u64 diag2 = diag - (st[0] - s1) - (st[2] - mid1);      // rank among the entries of the two sub-blocks, by low
     // (4) the low value of that rank among the four runs
     u64 x[4] = {st[0], st[1], st[2], st[3]};
@@ -459,8 +477,56 @@ __global__ void find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH,
     desc[j] = d;
 }
 
+// The tile between boundaries j and j + 1 as contiguous pieces of the input: the difference of two sets of four stored
+// ranges each (TileDesc2), at most seven pieces.  One thread per tile; the pass reads the table one tile ahead and only
+// has to issue the copies.  Entry (12 words): start index of pieces 0..7, then their lengths (32 bits each; 0 = no piece).
+__global__ void make_pieces2_kernel(const TileDesc2* __restrict__ desc, u32 ntiles, u64* __restrict__ table) {
+    const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= ntiles) return;
+    const TileDesc2 d0 = desc[j], d1 = desc[j + 1];
+    const u64 as_[4] = {0, d0.m2a, d0.m1, d0.m2b}, ae_[4] = {d0.p00, d0.p01, d0.p10, d0.p11};
+    const u64 bs_[4] = {0, d1.m2a, d1.m1, d1.m2b}, be_[4] = {d1.p00, d1.p01, d1.p10, d1.p11};
+    u64 ps[SV_PIECES2];
+    u32 pl[SV_PIECES2];
+#pragma unroll
+    for (int q = 0; q < SV_PIECES2; ++q) { ps[q] = 0; pl[q] = 0; }
+    int np = 0;
+    u64 last_end = ~0ull;
+#pragma unroll
+    for (int bi = 0; bi < 4; ++bi) {
+        u64 cur = bs_[bi];
+        const u64 be = be_[bi];
+#pragma unroll
+        for (int ai = 0; ai <= 4; ++ai) {
+            // the part of [cur, be) before range ai of the earlier boundary (ai == 4: what is left)
+            u64 a0 = be, a1 = be;
+            if (ai < 4) { a0 = as_[ai]; a1 = ae_[ai]; if (a1 <= a0 || a1 <= cur || a0 >= be) continue; }
+            const u64 e = a0 < be ? a0 : be;
+            if (e > cur) {
+                if (last_end == cur) {            // contiguous with the previous piece
+#pragma unroll
+                    for (int q = 0; q < SV_PIECES2; ++q) if (q == np - 1) pl[q] += (u32)(e - cur);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < SV_PIECES2; ++q) if (q == np) { ps[q] = cur; pl[q] = (u32)(e - cur); }
+                    ++np;
+                }
+                last_end = e;
+            }
+            if (ai < 4) { const u64 nx = a1 < be ? a1 : be; if (nx > cur) cur = nx; }
+        }
+    }
+    SV_CHK(np <= SV_PIECES2);
+    u64* t = table + (size_t)j * SV_PIECES2_WORDS;
+#pragma unroll
+    for (int q = 0; q < SV_PIECES2; ++q) t[q] = ps[q];
+#pragma unroll
+    for (int q = 0; q < SV_PIECES2; q += 2) t[SV_PIECES2 + q / 2] = (u64)pl[q] | ((u64)pl[q + 1] << 32);
+}
+
 int svk_find_splits2(const u64* keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles, TileDesc2* desc, cudaStream_t st) {
     const u32 nb = (ntiles + 1 + 127) / 128;
     find_splits2_kernel<<<nb, 128, 0, st>>>(keys, n, pH, pL, w, tnom, ntiles, desc);
-    return 1;
+    make_pieces2_kernel<<<(ntiles + 127) / 128, 128, 0, st>>>(desc, ntiles, reinterpret_cast<u64*>(desc + ntiles + 1));
+    return 2;
 }

@@ -391,7 +391,9 @@ int svk_grouppass(const u64* kin, const double2* ain, u64* kout, double2* aout, 
     else { find_starts_kernel<<<(ntiles + 1 + 127) / 128, 128, 0, st>>>(kin, n, ma, tnom, ntiles, desc); launches += 1; }
     if (e0) cudaEventRecord(e0, st);
     if (dense && ma >= 2 && ma <= 4) {   // every entry of U nonzero, no control-like bit: sv_dense.cu
-        const u32 g = svk_densepass_launch(ma, pre != nullptr, kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st,
+        // (two bits: the pass reads the piece table that follows the ntiles + 1 boundaries)
+        TileDesc* dd = two ? reinterpret_cast<TileDesc*>(reinterpret_cast<TileDesc2*>(desc) + ntiles + 1) : desc;
+        const u32 g = svk_densepass_launch(ma, pre != nullptr, kin, ain, kout, aout, p, tab, pend, dd, status, d_count, cap, ntiles, st,
                                            pre, pre_mass, pre_cnt, maybe_dead, two ? p2 : -1);
         if (pre && pre_parts) *pre_parts = g;
     } else if (pre) {

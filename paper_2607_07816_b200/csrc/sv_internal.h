@@ -38,6 +38,11 @@ struct TileDesc {
 struct TileDesc2 {
     u64 p00, m2a, p01, m1, p10, m2b, p11, pad_;
 };
+// ... and the tile between two boundaries as contiguous pieces of the input (make_pieces2 in sv_gate.cu): the table
+// follows the ntiles + 1 boundaries in the descriptor area; per tile the start indices of pieces 0 .. 7, then their
+// lengths, 32 bits each (0: no piece; the pieces are in stored order and not empty).
+#define SV_PIECES2 8
+#define SV_PIECES2_WORDS 12
 
 // Radix-select state (device resident; one per handle).  See sv_radix_select.cu.
 struct SelState {
@@ -158,7 +163,8 @@ int svk_pre_sample_group(const u64* keys, const double2* amps, u64 n, int p, int
 int svk_pre_pivot(const u64* smp_sorted, u32 M, u64 n, u32 mult, u64 max_terms, long long slack, PreCut* pre, cudaStream_t st);
 int svk_pre_finish(const double* part_mass, const u64* part_cnt, u32 nparts, PreCut* pre, u64* d_count, cudaStream_t st);
 int svk_find_splits(const u64* keys, u64 n, int p, int w, u32 tnom, u32 ntiles, TileDesc* desc, cudaStream_t st);
-// boundaries of a two-bit pass: bits pH > pL; w low bits of the key belong to the tuple (boundaries are aligned to it)
+// boundaries of a two-bit pass: bits pH > pL; w low bits of the key belong to the tuple (boundaries are aligned to it);
+// desc[0 .. ntiles] and, behind them, the piece table of the ntiles tiles
 int svk_find_splits2(const u64* keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles, TileDesc2* desc, cudaStream_t st);
 // Diagonal gate fused with a pending truncation (out of place, compacting).
 int svk_diag_compact(const u64* kin, const double2* ain, u64* kout, double2* aout, u64 n, const GateTab* tab,
