@@ -171,3 +171,55 @@ def test_two_bit_pass_with_pending_cut_and_fused_call(eng):
         assert_truncation_parity(sv.export()[:2], o.export()[:2])
         assert sv.check_invariants()
     assert used_two >= 3
+
+
+def test_two_bit_option_values_and_pass_counts(eng):
+    """SV_OPT_TWO_BIT_PASS: 0 = one pass per missing qubit, 1 = two-bit final pass for every dense gate, 2 (the default) =
+    for dense gates on three or four mixing qubits only.  Same bits in every mode."""
+    rng = np.random.default_rng(7001)
+    n = 30
+    keys, amps = W.random_state(rng, n, 20000)
+    gates = [([25, 11], W.haar_unitary(rng, 4)), ([29, 3, 17], W.haar_unitary(rng, 8)), ([8, 21, 14, 27], W.haar_unitary(rng, 16))]
+    want = {0: [2, 3, 4], 1: [1, 2, 3], 2: [2, 2, 3], None: [2, 2, 3]}
+    ref = None
+    for mode, passes in want.items():
+        sv = eng.SparseSV(n, 1 << 22)
+        if mode is not None:
+            sv.set_option(eng.OPT_TWO_BIT_PASS, mode)
+        out = []
+        for (qs, U), p in zip(gates, passes):
+            sv.load(keys, amps)
+            sv.apply_gate(qs, U)
+            assert sv.stats()["passes"] == p, (mode, qs, sv.stats()["passes"])
+            k, a, _ = sv.export()
+            out.append((k, a))
+        if ref is None:
+            ref = out
+        for (k, a), (k0, a0) in zip(out, ref):
+            assert np.array_equal(k, k0) and np.array_equal(a.view(np.uint64), a0.view(np.uint64))
+
+
+def test_definite_qubits_hook(eng):
+    """sv_test_definite_qubits (include/sparse_sv_test.h): the qubits with one value over the whole state, through the lazy
+    layout (an X only flips the mask), a gate that spreads one of them, and a pending truncation that removes the spread."""
+    rng = np.random.default_rng(7002)
+    n = 20
+    free = [0, 2, 5, 7, 8, 11, 13, 16]
+    const = (1 << 3) | (1 << 19)                       # qubits 3 and 19 are 1, the other non-free ones 0
+    idx = np.arange(1 << len(free), dtype=np.uint64)
+    keys = np.full(idx.size, const, dtype=np.uint64)
+    for j, b in enumerate(free):
+        keys |= ((idx >> np.uint64(j)) & np.uint64(1)) << np.uint64(b)
+    amps = (rng.standard_normal(keys.size) + 1j * rng.standard_normal(keys.size)).astype(np.complex128)
+    amps /= np.sqrt(np.sum(np.abs(amps) ** 2))
+    sv = eng.SparseSV(n, 1 << 12)
+    sv.load(keys, amps)
+    definite = sum(1 << q for q in range(n) if q not in free)
+    assert sv.test_definite_qubits() == definite
+    sv.apply_gate([19], W.mat_x())                     # lazy: still definite (now 0)
+    sv.apply_gate([3, 0], W.mat_mcx(2))                # CNOT 3 -> 0: qubit 0 stays spread, qubit 3 stays definite
+    assert sv.test_definite_qubits() == definite
+    sv.apply_gate([4], W.mat_rx(0.02))                 # qubit 4 is spread, weakly: |1> carries sin^2(0.01) of the mass
+    assert sv.test_definite_qubits() == definite & ~(1 << 4)
+    sv.truncate(0, 0.999)                              # the cut (pending) drops the weak branch again
+    assert sv.test_definite_qubits() == definite
