@@ -1,7 +1,7 @@
 // Final pass of a DENSE gate with MA >= 2 active bits -- every entry of U nonzero, no control-like bit (Haar SU(4),
 // Haar 8x8, 16x16, fused blocks): SURVEY.md rows a-4 .. a-7.
 //
-// Front end as in sv_group.cu (persistent blocks, the next tile landing through cp.async, A* | B* partition, one
+// Front end as in sv_group.cu (persistent blocks, the next tile landing by bulk copies, A* | B* partition, one
 // merge-path split per thread, the tile left in shared memory in its NEW order where the members of a tuple --
 // the terms that differ only in the gate's qubits -- are neighbours), except that dead entries and the
 // terms a pending truncation drops are squeezed out while the tile is partitioned: behind the front end every
@@ -12,9 +12,9 @@
 // index, every operation rounded separately: DESIGN.md D1): the tuple's members are read once, U comes from shared memory
 // with the lanes of a warp spread over its columns (conflict free), and a round of 256 * TPR tuples costs no per-candidate
 // bookkeeping.
-//   two calls (PRE = false): the tile's output count is known before any arithmetic; every warp transposes its round
-//     through 4 KB of swizzled shared memory so that consecutive lanes store consecutive entries (an exact cancellation
-//     is written as a counted dead entry); the look-back resolves behind the first round's arithmetic.
+//   two calls (PRE = false): the tile's output count is known before any arithmetic; a thread's 2^MA rows are consecutive
+//     outputs and go out straight from registers with 256-bit stores (an exact cancellation is written as a counted dead
+//     entry); the look-back resolves behind the first round's arithmetic.
 //   fused apply + truncate (PRE = true): every candidate is computed ONCE, tested against the floor of the cut that
 //     follows (sv_presample.cu); survivors are ranked by warp scans + one block scan per round and staged in output
 //     order in shared memory; the tile's total is published when its last round is done and the staged outputs stay
@@ -28,7 +28,6 @@
 #ifndef DP_NOPRE_BLOCKS
 #define DP_NOPRE_BLOCKS 4                  // resident blocks per SM of the two-call variant (ma <= 3): 64 registers, ~51 KB of shared memory
 #endif
-#define DP_WENT 128                        // !PRE: entries of a warp's transposition buffer
 // The tile arrays (keys sk, amplitudes sa) are addressed through an XOR swizzle of the entry index with its 128-byte row
 // (16 keys / 8 amplitudes per row), as the staging arrays of sv_pair.cu: threads that own a few CONSECUTIVE entries each
 // (the merges write 4 per thread, read ~2 apart per lane) would otherwise hit the same banks 4 to 16 ways -- measured: a

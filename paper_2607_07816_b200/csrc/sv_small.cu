@@ -29,10 +29,15 @@
 
 // bitonic sort of P (power of two) entries by (k1, k2) ascending with payload idx; entries with idx == 0xffff are pads
 // and sort last.  TWO: compare k2 on equal k1.
+// Pair t of a stage with distance j <= 32 lies inside the 64-entry chunk t / 32: a warp (32 consecutive t per iteration,
+// the same t in every stage) then reads only what it wrote itself in the previous stage, so stages with j <= 32 that also
+// FOLLOW a stage with j <= 32 are separated by __syncwarp(); only the stages with j >= 64 (10 of the 55 of a 1024-entry
+// sort) are bracketed by block barriers.  The sort ends with a block barrier.
 template <bool TWO>
 __device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, int P, int A) {
     for (int k = 2; k <= P; k <<= 1) {
         for (int j = k >> 1; j > 0; j >>= 1) {
+            const int next_j = (j > 1) ? (j >> 1) : ((2 * k <= P) ? k : 1 << 30);   // distance of the stage that follows (none: block barrier)
             for (int t = threadIdx.x; t < (P >> 1); t += A) {
                 const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
                 const int l = i | j;
@@ -51,7 +56,7 @@ __device__ __forceinline__ void bitonic(u64* k1, u64* k2, unsigned short* idx, i
                     if (TWO) { k2[i] = b2; k2[l] = a2; }
                 }
             }
-            __syncthreads();
+            if (j > 32 || next_j > 32) __syncthreads(); else __syncwarp();
         }
     }
 }
