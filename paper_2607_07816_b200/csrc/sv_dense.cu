@@ -28,12 +28,12 @@
 #ifndef DP_NOPRE_BLOCKS
 #define DP_NOPRE_BLOCKS 4                  // resident blocks per SM of the two-call variant (ma <= 3): 64 registers, ~51 KB of shared memory
 #endif
-// The tile arrays (keys sk, amplitudes sa) are addressed through an XOR swizzle of the entry index with its 128-byte row
-// (16 keys / 8 amplitudes per row), as the staging arrays of sv_pair.cu: threads that own a few CONSECUTIVE entries each
-// (the merges write 4 per thread, read ~2 apart per lane) would otherwise hit the same banks 4 to 16 ways -- measured: a
-// third of the kernel's shared-memory wavefronts were such replays and the shared-memory pipe its busiest unit (72 %).
+// The tile's key array sk is addressed through an XOR swizzle of the entry index with its 128-byte row (16 keys per row), as
+// the staging arrays of sv_pair.cu: threads that own a few CONSECUTIVE entries each (the merges write 4 per thread, read ~2
+// apart per lane) would otherwise hit the same banks 4 to 8 ways -- measured: a third of the kernel's shared-memory wavefronts
+// were such replays and the shared-memory pipe its busiest unit (72 %).
 #define DK(x) ((x) ^ (((x) >> 4) & 15))
-#define DA(x) ((x) ^ (((x) >> 3) & 7))
+
 #ifndef DP_STAGE
 #define DP_STAGE 2048                      // PRE: staged survivors per tile (about twice the mean at the cap)
 #endif
@@ -57,12 +57,16 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     constexpr u64 AM = (u64)NP - 1;
     constexpr int TPR = NP >= 8 ? 1 : 8 / NP;   // tuples per thread and round
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double2* La = reinterpret_cast<double2*>(smem_raw);        // landing buffer (next tile)
-    double2* sa = La + BP_TILE;                                // the tile: partitioned, then in its new order
-    u64* Lk = reinterpret_cast<u64*>(sa + BP_TILE);
+    // Amplitudes never move inside shared memory: a tile's amplitudes stay where the bulk copies put them (two landing
+    // buffers used in turns, the next tile landing in the other one) and the partition and the merges move (key, 16-bit
+    // landing index) pairs only; the tuple arithmetic reads each amplitude once, by its index.
+    double2* La0 = reinterpret_cast<double2*>(smem_raw);
+    double2* La1 = La0 + BP_TILE;
+    u64* Lk = reinterpret_cast<u64*>(La1 + BP_TILE);
     u64* sk = Lk + BP_TILE + LKX;
     unsigned short* tst = reinterpret_cast<unsigned short*>(sk + BP_TILE);   // first member of every tuple (+ sentinel)
-    double2* stg_a = reinterpret_cast<double2*>(tst + BP_TILE + 8);          // PRE only: staged survivors, output order
+    unsigned short* si = tst + BP_TILE + 8;                                  // landing index of the entry whose key sits in sk (same slot, unswizzled)
+    double2* stg_a = reinterpret_cast<double2*>(si + BP_TILE);               // PRE only: staged survivors, output order
     u64* stg_k = reinterpret_cast<u64*>(stg_a + DP_STAGE);
     __shared__ int wcA[BP_VT][BP_WARPS], wcB[BP_VT][BP_WARPS];
     __shared__ int s_nA, s_nB, s_nt;
@@ -104,13 +108,13 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     u32 pk_tile = 0; int pk_total = 0;
 
     // The tile lands by bulk copies (TMA): one thread arms the barrier and issues up to six copies (sv_tile.cuh).
-    auto issue_loads = [&](const Pieces3& q) {
+    auto issue_loads = [&](const Pieces3& q, double2* La) {
         if (tid == 0) land_tile_bulk(q, kin, ain, Lk, La, &s_bar);
     };
     // TWO, called by ONE thread: w = the tile's entry of the piece table (make_pieces2 in sv_gate.cu: start index and length
     // of its up to seven contiguous pieces of the input).  Fills the table the pick-up reads (s_pcum / s_pko[slot]) and
     // issues the bulk copies.  A key piece that starts at an odd index is fetched from the even index before it (sv_tile.cuh).
-    auto issue_loads2 = [&](const u64* w, int slot) {
+    auto issue_loads2 = [&](const u64* w, int slot, double2* La) {
         u64 ps[DP_MAXPIECES]; int pl[DP_MAXPIECES];
         int np = 0;
 #pragma unroll
@@ -167,16 +171,17 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
     if constexpr (TWO) {
         if (tid < SV_PIECES2_WORDS) s_desc[0][tid] = (reinterpret_cast<const u64*>(desc) + (size_t)tile0 * SV_PIECES2_WORDS)[tid];
         __syncthreads();
-        if (tid == 0) issue_loads2(s_desc[0], 0);
+        if (tid == 0) issue_loads2(s_desc[0], 0, La0);
         __syncthreads();      // the piece table of the first tile is visible
     } else {
         if (tid < 8) s_desc[0][tid] = reinterpret_cast<const u64*>(desc + tile0)[tid];
         __syncthreads();
-        issue_loads(pieces_of(s_desc[0]));
+        issue_loads(pieces_of(s_desc[0]), La0);
     }
     int par = 0;
     for (u32 tile = tile0; tile < ntiles; tile += gridDim.x, par ^= 1) {
         const u32 next = tile + gridDim.x;
+        double2* La = par ? La1 : La0;     // this tile's amplitudes, by landing index
         u64 dnext = 0;
         if constexpr (TWO) { if (tid < SV_PIECES2_WORDS && next < ntiles) dnext = (reinterpret_cast<const u64*>(desc) + (size_t)next * SV_PIECES2_WORDS)[tid]; }
         else { if (tid < 8 && next < ntiles) dnext = reinterpret_cast<const u64*>(desc + next)[tid]; }
@@ -211,12 +216,14 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     la[r] = La[e];
                 }
             }
-            if (pd.active) {
+            if (pd.active) {   // (survivors are rescaled in place; what the cut drops is not given a slot below)
 #pragma unroll
                 for (int r = 0; r < BP_VT; ++r) {
                     if (tid + r * SV_THREADS < cnt) {
-                        if (pend_keep(pd, lk[r], la[r])) { la[r].x = __dmul_rn(la[r].x, pd.scale); la[r].y = __dmul_rn(la[r].y, pd.scale); }
-                        else { la[r].x = 0.0; la[r].y = 0.0; }
+                        if (pend_keep(pd, lk[r], la[r])) {
+                            la[r].x = __dmul_rn(la[r].x, pd.scale); la[r].y = __dmul_rn(la[r].y, pd.scale);
+                            La[tid + r * SV_THREADS] = la[r];
+                        } else { la[r].x = 0.0; la[r].y = 0.0; }
                     }
                 }
             }
@@ -257,7 +264,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if (slot >= 0) {
                         const u64 k = lk[r];
                         sk[DK(slot)] = (k & himask) | ((k & midmask) << 1) | ((k & lowmask2) << 2) | ((k & bit) ? 2ull : 0ull) | ((k & bit2) ? 1ull : 0ull);
-                        sa[DA(slot)] = la[r];
+                        si[slot] = (unsigned short)(tid + r * SV_THREADS);
                     }
                 }
             } else if (!maybe_dead && (!mv || pc.oneblock)) {   // load order = A* | B* already and nothing to squeeze out
@@ -265,7 +272,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
 #pragma unroll
                 for (int r = 0; r < BP_VT; ++r) {
                     const int e = tid + r * SV_THREADS;
-                    if (e < cnt) { sk[DK(e)] = lk[r] & ~bit; sa[DA(e)] = la[r]; }
+                    if (e < cnt) { sk[DK(e)] = lk[r] & ~bit; si[e] = (unsigned short)e; }
                 }
             } else {
                 u32 balA[BP_VT], balB[BP_VT];
@@ -295,14 +302,14 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if ((balA[r] >> lane) & 1u) slot = wcA[r][warp] + __popc(balA[r] & lt);
                     else if ((balB[r] >> lane) & 1u) slot = nA + wcB[r][warp] + __popc(balB[r] & lt);
                     SV_CHK(slot < nL);
-                    if (slot >= 0) { sk[DK(slot)] = lk[r] & ~bit; sa[DA(slot)] = la[r]; }
+                    if (slot >= 0) { sk[DK(slot)] = lk[r] & ~bit; si[slot] = (unsigned short)(tid + r * SV_THREADS); }
                 }
             }
         }
         if (tid < (TWO ? SV_PIECES2_WORDS : 8) && next < ntiles) s_desc[par ^ 1][tid] = dnext;
         __syncthreads();
-        if constexpr (TWO) { if (next < ntiles && tid == 0) issue_loads2(s_desc[par ^ 1], par ^ 1); }
-        else { if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1])); }
+        if constexpr (TWO) { if (next < ntiles && tid == 0) issue_loads2(s_desc[par ^ 1], par ^ 1, par ? La0 : La1); }
+        else { if (next < ntiles) issue_loads(pieces_of(s_desc[par ^ 1]), par ? La0 : La1); }
 
         // ---- TWO, level 1: inside either bH class, merge its bL = 0 and bL = 1 entries by the rest of the key (two merges
         // side by side over the output positions [0, nA) and [nA, nL)); bL goes to bit 0 ----
@@ -323,10 +330,10 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 i = lo; j = dg - lo;
             }
             u64 ka = (i < na) ? sk[DK(ob + i)] : ~0ull, kb = (j < nb) ? sk[DK(ob + na + j)] : ~0ull;
-            u64 mk[BP_VT]; double2 ma_[BP_VT];
+            u64 mk[BP_VT]; unsigned short mi[BP_VT];
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v) {
-                mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
+                mk[v] = 0; mi[v] = 0;
                 if (d0 + v < nL) {
                     if (seg == 0 && d0 + v == nA) {   // this thread's outputs run over into the bH = 1 merge: it starts there
                         seg = 1; ob = nA; na = n10; nb = nL - nA - n10; i = 0; j = 0;
@@ -334,14 +341,14 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     }
                     const bool takeA = ka <= kb;
                     mk[v] = takeA ? ka : kb;
-                    ma_[v] = sa[DA(takeA ? ob + i : ob + na + j)];
+                    mi[v] = si[takeA ? ob + i : ob + na + j];
                     if (takeA) { ++i; ka = (i < na) ? sk[DK(ob + i)] : ~0ull; } else { ++j; kb = (j < nb) ? sk[DK(ob + na + j)] : ~0ull; }
                 }
             }
             __syncthreads();   // every read of the partitioned tile is done
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v)
-                if (d0 + v < nL) { sk[DK(d0 + v)] = mk[v]; sa[DA(d0 + v)] = ma_[v]; }
+                if (d0 + v < nL) { sk[DK(d0 + v)] = mk[v]; si[d0 + v] = mi[v]; }
             __syncthreads();
         }
 
@@ -361,14 +368,14 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
             SV_CHK(i >= 0 && i <= nA && j >= 0 && j <= nB);
             const int endpos = min(diag + BP_VT, nL);
             u64 ka = (i < nA) ? sk[DK(i)] : ~0ull, kb = (j < nB) ? sk[DK(nA + j)] : ~0ull;
-            u64 mk[BP_VT]; double2 ma_[BP_VT];
+            u64 mk[BP_VT]; unsigned short mi[BP_VT];
 #pragma unroll
             for (int v = 0; v < BP_VT; ++v) {
-                mk[v] = 0; ma_[v] = make_double2(0.0, 0.0);
+                mk[v] = 0; mi[v] = 0;
                 if (diag + v < endpos) {
                     const bool takeA = ka <= kb;
                     const u64 k = takeA ? ka : kb;
-                    ma_[v] = sa[DA(takeA ? i : nA + j)];
+                    mi[v] = si[takeA ? i : nA + j];
                     mk[v] = TWO ? k : ((k & himask) | ((k & lowmask) << 1) | (takeA ? 0ull : 1ull));
                     if (takeA) { ++i; ka = (i < nA) ? sk[DK(i)] : ~0ull; } else { ++j; kb = (j < nB) ? sk[DK(nA + j)] : ~0ull; }
                 }
@@ -390,7 +397,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                 if (diag + v < endpos) {
                     const u64 before = v == 0 ? prev : mk[v - 1];
                     if ((diag + v == 0) || (before >> MA) != (mk[v] >> MA)) om |= 1u << v;
-                    sk[DK(diag + v)] = mk[v]; sa[DA(diag + v)] = ma_[v];
+                    sk[DK(diag + v)] = mk[v]; si[diag + v] = mi[v];
                 }
             }
             int cinc = __popc(om);
@@ -462,7 +469,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if (col_ident || nm <= 2) {          // members in stored order = ascending logical column (or the order cannot matter)
                         for (int j = 0; j < nm; ++j) {
                             const int x = (int)(sk[DK(e + j)] & AM);
-                            const double2 a = sa[DA(e + j)];
+                            const double2 a = La[si[e + j]];
 #pragma unroll
                             for (int r = 0; r < NP; ++r) {
                                 const double2 uu = Us[r * NP + x];
@@ -475,7 +482,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                         for (int t = 0; t < NP; ++t) {
                             const int x = (int)((colpack >> (4 * t)) & 15ull);
                             if ((pk >> x) & 1u) {
-                                const double2 a = sa[DA(e + __popc(pk & ((1u << x) - 1u)))];
+                                const double2 a = La[si[e + __popc(pk & ((1u << x) - 1u))]];
 #pragma unroll
                                 for (int r = 0; r < NP; ++r) {
                                     const double2 uu = Us[r * NP + x];
@@ -636,7 +643,7 @@ template <int MA, bool PRE, bool TWO>
 static u32 launch_densepass(const u64* kin, const double2* ain, u64* kout, double2* aout, int p, const GateTab* tab,
                             const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                             const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2) {
-    const size_t smem = (size_t)2 * BP_TILE * 24 + (TWO ? 128 : 64) + (size_t)(BP_TILE + 8) * 2 +
+    const size_t smem = (size_t)2 * BP_TILE * 24 + (TWO ? 128 : 64) + (size_t)(BP_TILE + 8) * 2 + (size_t)BP_TILE * 2 +
                         (PRE ? (size_t)DP_STAGE * 24 : 0);   // (two calls: the outputs are stored straight from registers)
     static int per_sm[SV_MAX_DEV];
     return sv_launch_persistent(densepass_kernel<MA, PRE, TWO>, per_sm, smem, ntiles, st, kin, ain, kout, aout, p, tab, pend,
