@@ -175,8 +175,9 @@ int sv_load_device(sv_state *s, const uint64_t *dev_keys, const sv_c128 *dev_amp
 enum { SV_OPT_SAMPLE_MIN_TERMS = 0, SV_OPT_SMALL_STATE_PATH = 2,   /* 2: 1 (default) / 0: sv_apply_circuit may / may not use its single-block path */
        SV_OPT_TWO_BIT_PASS = 3 };   /* the final pass of a dense multi-qubit gate (every entry of U nonzero) brings its last TWO missing qubits to
                                      * the low bit positions at once -- one pass over the state less --: 0 never (one pass per missing qubit),
-                                     * 1 for every such gate, 2 (default) for gates on three or four mixing qubits applied through
-                                     * sv_apply_gate, where it is measured faster.  The result is the same bit for bit. */
+                                     * 1 for every such gate applied through sv_apply_gate, 2 (default) for those on three or four mixing
+                                     * qubits, where it is measured faster.  sv_apply_gate_truncate and sv_apply_circuit never use it.
+                                     * The result is the same bit for bit. */
 int sv_set_option(sv_state *s, int option, uint64_t value);
 
 /* Statistics of the last call and the launch counter. */

@@ -547,10 +547,9 @@ extern "C" int sv_apply_gate(sv_state* s, const int* qubits, int m, const sv_c12
     // itself (a four-way merge per tile, sv_dense.cu TWO): one full pass over the state less.
     bool dense0 = (ma >= 2 && mc == 0);
     for (int i = 0; i < d * d && dense0; ++i) dense0 = !is_zero(U[i]);
-    // (default: only for ma >= 3 and outside the fused call -- the fused variant of the two-bit pass, 2 resident blocks per SM,
-    // is measured 1 to 5 % slower than move + final pass, the two-call variant 2 % faster: profiles/r2_final.md)
-    const bool two = s->two_bit_min_ma != 0 && ma >= s->two_bit_min_ma && dense0 && nneed >= 2 &&
-                     (s->two_bit_min_ma == 2 || s->fuse_K == 0);
+    // (never inside the fused call: the fused variant of the two-bit pass, 2 resident blocks per SM, measured 1 to 5 % slower than
+    // move + final pass -- profiles/r2_final.md -- and is not built)
+    const bool two = s->two_bit_min_ma != 0 && ma >= s->two_bit_min_ma && dense0 && nneed >= 2 && s->fuse_K == 0;
     for (int t = 0; t + (two ? 2 : 1) < nneed; ++t) {   // pure moves: state preserving, committed one by one
         const int p = s->phys_of_log[qubits[need[t]]];
         if (p == 0) continue;

@@ -655,10 +655,8 @@ u32 svk_densepass_launch(int ma, bool use_pre, const u64* kin, const double2* ai
                          const PendPred& pend, TileDesc* desc, u64* status, u64* d_count, u64 cap, u32 ntiles, cudaStream_t st,
                          const PreCut* pre, double* pre_mass, u64* pre_cnt, int maybe_dead, int p2) {
 #define SV_DP(MA_, PRE_) launch_densepass<MA_, PRE_, true>(kin, ain, kout, aout, p, tab, pend, desc, status, d_count, cap, ntiles, st, pre, pre_mass, pre_cnt, maybe_dead, p2)
-    if (p2 >= 0) {   // two bits moved by this pass (desc: TileDesc2)
-        if (use_pre) {
-            switch (ma) { case 2: return SV_DP(2, true); case 3: return SV_DP(3, true); case 4: return SV_DP(4, true); default: return 0; }
-        }
+    if (p2 >= 0) {   // two bits moved by this pass (desc: the piece table of make_pieces2); two calls only (sv_api.cu)
+        if (use_pre) return 0;
         switch (ma) { case 2: return SV_DP(2, false); case 3: return SV_DP(3, false); case 4: return SV_DP(4, false); default: return 0; }
     }
 #undef SV_DP

@@ -136,8 +136,9 @@ def test_two_bit_pass_random_states(eng, n, count, seed):
 
 
 def test_two_bit_pass_with_pending_cut_and_fused_call(eng):
-    """A truncation is pending when the gate runs (dropped terms are squeezed out in the partition), and the fused
-    call leaves out what lies below its floor: both against the oracle, step-locked."""
+    """A truncation is pending when the gate runs (dropped terms are squeezed out in the partition); every third gate goes
+    through the fused call, which never uses the two-bit pass (sv_api.cu) and must leave the layout in a state the next
+    two-bit pass can start from: all against the oracle, step-locked."""
     rng = np.random.default_rng(6001)
     n = 40
     fb = [2, 5, 6, 9, 13, 17, 18, 22, 25, 29, 31, 33, 36, 38, 39]
