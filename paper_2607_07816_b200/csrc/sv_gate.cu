@@ -318,7 +318,7 @@ __device__ __forceinline__ void multi_lower_bound(const u64* __restrict__ keys, 
     }
 }
 
-__global__ void find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles,
+__global__ void __launch_bounds__(128, 8) find_splits2_kernel(const u64* __restrict__ keys, u64 n, int pH, int pL, int w, u32 tnom, u32 ntiles,
                                     TileDesc2* __restrict__ desc) {
     const u32 j = blockIdx.x * blockDim.x + threadIdx.x;
     TileDesc2 d;
