@@ -469,6 +469,7 @@ __global__ void __launch_bounds__(SV_THREADS, (PRE || MA > 3) ? 2 : DP_NOPRE_BLO
                     if (col_ident || nm <= 2) {          // members in stored order = ascending logical column (or the order cannot matter)
                         for (int j = 0; j < nm; ++j) {
                             const int x = (int)(sk[DK(e + j)] & AM);
+                            SV_CHK(si[e + j] < cnt);
                             const double2 a = La[si[e + j]];
 #pragma unroll
                             for (int r = 0; r < NP; ++r) {
